@@ -1,0 +1,198 @@
+/*
+ * mesh_attn.h -- C ABI of the B200-native per-GPU compute core of Mesh-Attention
+ * (arxiv 2512.20968).  "P:Lnnn" cites a line of the paper text.
+ *
+ * One B200 simulates the n logical GPUs of the paper.  Q and KV are split into n
+ * sequence partitions; simulated GPU g owns an a x b tile of the n x n
+ * assignment matrix and, for every (Q_u, KV_v) pair of that tile,
+ * computes blockwise softmax attention emitting a partial output and its log-sum-exp
+ * (Alg.2 l.3-5 P:L171-173).  A second step merges the partial outputs of each
+ * Q partition with the online-softmax (LSE-weighted) reducer.  Backward
+ * follows Alg.3.  The paper's collectives (all-gather, reduce-scatter) do
+ * not exist here: there is one GPU, no sharding and no inter-GPU exchange; the planner
+ * only builds the assignment matrix, the per-simulated-GPU tile lists and their order.
+ *
+ * Conventions
+ *   - All tensor pointers are DEVICE pointers (allocated by the caller, e.g. torch);
+ *     `stream` is a cudaStream_t passed as void*.  The *_host entry point is the only
+ *     one taking HOST pointers and says so.
+ *   - The caller owns every buffer, including workspaces whose size the plan reports.
+ *     The library owns only the plan object and its small device-resident work lists.
+ *   - Hot calls (tile_fwd, merge, bwd_preprocess, tile_bwd, forward, backward) never
+ *     allocate, never synchronise the host, never touch the default stream implicitly:
+ *     everything is enqueued on `stream`.
+ *   - Every function returns a mesh_attn_status (0 = OK, negative = error) and never
+ *     throws or aborts; mesh_attn_last_error() gives a thread-local detail string.
+ *   - There is no CPU fallback: on a machine without a CUDA device the planner calls
+ *     work, every compute call returns MESH_ATTN_ECUDA.
+ *
+ * Tensor layouts (rows in PARTITION-MAJOR order: partition p, local row s -> row p*L+s,
+ * L = seq_total / n):
+ *   Q, dO      bf16  [B, N, Hq,  D]   (tensor_layout 0)  or [B, Hq,  N, D] (tensor_layout 1)
+ *   K, V       bf16  [B, N, Hkv, D]                      or [B, Hkv, N, D]
+ *   O, dQ      fp32  same shape as Q;   dK, dV fp32 same shape as K
+ *   lse, delta fp32  [B, Hq, N]   natural log of the sum of exp of the SCALED scores
+ *   partial_O  fp32  [g_count][slots][B][L][Hq][D]   slots = a (partial_mode 0) or a*b (1)
+ *   partial_lse fp32 [g_count][slots][B][Hq][L]
+ * Token position of (p, s): seq_layout 0: p*L+s;  seq_layout 1 (striped): s*n+p.
+ * Causal: key visible iff pos(key) <= pos(query).  A row with no visible key
+ * gets O = 0, lse = -inf.  GQA: query head h reads KV head h / (Hq/Hkv).
+ */
+#ifndef MESH_ATTN_H
+#define MESH_ATTN_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct mesh_attn_plan mesh_attn_plan; /* opaque, library-owned, immutable after create */
+
+typedef enum {
+    MESH_ATTN_OK = 0,
+    MESH_ATTN_EINVAL = -1,       /* bad geometry / null pointer / out-of-range index      */
+    MESH_ATTN_EUNSUPPORTED = -2, /* valid but not built (e.g. head_dim not in {64,128})   */
+    MESH_ATTN_EWORKSPACE = -3,   /* caller-provided buffer too small for the query        */
+    MESH_ATTN_ECUDA = -4,        /* CUDA error or no CUDA device                           */
+    MESH_ATTN_ENOMEM = -5
+} mesh_attn_status;
+
+typedef struct {
+    int32_t n, a, b;          /* n == a*b; a = tile height = Q-group size, b = tile width = KV-group size */
+    int32_t batch, seq_total, heads_q, heads_kv, head_dim; /* L = seq_total/n, L % 128 == 0, head_dim in {64,128} */
+    int32_t causal;           /* 0 | 1                                                        */
+    int32_t kvr;              /* 1: KV partition rotation, I_g^KV = {c + t*a}; 0: contiguous */
+    int32_t seq_layout;       /* 0 contiguous (pos = p*L+s), 1 striped (pos = s*n+p)          */
+    int32_t order;            /* 0 row-major tile order, 1 greedy / GOO                   */
+    int32_t k_q, k_kv;        /* GOO chunk counts, k_q*k_kv <= 16; (L/k) % 128 == 0; <=0 -> 1 */
+    float gamma;              /* GOO safety factor, <=0 -> 1.05                               */
+    float t_ag_q, t_ag_kv, t_rs_q, t_c; /* GOO task costs; any <=0 -> built-in cost model      */
+    float softmax_scale;      /* <=0 -> 1/sqrt(head_dim)                                       */
+    int32_t tensor_layout;    /* 0: [B,N,H,D], 1: [B,H,N,D]                                            */
+    int32_t partial_mode;     /* 0: one partial per (g,u), fused over I_g^KV (Alg.2 l.5);
+                                 1: one partial per pair (u,v): literal O_ij, lse_ij           */
+    int32_t precision;        /* backward MMA operands P, dS: 0 single bf16, 1 split hi+lo bf16        */
+    int32_t reserved[5];      /* must be 0                                                             */
+} mesh_attn_plan_desc;
+
+/* what = ... for mesh_attn_plan_query */
+enum {
+    MESH_ATTN_Q_PARTIAL_O_BYTES = 0,   /* bytes of partial_O for ONE simulated GPU (multiply by g_count)  */
+    MESH_ATTN_Q_PARTIAL_LSE_BYTES = 1, /* bytes of partial_lse for ONE simulated GPU                      */
+    MESH_ATTN_Q_SLOTS_PER_GPU = 2,     /* a or a*b                                                        */
+    MESH_ATTN_Q_FLOPS_FWD = 3,         /* algorithmic: 4*D*Hq*B*visible pairs                             */
+    MESH_ATTN_Q_FLOPS_BWD = 4,         /* algorithmic: 10*D*Hq*B*visible pairs                            */
+    MESH_ATTN_Q_WAVES = 5,             /* number of Q groups = b                                          */
+    MESH_ATTN_Q_MERGE_BYTES = 6,       /* algorithmic bytes moved by ONE merge call (one Q group)         */
+    MESH_ATTN_Q_FWD_ITEMS_PER_GPU = 7, /* tile-forward work items per simulated GPU                       */
+    MESH_ATTN_Q_BWD_ITEMS_PER_GPU = 8, /* tile-backward work items per simulated GPU                      */
+    MESH_ATTN_Q_BLOCKS_FWD = 9,        /* 128x128 score blocks the forward computes (all GPUs, heads)     */
+    MESH_ATTN_Q_COMM_UNITS = 10,       /* paper's aggregate communication units of this AM   */
+    MESH_ATTN_Q_HAS_DEVICE = 11        /* 1 if the plan's work lists are resident on a CUDA device        */
+};
+
+/* kinds in mesh_attn_plan_steps rows (step, kind, i, j) */
+enum {
+    MESH_ATTN_TASK_AG_KV = 0,  /* all-gather KV chunk j (idx in column 2, column 3 = -1)   */
+    MESH_ATTN_TASK_AG_Q = 1,   /* all-gather Q chunk i; backward: Q,O,dO chunk i     */
+    MESH_ATTN_TASK_RS_Q = 2,   /* reduce-scatter O chunk i; backward: dQ chunk i     */
+    MESH_ATTN_TASK_C = 3,      /* compute task C-i-j                                       */
+    MESH_ATTN_TASK_RS_KV = 4   /* backward only: reduce-scatter dKV chunk j                */
+};
+
+/* ---- planner (host only; works without a GPU) ------------------------------------------- */
+
+/* Validates desc, builds the assignment matrix, Q/KV groups
+ * (P:L178-180), the GOO step list and the ordered tile lists; if a CUDA
+ * device is present also uploads the work lists (the only allocation the library makes).
+ * Errors: EINVAL (n != a*b, seq_total % n, L % 128, Hq % Hkv, k_q*k_kv > 16, ...),
+ * EUNSUPPORTED (head_dim), ENOMEM, ECUDA (upload failed). *out is NULL on error. */
+int mesh_attn_plan_create(const mesh_attn_plan_desc* desc, mesh_attn_plan** out);
+void mesh_attn_plan_destroy(mesh_attn_plan* plan);
+
+/* am: host int32 [n*n] row-major, am[i*n+j] = g computing (Q_i, KV_j). */
+int mesh_attn_plan_am(const mesh_attn_plan* plan, int32_t* am);
+
+/* Footprints of simulated GPU g: I^Q (a entries), I^KV (b entries) in
+ * execution order; host int32 arrays of capacity >= a and >= b. */
+int mesh_attn_plan_footprint(const mesh_attn_plan* plan, int32_t g, int32_t* iq, int32_t* ikv);
+
+/* Tile list of simulated GPU g in execution order: rows (u, v, i, j) = Q partition, KV
+ * partition, Q chunk, KV chunk; host int32 [capacity][4]; *count receives the number of
+ * rows (= a*b*k_q*k_kv); if capacity is too small returns EWORKSPACE with *count set. */
+int mesh_attn_plan_tiles(const mesh_attn_plan* plan, int32_t g, int32_t* tiles, int32_t capacity, int32_t* count);
+
+/* GOO step list (same on every simulated GPU): rows (step, kind, i, j), host
+ * int32 [capacity][4]. pass: 0 forward, 1 backward (backward: DESIGN.md reading R12,
+ * parity unpinned). With order == 0 there is a single step holding every task. */
+int mesh_attn_plan_steps(const mesh_attn_plan* plan, int32_t pass, int32_t* steps, int32_t capacity, int32_t* count);
+
+int mesh_attn_plan_query(const mesh_attn_plan* plan, int32_t what, int64_t* value);
+
+/* ---- hot path (device pointers; enqueued on stream) -------------------------------------- */
+
+/* Alg.2 l.3-5 for simulated GPUs g_first .. g_first+g_count-1: for each Q_u
+ * (u in I_g^Q) the online-softmax attention over the KV partitions of I_g^KV in plan
+ * order; writes the normalised partial output and its LSE into slot (g - g_first, u_local)
+ * (partial_mode 1: slot (g - g_first, u_local*b + v_local), one KV partition each). */
+int mesh_attn_tile_fwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_count,
+                       const void* Q, const void* K, const void* V,
+                       float* partial_O, float* partial_lse, void* stream);
+
+/* Online-softmax reducer of Alg.2 l.6 as a local merge: for every Q partition
+ * u of Q group q_group (u = q_group*a + x), every row and head:
+ *   lse* = ln sum_k exp(lse_k),  O = sum_k exp(lse_k - lse*) O_k   over the slots holding u.
+ * partial_O / partial_lse are the buffers tile_fwd filled for g_first = q_group*a,
+ * g_count = a.  Writes rows of partitions u of O [B,N,Hq,D] and lse [B,Hq,N]. */
+int mesh_attn_merge(const mesh_attn_plan* plan, int32_t q_group,
+                    const float* partial_O, const float* partial_lse,
+                    float* O, float* lse, void* stream);
+
+/* delta[b,h,row] = sum_d dO * O  (needed by every pair touching the row; the paper
+ * passes O_i, dO_i to the backward kernel). All rows. */
+int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const float* O, const void* dO,
+                             float* delta, void* stream);
+
+/* Alg.3 l.3-5 for simulated GPUs g_first..: for each pair of the tile
+ * recompute P = exp(S - lse) with the FINAL merged lse, dP = dO V^T, dS = P o (dP - delta),
+ * and ACCUMULATE (atomic fp32 adds: the sums of Alg.3 l.6-7 and the GQA group sum)
+ *   dV_v += P^T dO_u,  dK_v += scale dS^T Q_u,  dQ_u += scale dS K_v.
+ * The caller zeroes dQ, dK, dV before the first call. */
+int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_count,
+                       const void* Q, const void* K, const void* V, const void* dO,
+                       const float* lse, const float* delta,
+                       float* dQ, float* dK, float* dV, void* stream);
+
+/* All waves: for each Q group r: tile_fwd(g_first = r*a, a) then merge(r). partial_O /
+ * partial_lse must hold `a` simulated GPUs (query PARTIAL_*_BYTES * a). */
+int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
+                      float* O, float* lse, float* partial_O, float* partial_lse, void* stream);
+
+/* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
+int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
+                       const float* O, const void* dO, const float* lse, float* delta,
+                       float* dQ, float* dK, float* dV, void* stream);
+
+/* End-to-end step with HOST buffers (pinned or pageable): copies Q,K,V(,dO) host->device
+ * into the caller's device staging buffers, runs forward (and backward if dO_host != NULL),
+ * copies O, lse (and dQ,dK,dV) device->host; all on `stream`, which is synchronised before
+ * returning.  d_* are caller-owned DEVICE buffers of the shapes above. */
+typedef struct {
+    const void *Q_host, *K_host, *V_host, *dO_host;      /* bf16 host inputs (dO_host may be NULL) */
+    float *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* fp32 host outputs (any may be NULL = not copied back) */
+    void *d_Q, *d_K, *d_V, *d_dO;                          /* device staging                         */
+    float *d_O, *d_lse, *d_delta, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;
+} mesh_attn_host_io;
+int mesh_attn_step_host(const mesh_attn_plan* plan, const mesh_attn_host_io* io, void* stream);
+
+/* number of kernels launched by this library in the calling process so far (bench bookkeeping) */
+int64_t mesh_attn_launch_count(void);
+
+const char* mesh_attn_strerror(int status);
+const char* mesh_attn_last_error(void); /* thread-local, valid until the next call on this thread */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MESH_ATTN_H */

@@ -1,0 +1,160 @@
+// aux_kernels.cu -- the two HBM-bound kernels of the hot path:
+//   merge_kernel   LSE-weighted merge of the partial outputs of a Q group (online-softmax
+//                  reducer of PAPER.md L77, Alg.2 l.6 L174; reading R4)
+//   delta_kernel   backward preprocess Delta = rowsum(dO o O)
+// Both are streaming kernels: 16-byte vector loads, many independent loads in flight per
+// thread, streaming cache hints, no shared-memory reuse of the bulk data.
+#include <cuda_bf16.h>
+
+#include "tile_kernels.hpp"
+
+namespace mesh_attn {
+namespace {
+
+__device__ __forceinline__ float4 ld_stream(const float4* p)
+{
+    float4 v;
+    asm volatile("ld.global.nc.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+}
+__device__ __forceinline__ void st_stream(float4* p, const float4& v)
+{
+    asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+constexpr int kMergeThreads = 256;
+constexpr int kMergeUnroll = 8;
+
+// grid: (L / rows_per_block, a, B).  One block merges rows_per_block rows x all Hq heads of one
+// Q partition.  Phase 1: one thread per (row, head) turns the m LSE values into weights
+// w_k = exp(lse_k - lse*) (smem) and writes lse*.  Phase 2: every thread streams float4 columns:
+// out = sum_k w_k * partial_k.
+template <int D>
+__global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams p)
+{
+    extern __shared__ float w_smem[];            // [rows][Hq][m]
+    const Geom& gm = p.gm;
+    const int rows = p.rows_per_block, m = p.m, Hq = gm.heads_q;
+    const int s0 = blockIdx.x * rows, ul = blockIdx.y, bt = blockIdx.z;
+    const int u = p.q_group * gm.a + ul;
+    const size_t unit_lse = (size_t)gm.batch * Hq * gm.L;          // one slot of partial_lse
+    const size_t unit_o = unit_lse * D;                             // one slot of partial_O
+
+    for (int idx = threadIdx.x; idx < rows * Hq; idx += kMergeThreads) {
+        const int r = idx % rows, h = idx / rows;                  // consecutive threads -> consecutive rows (coalesced lse)
+        float mx = -INFINITY;
+        for (int k = 0; k < m; ++k) {
+            const size_t slot = (size_t)(k / p.per) * gm.slots_per_gpu + (size_t)ul * p.per + (k % p.per);
+            const float x = p.partial_lse[slot * unit_lse + ((size_t)bt * Hq + h) * gm.L + s0 + r];
+            w_smem[(r * Hq + h) * m + k] = x;
+            mx = fmaxf(mx, x);
+        }
+        float sum = 0.f;
+        for (int k = 0; k < m; ++k) {
+            const float x = w_smem[(r * Hq + h) * m + k];
+            sum += (x == -INFINITY) ? 0.f : __expf(x - mx);
+        }
+        const float lse = (mx == -INFINITY) ? -INFINITY : mx + __logf(sum);
+        for (int k = 0; k < m; ++k) {
+            const float x = w_smem[(r * Hq + h) * m + k];
+            w_smem[(r * Hq + h) * m + k] = (x == -INFINITY) ? 0.f : __expf(x - lse);
+        }
+        p.lse[((size_t)bt * Hq + h) * ((size_t)gm.n * gm.L) + (size_t)u * gm.L + s0 + r] = lse;
+    }
+    __syncthreads();
+
+    constexpr int V = D / 4;                                        // float4 per (row, head)
+    const int total = rows * Hq * V;
+    const float4* src = reinterpret_cast<const float4*>(p.partial_O) + ((size_t)bt * gm.L + s0) * Hq * V;
+    for (int i = threadIdx.x; i < total; i += kMergeThreads) {
+        const int rh = i / V, d4 = i - rh * V;                     // rh = r*Hq + h : contiguous in the partial buffers
+        const float* w = w_smem + rh * m;
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int k0 = 0; k0 < m; k0 += kMergeUnroll) {
+            float4 x[kMergeUnroll];
+#pragma unroll
+            for (int kk = 0; kk < kMergeUnroll; ++kk) {
+                const int k = k0 + kk;
+                if (k < m) {
+                    const size_t slot = (size_t)(k / p.per) * gm.slots_per_gpu + (size_t)ul * p.per + (k % p.per);
+                    x[kk] = ld_stream(src + slot * (unit_o / 4) + i);
+                }
+            }
+#pragma unroll
+            for (int kk = 0; kk < kMergeUnroll; ++kk) {
+                const int k = k0 + kk;
+                if (k < m) {
+                    const float wk = w[k];
+                    acc.x = fmaf(wk, x[kk].x, acc.x); acc.y = fmaf(wk, x[kk].y, acc.y);
+                    acc.z = fmaf(wk, x[kk].z, acc.z); acc.w = fmaf(wk, x[kk].w, acc.w);
+                }
+            }
+        }
+        const int r = rh / Hq, h = rh - r * Hq;
+        float* dst = p.O + (size_t)bt * p.o_stride_b + ((size_t)u * gm.L + s0 + r) * p.o_stride_row + (size_t)h * p.o_stride_h + d4 * 4;
+        st_stream(reinterpret_cast<float4*>(dst), acc);
+    }
+}
+
+// one warp per (batch, row, head): delta = sum_d dO * O
+template <int D>
+__global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
+{
+    const Geom& gm = p.gm;
+    const long long N = (long long)gm.n * gm.L;
+    const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (wid >= (long long)gm.batch * N * gm.heads_q) return;
+    const int h = (int)(wid % gm.heads_q);
+    const long long row = (wid / gm.heads_q) % N;
+    const int bt = (int)(wid / ((long long)gm.heads_q * N));
+    const size_t base = (size_t)bt * p.stride_b + (size_t)row * p.stride_row + (size_t)h * p.stride_h;
+    const __nv_bfloat16* dO = reinterpret_cast<const __nv_bfloat16*>(p.dO) + base;
+    const float* O = p.O + base;
+    float acc = 0.f;
+    if (D == 128) {
+        const float4 o = *reinterpret_cast<const float4*>(O + lane * 4);
+        const uint2 g = *reinterpret_cast<const uint2*>(dO + lane * 4);
+        const __nv_bfloat162 g0 = *reinterpret_cast<const __nv_bfloat162*>(&g.x), g1 = *reinterpret_cast<const __nv_bfloat162*>(&g.y);
+        acc = o.x * __low2float(g0) + o.y * __high2float(g0) + o.z * __low2float(g1) + o.w * __high2float(g1);
+    } else {
+        const float2 o = *reinterpret_cast<const float2*>(O + lane * 2);
+        const __nv_bfloat162 g = *reinterpret_cast<const __nv_bfloat162*>(dO + lane * 2);
+        acc = o.x * __low2float(g) + o.y * __high2float(g);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) p.delta[((size_t)bt * gm.heads_q + h) * N + row] = acc;
+}
+
+}  // namespace
+
+int launch_merge(const MergeParams& p, cudaStream_t stream)
+{
+    const Geom& gm = p.gm;
+    const size_t smem = (size_t)p.rows_per_block * gm.heads_q * p.m * sizeof(float);
+    dim3 grid(gm.L / p.rows_per_block, gm.a, gm.batch);
+    cudaError_t e;
+    if (gm.head_dim == 128) {
+        e = cudaFuncSetAttribute(merge_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        merge_kernel<128><<<grid, kMergeThreads, smem, stream>>>(p);
+    } else {
+        e = cudaFuncSetAttribute(merge_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return (int)e;
+        merge_kernel<64><<<grid, kMergeThreads, smem, stream>>>(p);
+    }
+    return (int)cudaGetLastError();
+}
+
+int launch_delta(const DeltaParams& p, cudaStream_t stream)
+{
+    const Geom& gm = p.gm;
+    const long long warps = (long long)gm.batch * gm.n * gm.L * gm.heads_q;
+    const unsigned grid = (unsigned)((warps + 7) / 8);
+    if (gm.head_dim == 128) delta_kernel<128><<<grid, 256, 0, stream>>>(p);
+    else delta_kernel<64><<<grid, 256, 0, stream>>>(p);
+    return (int)cudaGetLastError();
+}
+
+}  // namespace mesh_attn

@@ -1,0 +1,285 @@
+// capi.cu -- C-ABI entry points of libmesh_attn.so (include/mesh_attn.h): argument checking,
+// TMA tensor-map construction, kernel launches.  No allocation and no host synchronisation in
+// the hot calls; every launch goes to the caller's stream.
+#include <atomic>
+#include <cstdio>
+#include <cstring>
+#include <string>
+
+#include "plan.hpp"
+#include "tile_kernels.hpp"
+#include "tmap.hpp"
+
+using namespace mesh_attn;
+
+namespace {
+thread_local std::string g_last_error;
+std::atomic<long long> g_launches{0};
+
+int fail(int code, const std::string& msg)
+{
+    g_last_error = msg;
+    return code;
+}
+int cuda_fail(const char* what, int err)
+{
+    g_last_error = std::string(what) + ": " + cudaGetErrorString((cudaError_t)err);
+    return MESH_ATTN_ECUDA;
+}
+
+struct Strides { long long b, row, h; };   // element strides of a [B,N,H,D] / [B,H,N,D] tensor
+Strides strides_of(const mesh_attn_plan* p, int H)
+{
+    const long long N = (long long)p->geom.n * p->geom.L, D = p->geom.head_dim;
+    if (p->desc.tensor_layout == 0) return {N * H * D, (long long)H * D, D};
+    return {N * H * D, D, N * D};
+}
+
+bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H)
+{
+    const Strides s = strides_of(p, H);
+    const uint64_t N = (uint64_t)p->geom.n * p->geom.L;
+    return make_tmap_bf16_4d(m, base, p->geom.head_dim, H, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, kBlock);
+}
+
+int check_device(const mesh_attn_plan* p, const char* who)
+{
+    if (!p) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null plan");
+    if (!p->d_blob) return fail(MESH_ATTN_ECUDA, std::string(who) + ": plan has no device work lists (no CUDA device at plan_create); there is no CPU fallback");
+    return MESH_ATTN_OK;
+}
+}  // namespace
+
+namespace mesh_attn {
+void set_error(const std::string& msg) { g_last_error = msg; }
+
+int upload_plan(mesh_attn_plan* p)
+{
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev == 0) {
+        (void)cudaGetLastError();
+        return MESH_ATTN_OK;   // host-only plan: planner queries work, compute calls return ECUDA
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return cuda_fail("cudaGetDevice", (int)cudaGetLastError());
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return cuda_fail("cudaGetDeviceProperties", (int)cudaGetLastError());
+    if (prop.major != 10) return fail(MESH_ATTN_EUNSUPPORTED, "plan_create: kernels are built for sm_100a (B200) only");
+    p->device = dev;
+    p->num_sms = prop.multiProcessorCount;
+    auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
+    const size_t b0 = al(p->fwd_items.size() * sizeof(FwdItem)), b1 = al(p->bwd_items.size() * sizeof(BwdItem)),
+                 b2 = al(p->fwd_segs.size() * sizeof(Seg)), b3 = al(p->bwd_segs.size() * sizeof(Seg)),
+                 b4 = al(p->fwd_seglists.size() * sizeof(SegList)), b5 = al(p->bwd_seglists.size() * sizeof(SegList));
+    char* d = nullptr;
+    cudaError_t e = cudaMalloc(&d, b0 + b1 + b2 + b3 + b4 + b5 + 256);
+    if (e != cudaSuccess) return cuda_fail("cudaMalloc(work lists)", (int)e);
+    p->d_blob = d;
+    auto put = [&](const void* src, size_t bytes, size_t cap) {
+        char* at = d;
+        if (bytes) e = cudaMemcpy(at, src, bytes, cudaMemcpyHostToDevice);
+        d += cap;
+        return at;
+    };
+    p->d_fwd_items = (const FwdItem*)put(p->fwd_items.data(), p->fwd_items.size() * sizeof(FwdItem), b0);
+    p->d_bwd_items = (const BwdItem*)put(p->bwd_items.data(), p->bwd_items.size() * sizeof(BwdItem), b1);
+    p->d_fwd_segs = (const Seg*)put(p->fwd_segs.data(), p->fwd_segs.size() * sizeof(Seg), b2);
+    p->d_bwd_segs = (const Seg*)put(p->bwd_segs.data(), p->bwd_segs.size() * sizeof(Seg), b3);
+    p->d_fwd_seglists = (const SegList*)put(p->fwd_seglists.data(), p->fwd_seglists.size() * sizeof(SegList), b4);
+    p->d_bwd_seglists = (const SegList*)put(p->bwd_seglists.data(), p->bwd_seglists.size() * sizeof(SegList), b5);
+    if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
+    return MESH_ATTN_OK;
+}
+
+void free_plan_device(mesh_attn_plan* p)
+{
+    if (p->d_blob) cudaFree(p->d_blob);
+    p->d_blob = nullptr;
+}
+}  // namespace mesh_attn
+
+extern "C" {
+
+int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
+                       float* partial_O, float* partial_lse, void* stream)
+{
+    if (int rc = check_device(p, "tile_fwd")) return rc;
+    if (!Q || !K || !V || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, "tile_fwd: null pointer");
+    if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_fwd: simulated GPU range out of bounds");
+    if ((long long)g_count * (long long)p->fwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_fwd: too many work items in one call");
+    CUtensorMap tmQ, tmK, tmV;
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv))
+        return fail(MESH_ATTN_ECUDA, "tile_fwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
+    FwdParams fp;
+    fp.gm = p->geom;
+    fp.items = p->d_fwd_items;
+    fp.segs = p->d_fwd_segs;
+    fp.seglists = p->d_fwd_seglists;
+    fp.items_per_gpu = (int)p->fwd_items.size();
+    fp.g_first = g_first;
+    fp.g_count = g_count;
+    fp.partial_O = partial_O;
+    fp.partial_lse = partial_lse;
+    const int e = launch_tile_fwd(fp, tmQ, tmK, tmV, p->num_sms, (cudaStream_t)stream);
+    if (e) return cuda_fail("tile_fwd launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, float* O, float* lse,
+                    void* stream)
+{
+    if (int rc = check_device(p, "merge")) return rc;
+    if (!partial_O || !partial_lse || !O || !lse) return fail(MESH_ATTN_EINVAL, "merge: null pointer");
+    if (q_group < 0 || q_group >= p->geom.b) return fail(MESH_ATTN_EINVAL, "merge: q_group out of range (there are b Q groups, PAPER.md L178)");
+    MergeParams mp;
+    mp.gm = p->geom;
+    mp.q_group = q_group;
+    mp.per = p->desc.partial_mode == 1 ? p->geom.b : 1;
+    mp.m = p->geom.a * mp.per;
+    int rows = 8;
+    while (rows > 1 && ((size_t)rows * p->geom.heads_q * mp.m * 4 > 64 * 1024 || p->geom.L % rows)) rows >>= 1;
+    if ((size_t)rows * p->geom.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, "merge: heads_q * partial count too large");
+    mp.rows_per_block = rows;
+    mp.partial_O = partial_O;
+    mp.partial_lse = partial_lse;
+    mp.O = O;
+    mp.lse = lse;
+    const Strides s = strides_of(p, p->geom.heads_q);
+    mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
+    const int e = launch_merge(mp, (cudaStream_t)stream);
+    if (e) return cuda_fail("merge launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void* dO, float* delta, void* stream)
+{
+    if (int rc = check_device(p, "bwd_preprocess")) return rc;
+    if (!O || !dO || !delta) return fail(MESH_ATTN_EINVAL, "bwd_preprocess: null pointer");
+    DeltaParams dp;
+    dp.gm = p->geom;
+    dp.O = O; dp.dO = dO; dp.delta = delta;
+    const Strides s = strides_of(p, p->geom.heads_q);
+    dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
+    const int e = launch_delta(dp, (cudaStream_t)stream);
+    if (e) return cuda_fail("bwd_preprocess launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
+                       const void* dO, const float* lse, const float* delta, float* dQ, float* dK, float* dV, void* stream)
+{
+    if (int rc = check_device(p, "tile_bwd")) return rc;
+    if (!Q || !K || !V || !dO || !lse || !delta || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
+    if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds");
+    if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
+    CUtensorMap tmQ, tmK, tmV, tmdO;
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv) ||
+        !make_map(p, &tmdO, dO, p->geom.heads_q))
+        return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
+    BwdParams bp;
+    bp.gm = p->geom;
+    bp.items = p->d_bwd_items;
+    bp.segs = p->d_bwd_segs;
+    bp.seglists = p->d_bwd_seglists;
+    bp.items_per_gpu = (int)p->bwd_items.size();
+    bp.g_first = g_first;
+    bp.g_count = g_count;
+    bp.split = p->desc.precision;
+    bp.lse = lse; bp.delta = delta;
+    bp.dQ = dQ; bp.dK = dK; bp.dV = dV;
+    const Strides sq = strides_of(p, p->geom.heads_q), sk = strides_of(p, p->geom.heads_kv);
+    bp.q_stride_b = sq.b; bp.q_stride_row = sq.row; bp.q_stride_h = sq.h;
+    bp.k_stride_b = sk.b; bp.k_stride_row = sk.row; bp.k_stride_h = sk.h;
+    const int e = launch_tile_bwd(bp, tmQ, tmK, tmV, tmdO, p->num_sms, (cudaStream_t)stream);
+    if (e) return cuda_fail("tile_bwd launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, float* O, float* lse, float* partial_O,
+                      float* partial_lse, void* stream)
+{
+    if (int rc = check_device(p, "forward")) return rc;
+    for (int r = 0; r < p->geom.b; ++r) {   // one wave per Q group
+        if (int rc = mesh_attn_tile_fwd(p, r * p->geom.a, p->geom.a, Q, K, V, partial_O, partial_lse, stream)) return rc;
+        if (int rc = mesh_attn_merge(p, r, partial_O, partial_lse, O, lse, stream)) return rc;
+    }
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const float* O, const void* dO,
+                       const float* lse, float* delta, float* dQ, float* dK, float* dV, void* stream)
+{
+    if (int rc = check_device(p, "backward")) return rc;
+    if (!dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward: null pointer");
+    const Geom& gm = p->geom;
+    const size_t N = (size_t)gm.n * gm.L;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemsetAsync(dQ, 0, (size_t)gm.batch * N * gm.heads_q * gm.head_dim * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dK, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dV, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
+    if (e != cudaSuccess) return cuda_fail("backward memset", (int)e);
+    if (int rc = mesh_attn_bwd_preprocess(p, O, dO, delta, stream)) return rc;
+    // keep each launch's work-item count below 2^31: one call per Q group
+    for (int r = 0; r < gm.b; ++r)
+        if (int rc = mesh_attn_tile_bwd(p, r * gm.a, gm.a, Q, K, V, dO, lse, delta, dQ, dK, dV, stream)) return rc;
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, void* stream)
+{
+    if (int rc = check_device(p, "step_host")) return rc;
+    if (!io || !io->Q_host || !io->K_host || !io->V_host || !io->d_Q || !io->d_K || !io->d_V || !io->d_O || !io->d_lse || !io->d_partial_O ||
+        !io->d_partial_lse)
+        return fail(MESH_ATTN_EINVAL, "step_host: null pointer");
+    const Geom& gm = p->geom;
+    const size_t N = (size_t)gm.n * gm.L;
+    const size_t nq = (size_t)gm.batch * N * gm.heads_q * gm.head_dim, nk = (size_t)gm.batch * N * gm.heads_kv * gm.head_dim;
+    const size_t nl = (size_t)gm.batch * N * gm.heads_q;
+    cudaStream_t st = (cudaStream_t)stream;
+    cudaError_t e = cudaMemcpyAsync(io->d_Q, io->Q_host, nq * 2, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, st);
+    if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, st);
+    const bool bwd = io->dO_host != nullptr;
+    if (bwd) {
+        if (!io->d_dO || !io->d_delta || !io->d_dQ || !io->d_dK || !io->d_dV) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
+        if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_dO, io->dO_host, nq * 2, cudaMemcpyHostToDevice, st);
+    }
+    if (e != cudaSuccess) return cuda_fail("step_host H2D", (int)e);
+    if (int rc = mesh_attn_forward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_lse, io->d_partial_O, io->d_partial_lse, stream)) return rc;
+    if (bwd)
+        if (int rc = mesh_attn_backward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_dO, io->d_lse, io->d_delta, io->d_dQ, io->d_dK, io->d_dV, stream))
+            return rc;
+    if (io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * 4, cudaMemcpyDeviceToHost, st);
+    if (e == cudaSuccess && io->lse_host) e = cudaMemcpyAsync(io->lse_host, io->d_lse, nl * 4, cudaMemcpyDeviceToHost, st);
+    if (bwd) {
+        if (e == cudaSuccess && io->dQ_host) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * 4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * 4, cudaMemcpyDeviceToHost, st);
+    }
+    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    if (e != cudaSuccess) return cuda_fail("step_host D2H", (int)e);
+    return MESH_ATTN_OK;
+}
+
+int64_t mesh_attn_launch_count(void) { return (int64_t)g_launches.load(); }
+
+const char* mesh_attn_strerror(int status)
+{
+    switch (status) {
+        case MESH_ATTN_OK: return "ok";
+        case MESH_ATTN_EINVAL: return "invalid argument";
+        case MESH_ATTN_EUNSUPPORTED: return "unsupported configuration";
+        case MESH_ATTN_EWORKSPACE: return "caller buffer too small";
+        case MESH_ATTN_ECUDA: return "CUDA error / no CUDA device";
+        case MESH_ATTN_ENOMEM: return "out of memory";
+        default: return "unknown status";
+    }
+}
+
+const char* mesh_attn_last_error(void) { return g_last_error.c_str(); }
+
+}  // extern "C"

@@ -1,0 +1,360 @@
+// tile_fwd.cu -- mesh_attn_tile_fwd: blockwise softmax attention of a simulated GPU's tile
+// (Alg.2 l.3-5, L171-173; per-pair form O_ij, lse_ij = Attention(Q_i, K_j, V_j), L81-84).
+//
+// One persistent CTA per SM walks the work list.  A work item is up to two 128-row Q
+// sub-tiles of one (simulated GPU g, Q partition u, head); the CTA streams the KV blocks
+// (128 keys) of the item's segment list in plan order and keeps the online softmax
+// (running max m, running sum l) in registers, one query row per thread:
+//
+//   warp 0      TMA producer: Q sub-tiles once per item, K/V blocks through a smem ring
+//   warp 1      MMA issuer (one thread): S_t = Q_t K^T and O_t += P_t V with tcgen05.mma,
+//               accumulators in TMEM (S_0,S_1: columns 0..255; O_0,O_1: columns 256..511)
+//   warp 2      TMEM allocator
+//   warps 4-7   softmax of sub-tile 0: tcgen05.ld S row -> mask (diagonal blocks only) ->
+//   warps 8-11  softmax of sub-tile 1:   exp2 -> P (bf16) back into TMEM over S -> rescale O
+//
+// The two sub-tiles ping-pong: while the tensor core runs PV/QK for one sub-tile the other
+// sub-tile's softmax runs on the CUDA cores.  P is consumed by the PV MMA straight from
+// TMEM (A operand), V is the MN-major B operand, so neither is re-staged through smem.
+#include <cuda_bf16.h>
+
+#include "plan.hpp"
+#include "sm100.cuh"
+#include "tile_kernels.hpp"
+
+namespace mesh_attn {
+using namespace sm100;
+
+namespace {
+
+constexpr int kThreads = 384;
+constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
+
+template <int D> struct FwdCfg {
+    static constexpr int kBoxes = D / 64;                  // 64-element (128-byte) TMA boxes per row
+    static constexpr int kTileBytes = kBlock * D * 2;      // one [128 x D] bf16 tile
+    static constexpr int kStages = D == 128 ? 5 : 8;       // K/V ring slots (each one tile)
+    static constexpr int kSmemQ = 2 * kTileBytes;
+    static constexpr int kSmemRing = kStages * kTileBytes;
+    static constexpr int kNumBars = 2 + 2 * kStages + 6;
+    static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 1024;   // + alignment slack
+    static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
+};
+
+// Walks the 128-key KV blocks of a work item in plan order; every role runs the same walk.
+struct KvWalk {
+    const Geom& gm;
+    const Seg* segs;
+    int nseg, g, u, q_last;   // q_last = last local query row of the item
+    int si = -1, t = 0, t_hi = 0, v = 0, off = 0;
+    __device__ KvWalk(const Geom& gm_, const Seg* segs_, int nseg_, int g_, int u_, int q_last_)
+        : gm(gm_), segs(segs_), nseg(nseg_), g(g_), u(u_), q_last(q_last_) {}
+    // next block: KV partition v, first local key row t0, causal offset off (key t visible to row s iff t <= s + off)
+    __device__ bool next(int& v_out, int& t0_out, int& off_out)
+    {
+        while (true) {
+            if (si >= 0 && t < t_hi) { v_out = v; t0_out = t; off_out = off; t += kBlock; return true; }
+            if (++si >= nseg) return false;
+            const Seg sg = segs[si];
+            v = kv_partition(gm, g, sg.part_local);
+            t = sg.begin;
+            t_hi = sg.end;
+            off = 0x20000000;
+            if (gm.causal) {
+                off = causal_off(gm, u, v);
+                const int lim = q_last + off;                 // last visible key row for the item's last query row
+                t_hi = lim < sg.begin ? sg.begin : min(sg.end, (lim / kBlock + 1) * kBlock);
+            }
+        }
+    }
+    __device__ int count()
+    {
+        int n = 0, a, b, c;
+        while (next(a, b, c)) ++n;
+        return n;
+    }
+};
+
+struct ItemCtx {
+    FwdItem it;
+    int g_local, g, u, nt, nseg;
+    const Seg* segs;
+};
+
+__device__ __forceinline__ ItemCtx load_item(const FwdParams& p, int idx)
+{
+    ItemCtx c;
+    c.g_local = idx / p.items_per_gpu;
+    c.it = p.items[idx - c.g_local * p.items_per_gpu];
+    c.g = p.g_first + c.g_local;
+    c.u = (c.g / p.gm.a) * p.gm.a + c.it.u_local;
+    c.nt = c.it.nrows / kBlock;
+    const SegList sl = p.seglists[c.it.seglist];
+    c.segs = p.segs + sl.offset;
+    c.nseg = sl.count;
+    return c;
+}
+
+template <int D>
+__global__ void __launch_bounds__(kThreads, 1)
+tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
+                const __grid_constant__ CUtensorMap tmV, const FwdParams p)
+{
+    using Cfg = FwdCfg<D>;
+    extern __shared__ uint8_t smem_raw[];
+    uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+    uint8_t* sQ = smem;
+    uint8_t* sRing = smem + Cfg::kSmemQ;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(sRing + Cfg::kSmemRing);
+    uint64_t* q_full = bars + 0;
+    uint64_t* q_empty = bars + 1;
+    uint64_t* kv_full = bars + 2;
+    uint64_t* kv_empty = kv_full + Cfg::kStages;
+    uint64_t* s_full = kv_empty + Cfg::kStages;   // [2]
+    uint64_t* p_full = s_full + 2;                // [2]
+    uint64_t* o_full = p_full + 2;                // [2]
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_full + 2);
+
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const Geom& gm = p.gm;
+    const int total_items = p.items_per_gpu * p.g_count;
+
+    if (warp == kLoaderWarp && lane == 0) {
+        prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        mbar_init(q_full, 1);
+        mbar_init(q_empty, 1);
+        for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
+        for (int t = 0; t < 2; ++t) { mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kBlock); mbar_init(&o_full[t], 1); }
+        fence_mbar_init();
+    }
+    if (warp == kAllocWarp) tmem_alloc<512>(tmem_slot);
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tmem_slot;
+
+    if (warp == kLoaderWarp) {
+        // =============================== TMA producer ===============================
+        if (lane == 0) {
+            uint32_t stage = 0, ring_phase = 0, q_phase = 0;
+            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+                const ItemCtx c = load_item(p, idx);
+                KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
+                int v, t0, off;
+                bool first = true;
+                while (walk.next(v, t0, off)) {
+                    if (first) {
+                        first = false;
+                        mbar_wait(q_empty, q_phase ^ 1);
+                        q_phase ^= 1;
+                        mbar_expect_tx(q_full, c.nt * Cfg::kTileBytes);
+                        for (int t = 0; t < c.nt; ++t)
+                            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+                                tma_load_4d(sQ + t * Cfg::kTileBytes + bx * (kBlock * 128), &tmQ, q_full, bx * 64, c.it.head,
+                                            c.u * gm.L + c.it.q0 + t * kBlock, c.it.batch, kEvictFirst);
+                    }
+                    const int hk = c.it.head / gm.group;
+                    for (int kv = 0; kv < 2; ++kv) {       // K block then V block through the ring
+                        mbar_wait(&kv_empty[stage], ring_phase ^ 1);
+                        mbar_expect_tx(&kv_full[stage], Cfg::kTileBytes);
+                        for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+                            tma_load_4d(sRing + stage * Cfg::kTileBytes + bx * (kBlock * 128), kv == 0 ? &tmK : &tmV, &kv_full[stage],
+                                        bx * 64, hk, v * gm.L + t0, c.it.batch, kEvictLast);
+                        if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
+                    }
+                }
+            }
+        }
+    } else if (warp == kMmaWarp) {
+        // =============================== MMA issuer ===============================
+        if (lane == 0) {
+            constexpr uint32_t idesc_qk = umma_idesc(kBlock, kBlock, false, false);
+            constexpr uint32_t idesc_pv = umma_idesc(kBlock, D, false, true);
+            uint32_t stage = 0, ring_phase = 0, q_phase = 0, p_phase[2] = {0, 0};
+            auto ring_wait = [&](uint32_t& slot) {
+                mbar_wait(&kv_full[stage], ring_phase);
+                slot = stage;
+                if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
+            };
+            auto issue_qk = [&](int t, uint32_t kslot) {
+                const uint32_t qa = smem_u32(sQ + t * Cfg::kTileBytes), ka = smem_u32(sRing + kslot * Cfg::kTileBytes);
+#pragma unroll
+                for (int kk = 0; kk < D / 16; ++kk) {
+                    const uint32_t o = (kk / 4) * (kBlock * 128) + (kk % 4) * 32;
+                    umma_ss(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc_qk, kk > 0);
+                }
+            };
+            auto issue_pv = [&](int t, uint32_t vslot, bool acc) {
+                const uint32_t va = smem_u32(sRing + vslot * Cfg::kTileBytes);
+#pragma unroll
+                for (int kk = 0; kk < kBlock / 16; ++kk)
+                    umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + kk * 8,
+                            umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || kk > 0) ? 1u : 0u);
+            };
+            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+                const ItemCtx c = load_item(p, idx);
+                KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
+                const int nb = walk.count();
+                if (nb == 0) continue;
+                mbar_wait(q_full, q_phase);
+                q_phase ^= 1;
+                uint32_t kslot, vslot;
+                ring_wait(kslot);
+                tc_fence_after();
+                for (int t = 0; t < c.nt; ++t) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
+                umma_commit(&kv_empty[kslot]);
+                for (int j = 0; j < nb; ++j) {
+                    const bool more = j + 1 < nb;
+                    ring_wait(vslot);
+                    if (more) ring_wait(kslot);
+                    for (int t = 0; t < c.nt; ++t) {
+                        mbar_wait(&p_full[t], p_phase[t]);
+                        p_phase[t] ^= 1;
+                        tc_fence_after();
+                        issue_pv(t, vslot, j > 0);
+                        if (more) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
+                        else umma_commit(&o_full[t]);
+                    }
+                    umma_commit(&kv_empty[vslot]);
+                    if (more) umma_commit(&kv_empty[kslot]);
+                }
+                umma_commit(q_empty);
+            }
+        }
+    } else if (warp >= kSoftmaxWarp0) {
+        // =============================== softmax / epilogue ===============================
+        const int t = (warp - kSoftmaxWarp0) >> 2;              // sub-tile of this warpgroup
+        const int row = threadIdx.x - kSoftmaxWarp0 * 32 - t * kBlock;   // 0..127 = TMEM lane
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
+        const uint32_t tS = tmem + lane_base + Cfg::kColS + t * kBlock;
+        const uint32_t tO = tmem + lane_base + Cfg::kColO + t * D;
+        uint32_t s_phase = 0, o_phase = 0;
+        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            const ItemCtx c = load_item(p, idx);
+            if (t >= c.nt) continue;
+            const int srow = c.it.q0 + t * kBlock + row;            // local query row
+            const size_t slot = ((size_t)c.g_local * gm.slots_per_gpu + c.it.slot) * gm.batch + c.it.batch;
+            float* out = p.partial_O + ((slot * gm.L + srow) * gm.heads_q + c.it.head) * (size_t)D;
+            float* out_lse = p.partial_lse + (slot * gm.heads_q + c.it.head) * (size_t)gm.L + srow;
+            KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
+            float m = -INFINITY, l = 0.f;     // running max (log2 domain, scaled) and running sum
+            int v, t0, off, j = 0;
+            while (walk.next(v, t0, off)) {
+                mbar_wait(&s_full[t], s_phase);
+                s_phase ^= 1;
+                tc_fence_after();
+                // key column c of this block is visible iff c <= row + dlt
+                const int dlt = c.it.q0 + t * kBlock + off - t0;
+                const bool masked = gm.causal && dlt < kBlock - 1;
+                // pass 1: row max
+                float mx = -INFINITY;
+#pragma unroll 1
+                for (int ch = 0; ch < kBlock / 32; ++ch) {
+                    uint32_t r[32];
+                    tmem_ld_x32(tS + ch * 32, r);
+                    tmem_ld_wait();
+                    if (masked) {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) if (ch * 32 + i <= row + dlt) mx = fmaxf(mx, __uint_as_float(r[i]));
+                    } else {
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
+                    }
+                }
+                const float m_new = fmaxf(m, mx * gm.scale_log2);
+                // rescale the accumulator when the running max moved (warp-uniform decision: TMEM ops are warp-collective)
+                if (j > 0 && __any_sync(0xffffffffu, m_new > m)) {
+                    const float alpha = (m_new == -INFINITY) ? 1.f : ex2(m - m_new);   // m = -inf -> 0
+                    l *= alpha;
+#pragma unroll 1
+                    for (int ch = 0; ch < D / 32; ++ch) {
+                        uint32_t r[32];
+                        tmem_ld_x32(tO + ch * 32, r);
+                        tmem_ld_wait();
+#pragma unroll
+                        for (int i = 0; i < 32; ++i) r[i] = __float_as_uint(__uint_as_float(r[i]) * alpha);
+                        tmem_st_x32(tO + ch * 32, r);
+                    }
+                }
+                m = m_new;
+                const float m_safe = (m == -INFINITY) ? 0.f : m;
+                // pass 2: p = exp2(s*scale_log2 - m), row sum, P (bf16) into TMEM over S
+                float lsum = 0.f;
+#pragma unroll 1
+                for (int ch = 0; ch < kBlock / 32; ++ch) {
+                    uint32_t r[32], pk[16];
+                    tmem_ld_x32(tS + ch * 32, r);
+                    tmem_ld_wait();
+#pragma unroll
+                    for (int i = 0; i < 32; i += 2) {
+                        float p0 = ex2(fmaf(__uint_as_float(r[i]), gm.scale_log2, -m_safe));
+                        float p1 = ex2(fmaf(__uint_as_float(r[i + 1]), gm.scale_log2, -m_safe));
+                        if (masked) {
+                            if (ch * 32 + i > row + dlt) p0 = 0.f;
+                            if (ch * 32 + i + 1 > row + dlt) p1 = 0.f;
+                        }
+                        lsum += p0 + p1;
+                        pk[i / 2] = pack_bf16x2(p0, p1);
+                    }
+                    // chunk ch of S (32 fp32 columns) was fully read above; P chunk ch occupies 16 columns
+                    // [16*ch, 16*ch+16) which only overlaps S columns this thread has already consumed
+                    tmem_st_x16(tS + ch * 16, pk);
+                }
+                l += lsum;
+                tmem_st_wait();
+                tc_fence_before();
+                mbar_arrive(&p_full[t]);
+                ++j;
+            }
+            if (j == 0) {                      // no visible key for the whole item (reading R5)
+#pragma unroll 4
+                for (int d = 0; d < D; d += 4) *reinterpret_cast<float4*>(out + d) = make_float4(0.f, 0.f, 0.f, 0.f);
+                *out_lse = -INFINITY;
+                continue;
+            }
+            mbar_wait(&o_full[t], o_phase);
+            o_phase ^= 1;
+            tc_fence_after();
+            const float inv_l = l > 0.f ? 1.f / l : 0.f;
+#pragma unroll 1
+            for (int ch = 0; ch < D / 32; ++ch) {
+                uint32_t r[32];
+                tmem_ld_x32(tO + ch * 32, r);
+                tmem_ld_wait();
+#pragma unroll
+                for (int i = 0; i < 32; i += 4)
+                    *reinterpret_cast<float4*>(out + ch * 32 + i) =
+                        make_float4(__uint_as_float(r[i]) * inv_l, __uint_as_float(r[i + 1]) * inv_l, __uint_as_float(r[i + 2]) * inv_l,
+                                    __uint_as_float(r[i + 3]) * inv_l);
+            }
+            *out_lse = l > 0.f ? (m + lg2(l)) * 0.6931471805599453f : -INFINITY;
+        }
+    }
+
+    tc_fence_before();
+    __syncthreads();
+    if (warp == kAllocWarp) tmem_dealloc<512>(tmem);
+}
+
+}  // namespace
+
+int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int num_sms,
+                    cudaStream_t stream)
+{
+    const int total = p.items_per_gpu * p.g_count;
+    if (total <= 0) return 0;
+    const int grid = total < num_sms ? total : num_sms;
+    cudaError_t e;
+    if (p.gm.head_dim == 128) {
+        e = cudaFuncSetAttribute(tile_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<128>::kSmemBytes);
+        if (e != cudaSuccess) return (int)e;
+        tile_fwd_kernel<128><<<grid, kThreads, FwdCfg<128>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
+    } else {
+        e = cudaFuncSetAttribute(tile_fwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<64>::kSmemBytes);
+        if (e != cudaSuccess) return (int)e;
+        tile_fwd_kernel<64><<<grid, kThreads, FwdCfg<64>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
+    }
+    return (int)cudaGetLastError();
+}
+
+}  // namespace mesh_attn

@@ -1,0 +1,66 @@
+// tile_kernels.hpp -- parameter blocks and launchers of the CUDA kernels (internal).
+#pragma once
+#include <cuda.h>
+#include <cuda_runtime.h>
+
+#include "plan.hpp"
+
+namespace mesh_attn {
+
+struct FwdParams {
+    Geom gm;
+    const FwdItem* items;      // per-simulated-GPU template, items_per_gpu entries
+    const Seg* segs;
+    const SegList* seglists;
+    int items_per_gpu;
+    int g_first, g_count;
+    float* partial_O;          // [g_count][slots][B][L][Hq][D]
+    float* partial_lse;        // [g_count][slots][B][Hq][L]
+};
+
+struct BwdParams {
+    Geom gm;
+    const BwdItem* items;
+    const Seg* segs;
+    const SegList* seglists;
+    int items_per_gpu;
+    int g_first, g_count;
+    int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
+    const float* lse;          // [B][Hq][N]
+    const float* delta;        // [B][Hq][N]
+    float *dQ, *dK, *dV;       // fp32 accumulators
+    // element strides of dQ (query-shaped) and dK/dV (key-shaped) tensors
+    long long q_stride_b, q_stride_row, q_stride_h;
+    long long k_stride_b, k_stride_row, k_stride_h;
+};
+
+struct MergeParams {
+    Geom gm;
+    int q_group;
+    int m;                     // partials per output row
+    int per;                   // 1 (fused partials) or b (per-pair partials): slot(k) = (k/per)*slots + u_local*per + k%per
+    int rows_per_block;
+    const float* partial_O;
+    const float* partial_lse;
+    float* O;
+    float* lse;
+    long long o_stride_b, o_stride_row, o_stride_h;   // element strides of O
+};
+
+struct DeltaParams {
+    Geom gm;
+    const float* O;
+    const void* dO;            // bf16
+    float* delta;              // [B][Hq][N]
+    long long stride_b, stride_row, stride_h;   // element strides shared by O and dO
+};
+
+// each returns a cudaError_t value (0 = success)
+int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int num_sms,
+                    cudaStream_t stream);
+int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
+                    const CUtensorMap& tmdO, int num_sms, cudaStream_t stream);
+int launch_merge(const MergeParams& p, cudaStream_t stream);
+int launch_delta(const DeltaParams& p, cudaStream_t stream);
+
+}  // namespace mesh_attn

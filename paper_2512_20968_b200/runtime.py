@@ -1,0 +1,36 @@
+"""Plumbing around the C-ABI calls: plan construction from a Workload and device buffers.
+No arithmetic of the method lives here."""
+from __future__ import annotations
+
+import torch
+
+from .binding import Plan, Q_PARTIAL_LSE_BYTES, Q_PARTIAL_O_BYTES
+from .workloads import Workload
+
+
+def plan_for(w: Workload, **overrides) -> Plan:
+    kw = dict(
+        a=w.a, b=w.b, n=w.n, batch=w.batch, seq_total=w.seq_total, heads_q=w.heads_q, heads_kv=w.heads_kv, head_dim=w.head_dim,
+        causal=int(w.causal), kvr=int(w.kvr), seq_layout=int(w.seq_layout == "striped"), order=int(w.order == "greedy"),
+        k_q=w.k_q, k_kv=w.k_kv,
+    )
+    kw.update(overrides)
+    return Plan(**kw)
+
+
+class Buffers:
+    """Caller-owned device buffers for one workload (the library never allocates in hot calls)."""
+
+    def __init__(self, plan: Plan, w: Workload, backward: bool = True, g_count: int | None = None, device="cuda"):
+        B, N, Hq, Hkv, D = w.batch, w.seq_total, w.heads_q, w.heads_kv, w.head_dim
+        g_count = w.a if g_count is None else g_count
+        f32 = dict(dtype=torch.float32, device=device)
+        self.partial_O = torch.empty(plan.query(Q_PARTIAL_O_BYTES) * g_count // 4, **f32)
+        self.partial_lse = torch.empty(plan.query(Q_PARTIAL_LSE_BYTES) * g_count // 4, **f32)
+        self.O = torch.empty((B, N, Hq, D), **f32)
+        self.lse = torch.empty((B, Hq, N), **f32)
+        if backward:
+            self.delta = torch.empty((B, Hq, N), **f32)
+            self.dQ = torch.empty((B, N, Hq, D), **f32)
+            self.dK = torch.empty((B, N, Hkv, D), **f32)
+            self.dV = torch.empty((B, N, Hkv, D), **f32)

@@ -1,0 +1,188 @@
+"""GPU parity: mesh_attn_tile_fwd + mesh_attn_merge (through the C ABI) against the fp64 oracle,
+element by element on the same seeded bf16 inputs.  Tolerances are BASELINE.json's:
+max|dO| <= 1e-2, mean|dO| <= 1e-3, max|dLSE| <= 1e-3."""
+import numpy as np
+import pytest
+import torch
+
+from paper_2512_20968_b200 import workloads as W
+from tests.util import torch_bits
+
+pytestmark = pytest.mark.gpu
+
+TOL_O_MAX, TOL_O_MEAN, TOL_LSE = 1e-2, 1e-3, 1e-3
+
+
+def sample_rows(w, per_part, rng):
+    """first, last and random local rows of EVERY Q partition (hits every pair and every simulated GPU)."""
+    L = w.L
+    rows = []
+    for p in range(w.n):
+        loc = {0, L - 1, 127 % L, 128 % L} | set(int(x) for x in rng.integers(0, L, per_part))
+        rows += [p * L + s for s in sorted(loc)]
+    return np.array(rows, dtype=np.int64)
+
+
+def run_forward(w, inp, **overrides):
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    plan = plan_for(w, **overrides)
+    buf = Buffers(plan, w, backward=False)
+    buf.O.fill_(float("nan"))
+    buf.lse.fill_(float("nan"))
+    plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+    torch.cuda.synchronize()
+    return plan, buf
+
+
+def check_against_oracle(oracle, w, inp, O, lse, rows=None, heads=None, batch_index=0):
+    """O: [N, Hq, D] float32 numpy, lse: [Hq, N]."""
+    q, k, v = (torch_bits(inp[x][batch_index]) for x in ("q", "k", "v"))
+    pos = oracle.positions(w.n, w.L, w.seq_layout)
+    heads = list(range(w.heads_q)) if heads is None else heads
+    rows = np.arange(w.seq_total) if rows is None else rows
+    rr = np.tile(rows, len(heads))
+    hh = np.repeat(np.asarray(heads, dtype=np.int32), len(rows))
+    O_ref, lse_ref = oracle.fwd_rows(q, k, v, w.scale, w.causal, pos, rr, hh)
+    O_gpu = O[rr, hh].astype(np.float64)
+    lse_gpu = lse[hh, rr].astype(np.float64)
+    assert np.isfinite(O_gpu).all(), "non-finite output"
+    dO = np.abs(O_gpu - O_ref)
+    finite = np.isfinite(lse_ref)
+    assert np.array_equal(np.isfinite(lse_gpu), finite)
+    dl = np.abs(lse_gpu[finite] - lse_ref[finite])
+    assert dO.max() <= TOL_O_MAX, f"max|dO| = {dO.max():.3e}"
+    assert dO.mean() <= TOL_O_MEAN, f"mean|dO| = {dO.mean():.3e}"
+    assert dl.max() <= TOL_LSE, f"max|dLSE| = {dl.max():.3e}"
+    return dO.max(), dO.mean(), dl.max()
+
+
+def test_c1_full(oracle):
+    """BASELINE.json configs[0] exactly: non-causal MHA 2x2, N=1024, 4 heads, D=64; forward + merge."""
+    w = W.C1
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    _, buf = run_forward(w, inp)
+    check_against_oracle(oracle, w, inp, buf.O[0].cpu().numpy(), buf.lse[0].cpu().numpy())
+
+
+@pytest.mark.parametrize("name,L,hq", [("C2", 384, 4), ("C3", 512, 2), ("C4", 256, 8), ("C5", 256, 2)])
+def test_scaled_configs(oracle, name, L, hq):
+    """Structure of configs[1..4] (mesh, mask, GQA ratio, outliers, order) at a partition length the oracle
+    finishes in seconds; L=384 has an odd number of 128-row blocks (a ragged 128-row work item)."""
+    w = W.scaled_down(W.CONFIGS[name], L, heads_q=hq)
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    _, buf = run_forward(w, inp)
+    rng = np.random.default_rng(1)
+    rows = None if w.seq_total <= 4096 else sample_rows(w, 2, rng)
+    heads = None if w.seq_total <= 4096 else [0, w.heads_q - 1]
+    check_against_oracle(oracle, w, inp, buf.O[0].cpu().numpy(), buf.lse[0].cpu().numpy(), rows, heads)
+
+
+@pytest.mark.parametrize("layout", ["contiguous", "striped"])
+@pytest.mark.parametrize("kvr", [False, True])
+def test_causal_layouts_and_kvr(oracle, layout, kvr):
+    """contiguous causal layout has fully masked pairs (work items with zero blocks) and diagonal pairs;
+    basic tiling (kvr off) changes which simulated GPU computes which pair -- the merged result is the same."""
+    from dataclasses import replace
+
+    w = replace(W.scaled_down(W.C3, 256, heads_q=2), seq_layout=layout, kvr=kvr, outlier=False, order="row_major", k_q=1, k_kv=1)
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    _, buf = run_forward(w, inp)
+    check_against_oracle(oracle, w, inp, buf.O[0].cpu().numpy(), buf.lse[0].cpu().numpy())
+
+
+def test_partials_fused_and_per_pair(oracle):
+    """Partial outputs themselves: fused partial of (g, u) = attention of Q_u over the keys of I_g^KV
+    (Alg.2 l.5); per-pair partial (u, v) = Attention(Q_u, K_v, V_v); a striped pair with
+    v > u has row s = 0 with no visible key: (0, -inf)."""
+    from dataclasses import replace
+
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    w = replace(W.scaled_down(W.C3, 128, heads_q=2), outlier=False, order="row_major", k_q=1, k_kv=1, a=2, b=3, seq_total=6 * 128)
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    q, k, v = (torch_bits(inp[x][0]) for x in ("q", "k", "v"))
+    pos = oracle.positions(w.n, w.L, w.seq_layout)
+    part = np.arange(w.seq_total) // w.L
+    for mode in (0, 1):
+        plan = plan_for(w, partial_mode=mode)
+        buf = Buffers(plan, w, backward=False, g_count=w.n)
+        plan.tile_fwd(0, w.n, inp["q"], inp["k"], inp["v"], buf.partial_O, buf.partial_lse)
+        torch.cuda.synchronize()
+        slots = w.a * (w.b if mode else 1)
+        pO = buf.partial_O.view(w.n, slots, 1, w.L, w.heads_q, w.head_dim).cpu().numpy()
+        pl = buf.partial_lse.view(w.n, slots, 1, w.heads_q, w.L).cpu().numpy()
+        saw_empty = False
+        for g in range(w.n):
+            iq, ikv = plan.footprint(g)
+            for ul, u in enumerate(iq):
+                groups = [[x] for x in ikv] if mode else [list(ikv)]
+                for gi, kvs in enumerate(groups):
+                    slot = ul * w.b + gi if mode else ul
+                    sel = np.isin(part, kvs).astype(np.uint8)
+                    rows = np.arange(u * w.L, (u + 1) * w.L)
+                    for h in range(w.heads_q):
+                        O_ref, l_ref = oracle.fwd_rows(q, k, v, w.scale, True, pos, rows, np.full(len(rows), h, np.int32), key_sel=sel)
+                        O_g, l_g = pO[g, slot, 0, :, h], pl[g, slot, 0, h]
+                        fin = np.isfinite(l_ref)
+                        saw_empty |= (~fin).any()
+                        assert np.array_equal(np.isfinite(l_g), fin)
+                        assert np.all(O_g[~fin] == 0) and np.all(l_g[~fin] == -np.inf)
+                        assert np.abs(O_g - O_ref).max() <= TOL_O_MAX
+                        assert np.abs(l_g[fin] - l_ref[fin]).max() <= TOL_LSE
+        if mode:
+            assert saw_empty
+        # merged result of this mode
+        buf2 = Buffers(plan, w, backward=False)
+        plan.forward(inp["q"], inp["k"], inp["v"], buf2.O, buf2.lse, buf2.partial_O, buf2.partial_lse)
+        torch.cuda.synchronize()
+        check_against_oracle(oracle, w, inp, buf2.O[0].cpu().numpy(), buf2.lse[0].cpu().numpy())
+
+
+def test_batch_and_bhnd_layout(oracle):
+    from dataclasses import replace
+
+    w = replace(W.scaled_down(W.C4, 128, heads_q=4), batch=2, a=2, b=2, seq_total=4 * 128)
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    _, buf = run_forward(w, inp)
+    for bi in range(2):
+        check_against_oracle(oracle, w, inp, buf.O[bi].cpu().numpy(), buf.lse[bi].cpu().numpy(), batch_index=bi)
+    # [B, H, N, D] tensors: same values, different strides
+    inp_t = {kk: vv.permute(0, 2, 1, 3).contiguous() for kk, vv in inp.items()}
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    plan = plan_for(w, tensor_layout=1)
+    b2 = Buffers(plan, w, backward=False)
+    O_t = torch.empty((w.batch, w.heads_q, w.seq_total, w.head_dim), dtype=torch.float32, device="cuda")
+    plan.forward(inp_t["q"], inp_t["k"], inp_t["v"], O_t, b2.lse, b2.partial_O, b2.partial_lse)
+    torch.cuda.synchronize()
+    assert torch.equal(O_t.permute(0, 2, 1, 3), buf.O) and torch.equal(b2.lse, buf.lse)
+
+
+def test_merge_kernel_alone(oracle):
+    """mesh_attn_merge on synthetic partials incl. -inf entries, against oracle.merge (fp32 tolerance)."""
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    w = W.scaled_down(W.C2, 128, heads_q=4)
+    plan = plan_for(w)
+    buf = Buffers(plan, w, backward=False)
+    g = torch.Generator(device="cuda").manual_seed(5)
+    pO = torch.randn(buf.partial_O.shape, generator=g, device="cuda")
+    pl = torch.randn(buf.partial_lse.shape, generator=g, device="cuda") * 4
+    pl[torch.rand(pl.shape, generator=g, device="cuda") < 0.2] = float("-inf")
+    plv = pl.view(w.a, w.a, 1, w.heads_q, w.L)
+    plv[:, 0, 0, 0, 5] = float("-inf")                      # one (row, head) with every partial empty
+    buf.O.zero_()
+    plan.merge(1, pO, pl, buf.O, buf.lse)
+    torch.cuda.synchronize()
+    pOv = pO.view(w.a, w.a, 1, w.L, w.heads_q, w.head_dim).cpu().numpy().astype(np.float64)
+    plc = plv.cpu().numpy().astype(np.float64)
+    O, lse = buf.O[0].cpu().numpy(), buf.lse[0].cpu().numpy()
+    rng = np.random.default_rng(0)
+    cases = [(0, 5, 0)] + [(int(rng.integers(w.a)), int(rng.integers(w.L)), int(rng.integers(w.heads_q))) for _ in range(300)]
+    for ul, s, h in cases:
+        O_ref, l_ref = oracle.merge(pOv[:, ul, 0, s, h], plc[:, ul, 0, h, s])
+        row = (1 * w.a + ul) * w.L + s
+        assert np.abs(O[row, h] - O_ref).max() <= 1e-5
+        assert (l_ref == -np.inf and lse[h, row] == -np.inf) or abs(lse[h, row] - l_ref) <= 1e-5
+    assert torch.all(buf.O[0, : w.a * w.L] == 0)              # other Q groups untouched

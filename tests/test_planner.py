@@ -1,0 +1,152 @@
+"""C++ planner (through the C ABI, host only) against oracle/plan_oracle.py, the paper's printed
+examples and structural invariants.  No GPU needed."""
+import numpy as np
+import pytest
+
+from oracle import plan_oracle as po
+from paper_2512_20968_b200 import binding as B
+from paper_2512_20968_b200.binding import MeshAttnError, Plan
+
+
+def mk(a, b, L=128, **kw):
+    base = dict(a=a, b=b, batch=1, seq_total=a * b * L, heads_q=2, heads_kv=1, head_dim=64)
+    base.update(kw)
+    return Plan(**base)
+
+
+def test_library_exports_every_declared_symbol():
+    import re
+    from pathlib import Path
+
+    header = (Path(__file__).parent.parent / "include" / "mesh_attn.h").read_text()
+    code = re.sub(r"/\*.*?\*/", "", header, flags=re.S)          # declarations only, comments stripped
+    declared = set(re.findall(r"\b(mesh_attn_[a-z_]+)\s*\(", code))
+    assert declared == set(B.EXPORTED)
+    for name in declared:
+        assert hasattr(B.lib, name), name
+
+
+@pytest.mark.parametrize("a,b", [(2, 2), (3, 3), (3, 5), (5, 3), (4, 4), (1, 4), (4, 1), (8, 8), (16, 16)])
+@pytest.mark.parametrize("kvr", [0, 1])
+def test_am_and_footprints_match_oracle(a, b, kvr):
+    n = a * b
+    p = mk(a, b, kvr=kvr)
+    A = po.assignment_matrix(n, a, b, bool(kvr))
+    assert p.am().tolist() == A
+    for g in range(n):
+        IQ, IKV, _, _ = po.footprints(A, g)
+        iq, ikv = p.footprint(g)
+        assert iq.tolist() == IQ and ikv.tolist() == IKV
+    assert p.query(B.Q_COMM_UNITS) == po.comm_units(A)
+    assert p.query(B.Q_WAVES) == b and p.query(B.Q_HAS_DEVICE) in (0, 1)
+
+
+def test_paper_fig1_units():
+    assert mk(3, 3, kvr=0).query(B.Q_COMM_UNITS) == 84
+    assert mk(3, 3, kvr=1).query(B.Q_COMM_UNITS) == 72
+    assert mk(3, 3, kvr=1).footprint(3)[1].tolist() == [0, 3, 6]
+
+
+def _steps_to_oracle_form(rows):
+    out = {}
+    for step, kind, i, j in rows.tolist():
+        comm, fill = out.setdefault(step, [None, []])
+        if kind == B.TASK_C:
+            fill.append((i, j))
+        else:
+            out[step][0] = (kind, j if kind in (B.TASK_AG_KV, B.TASK_RS_KV) else i)
+    return [(tuple(v[0]) if v[0] else None, v[1]) for _, v in sorted(out.items())]
+
+
+def test_goo_fig4_example():
+    # k_Q = k_KV = 3, T = (AG-KV 1, AG-Q .5, RS-Q .5, C .5), gamma = 1
+    p = mk(2, 2, L=384, order=1, k_q=3, k_kv=3, gamma=1.0, t_ag_kv=1.0, t_ag_q=0.5, t_rs_q=0.5, t_c=0.5)
+    steps = _steps_to_oracle_form(p.steps())
+    assert steps == po.goo_forward(3, 3, 1.0, 0.5, 0.5, 0.5, gamma=1.0)
+    comm = [c for c, _ in steps]
+    assert comm[:6] == [(B.TASK_AG_KV, 0), (B.TASK_AG_Q, 0), (B.TASK_AG_Q, 1), (B.TASK_AG_KV, 1), (B.TASK_AG_Q, 2), (B.TASK_AG_KV, 2)]
+    assert steps[2][1] == [(0, 0)] and steps[5][1] == [(1, 1), (2, 0)]
+    assert [k + 1 for k, c in enumerate(comm) if c is None] == [7, 10] and len(steps) == 11
+
+
+@pytest.mark.parametrize("kq,kkv", [(1, 1), (2, 2), (4, 4), (2, 8), (8, 2), (1, 16), (16, 1), (3, 5)])
+@pytest.mark.parametrize("costs", [(1.0, 0.5, 0.5, 0.5), (0.3, 0.7, 0.2, 1.0), (2.0, 2.0, 2.0, 0.1)])
+def test_goo_matches_oracle_and_tile_lists(kq, kkv, costs):
+    L = 128 * kq * kkv
+    p = mk(2, 3, L=L, kvr=1, order=1, k_q=kq, k_kv=kkv, t_ag_kv=costs[0], t_ag_q=costs[1], t_rs_q=costs[2], t_c=costs[3])
+    ref = po.goo_forward(kq, kkv, *costs, gamma=1.05)
+    assert _steps_to_oracle_form(p.steps()) == ref
+    order = po.compute_order(ref)
+    for g in range(6):
+        assert [tuple(r) for r in p.tiles(g).tolist()] == po.tile_list(6, 2, 3, True, g, order)
+
+
+def test_backward_goo_is_valid():
+    # PAPER.md L238 omits the backward schedule: validity invariants only (parity unpinned)
+    p = mk(2, 2, L=512, order=1, k_q=2, k_kv=2)
+    rows = p.steps(backward=True).tolist()
+    have_q, have_kv, done = set(), set(), set()
+    for step in sorted({r[0] for r in rows}):
+        cur = [r for r in rows if r[0] == step]
+        for _, kind, i, j in cur:
+            if kind == B.TASK_C:
+                assert i in have_q and j in have_kv and (i, j) not in done
+        for _, kind, i, j in cur:
+            if kind == B.TASK_RS_Q:
+                assert all((i, jj) in done for jj in range(2))
+            if kind == B.TASK_RS_KV:
+                assert all((ii, j) in done for ii in range(2))
+        for _, kind, i, j in cur:
+            if kind == B.TASK_C:
+                done.add((i, j))
+            elif kind == B.TASK_AG_Q:
+                have_q.add(i)
+            elif kind == B.TASK_AG_KV:
+                have_kv.add(j)
+        assert sum(1 for r in cur if r[1] != B.TASK_C) <= 1
+    assert len(done) == 4
+    kinds = [r[1] for r in rows]
+    assert kinds.count(B.TASK_RS_Q) == 2 and kinds.count(B.TASK_RS_KV) == 2
+
+
+def test_row_major_order_and_queries():
+    p = mk(3, 3, L=256, kvr=1, heads_q=4, heads_kv=2, head_dim=128, batch=2)
+    t = p.tiles(4)
+    assert [tuple(r) for r in t.tolist()] == po.tile_list(9, 3, 3, True, 4, [(0, 0)])
+    N = 9 * 256
+    assert p.query(B.Q_FLOPS_FWD) == 4 * 128 * 4 * 2 * N * N
+    assert p.query(B.Q_FLOPS_BWD) == 10 * 128 * 4 * 2 * N * N
+    assert p.query(B.Q_SLOTS_PER_GPU) == 3
+    assert p.query(B.Q_PARTIAL_O_BYTES) == 3 * 2 * 256 * 4 * 128 * 4
+    assert p.query(B.Q_PARTIAL_LSE_BYTES) == 3 * 2 * 256 * 4 * 4
+    assert p.query(B.Q_BLOCKS_FWD) == (N // 128) ** 2 * 4 * 2
+    assert p.query(B.Q_FWD_ITEMS_PER_GPU) == 2 * 4 * 3 * 1           # batch x heads x a x (256/256)
+    assert p.query(B.Q_BWD_ITEMS_PER_GPU) == 2 * 2 * 3 * 2           # batch x kv heads x b x (256/128)
+    pc = mk(2, 2, L=256, causal=1, seq_layout=1)
+    # striped causal: pairs v<=u are lower-triangular incl. diagonal (3 of 4 blocks at L=256), v>u strictly lower (3 of 4 too:
+    # block (0,1) fully masked, diagonal blocks partially) -> every pair computes 3 blocks
+    assert pc.query(B.Q_BLOCKS_FWD) == 16 * 3 * 2
+    assert pc.query(B.Q_FLOPS_FWD) == 4 * 64 * 2 * (1024 * 1025 // 2)
+
+
+@pytest.mark.parametrize("bad", [
+    dict(n=5), dict(seq_total=1000), dict(seq_total=4 * 64), dict(heads_q=3, heads_kv=2), dict(head_dim=96),
+    dict(k_q=5, k_kv=4), dict(k_q=3), dict(causal=2), dict(batch=0),
+])
+def test_invalid_geometry_is_rejected_at_plan_creation(bad):
+    kw = dict(a=2, b=2, n=4, batch=1, seq_total=4 * 256, heads_q=2, heads_kv=1, head_dim=64)
+    kw.update(bad)
+    with pytest.raises(MeshAttnError) as e:
+        Plan(**kw)
+    assert e.value.status in (B.EINVAL, B.EUNSUPPORTED)
+
+
+def test_compute_calls_fail_loudly_without_gpu():
+    import torch
+
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    p = mk(2, 2)
+    with pytest.raises(MeshAttnError) as e:
+        p.tile_fwd(0, 1, 16, 16, 16, 16, 16, stream=0)
+    assert e.value.status == B.ECUDA
