@@ -1,0 +1,154 @@
+"""GPU parity: mesh_attn_bwd_preprocess + mesh_attn_tile_bwd (through the C ABI) against the fp64
+oracle on the same seeded bf16 inputs.  Tolerance (BASELINE.json): gradients within 2e-2 max abs."""
+from dataclasses import replace
+
+import numpy as np
+import pytest
+import torch
+
+from paper_2512_20968_b200 import workloads as W
+from tests.util import bits_to_f64, torch_bits
+
+pytestmark = pytest.mark.gpu
+
+TOL_GRAD = 2e-2
+
+
+def run_fwd_bwd(w, inp, **overrides):
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    plan = plan_for(w, **overrides)
+    buf = Buffers(plan, w, backward=True)
+    plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+    for t in (buf.dQ, buf.dK, buf.dV):
+        t.fill_(float("nan"))                     # mesh_attn_backward zeroes the accumulators itself
+    plan.backward(inp["q"], inp["k"], inp["v"], buf.O, inp["do"], buf.lse, buf.delta, buf.dQ, buf.dK, buf.dV)
+    torch.cuda.synchronize()
+    return plan, buf
+
+
+def check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads, qs_rows=None, bi=0, tol=TOL_GRAD):
+    q, k, v, do = (torch_bits(inp[x][bi]) for x in ("q", "k", "v", "do"))
+    pos = oracle.positions(w.n, w.L, w.seq_layout)
+    dq_ref, _, delta_ref = oracle.bwd_dq_rows(q, k, v, do, w.scale, w.causal, pos, qrows, qheads)
+    dq = buf.dQ[bi].cpu().numpy()[qrows, qheads].astype(np.float64)
+    delta = buf.delta[bi].cpu().numpy()[qheads, qrows].astype(np.float64)
+    dk_ref, dv_ref = oracle.bwd_dkv_keys(q, k, v, do, w.scale, w.causal, pos, krows, kheads, qs_rows=qs_rows)
+    dk = buf.dK[bi].cpu().numpy()[krows, kheads].astype(np.float64)
+    dv = buf.dV[bi].cpu().numpy()[krows, kheads].astype(np.float64)
+    errs = dict(dq=np.abs(dq - dq_ref).max(), dk=np.abs(dk - dk_ref).max(), dv=np.abs(dv - dv_ref).max(),
+                delta=np.abs(delta - delta_ref).max())
+    assert np.isfinite(dq).all() and np.isfinite(dk).all() and np.isfinite(dv).all()
+    # delta = dO . O inherits the forward's output error: |d delta| <= sum_d |dO_d| |dO_d err| ~ sqrt(D) * max|dO| ~ 5e-2
+    assert errs["delta"] <= 5e-2, errs
+    assert max(errs["dq"], errs["dk"], errs["dv"]) <= tol, errs
+    return errs
+
+
+def check_invariants(w, inp, buf, bi=0):
+    """hold for any mask, per KV head: sum_t dV[t] = sum_s dO[s] (rows of P sum to 1), sum_t dK[t] = 0
+    (rows of dS sum to 0), <Q,dQ> = <K,dK>."""
+    g = w.heads_q // w.heads_kv
+    do = inp["do"][bi].double()
+    dV, dK, dQ = buf.dV[bi].double(), buf.dK[bi].double(), buf.dQ[bi].double()
+    N = w.seq_total
+    sum_do = do.view(N, w.heads_kv, g, w.head_dim).sum((0, 2))
+    # N terms of per-element error <= 2e-2 add up like sqrt(N); outlier data adds a relative part (bf16 operands)
+    tol = 2e-2 * max(1.0, N ** 0.5 / 8)
+    assert (dV.sum(0) - sum_do).abs().max().item() <= tol + 4e-3 * sum_do.abs().max().item()
+    assert dK.sum(0).abs().max().item() <= tol + 4e-3 * dK.abs().sum(0).max().item() / N ** 0.5
+    a = (inp["q"][bi].double() * dQ).sum().item()
+    b = (inp["k"][bi].double() * dK).sum().item()
+    scale = (inp["q"][bi].double() * dQ).abs().sum().item()
+    assert abs(a - b) <= 1e-3 * scale
+
+
+def all_pairs(rows, heads):
+    return np.repeat(np.asarray(rows, dtype=np.int64), len(heads)), np.tile(np.asarray(heads, dtype=np.int32), len(rows))
+
+
+@pytest.mark.parametrize("name,L,hq", [("C2", 384, 4), ("C4", 128, 8)])
+def test_scaled_configs_full_keys(oracle, name, L, hq):
+    w = W.scaled_down(W.CONFIGS[name], L, heads_q=hq)
+    inp = W.make_inputs(w, "cuda")
+    _, buf = run_fwd_bwd(w, inp)
+    rng = np.random.default_rng(3)
+    rows = np.unique(np.concatenate([rng.integers(0, w.seq_total, 48), [0, w.seq_total - 1, w.L - 1, w.L]]))
+    qrows, qheads = all_pairs(rows, [0, w.heads_q - 1])
+    krows, kheads = all_pairs(rows[:24], [0, w.heads_kv - 1] if w.seq_total <= 4096 else [w.heads_kv - 1])
+    check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
+    check_invariants(w, inp, buf)
+
+
+@pytest.mark.parametrize("layout,kvr", [("contiguous", True), ("striped", False), ("striped", True)])
+def test_causal_small_full(oracle, layout, kvr):
+    """every row / key of a small causal problem (3x2 mesh, GQA 2:1): exercises diagonal blocks, fully masked
+    pairs (contiguous), both tilings."""
+    w = replace(W.scaled_down(W.C4, 128, heads_q=4), a=3, b=2, seq_total=6 * 128, heads_kv=2, seq_layout=layout, kvr=kvr)
+    inp = W.make_inputs(w, "cuda")
+    _, buf = run_fwd_bwd(w, inp)
+    qrows, qheads = all_pairs(np.arange(w.seq_total), range(w.heads_q))
+    krows, kheads = all_pairs(np.arange(w.seq_total), range(w.heads_kv))
+    check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
+    check_invariants(w, inp, buf)
+
+
+def test_c5_shape_sparse_do_probe(oracle):
+    """16x16 mesh, causal striped, greedy order, k_q = k_kv = 2 (configs[4] structure) at L = 256.
+    dK/dV are checked in full-tensor fashion with the sparse-dO probe: dO non-zero on R sampled query rows
+    only, so all of dK, dV depends on R oracle rows (gradients are linear in dO)."""
+    w = W.scaled_down(W.C5, 256, heads_q=2)
+    inp = W.make_inputs(w, "cuda")
+    rng = np.random.default_rng(11)
+    live = np.unique(np.concatenate([rng.integers(0, w.seq_total, 40), [w.seq_total - 1, 5 * w.L]]))
+    mask = torch.zeros(w.seq_total, dtype=torch.bool, device="cuda")
+    mask[torch.as_tensor(live, device="cuda")] = True
+    inp["do"] = inp["do"] * mask[None, :, None, None]
+    _, buf = run_fwd_bwd(w, inp)
+    qrows, qheads = all_pairs(live, [0, 1])
+    krows = np.unique(np.concatenate([rng.integers(0, w.seq_total, 200), [0, 1, w.L - 1, w.L, w.seq_total - 1]]))
+    krows, kheads = all_pairs(krows, [0, 1])
+    check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads, qs_rows=live)
+    check_invariants(w, inp, buf)
+    # rows with dO = 0 have dQ = 0 exactly
+    assert torch.all(buf.dQ[0][~mask] == 0)
+
+
+def test_batch_and_bhnd_layout(oracle):
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    w = replace(W.scaled_down(W.C4, 128, heads_q=4), batch=2, a=2, b=2, seq_total=4 * 128)
+    inp = W.make_inputs(w, "cuda")
+    _, buf = run_fwd_bwd(w, inp)
+    rows = np.arange(0, w.seq_total, 7)
+    for bi in range(2):
+        qrows, qheads = all_pairs(rows, range(w.heads_q))
+        krows, kheads = all_pairs(rows, range(w.heads_kv))
+        check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads, bi=bi)
+    inp_t = {kk: vv.permute(0, 2, 1, 3).contiguous() for kk, vv in inp.items()}
+    plan = plan_for(w, tensor_layout=1)
+    b2 = Buffers(plan, w, backward=True)
+    tr = lambda t: torch.empty_like(t.permute(0, 2, 1, 3).contiguous())
+    O_t, dQ_t, dK_t, dV_t = tr(b2.O), tr(b2.dQ), tr(b2.dK), tr(b2.dV)
+    plan.forward(inp_t["q"], inp_t["k"], inp_t["v"], O_t, b2.lse, b2.partial_O, b2.partial_lse)
+    plan.backward(inp_t["q"], inp_t["k"], inp_t["v"], O_t, inp_t["do"], b2.lse, b2.delta, dQ_t, dK_t, dV_t)
+    torch.cuda.synchronize()
+    # atomics make the summation order run-dependent: compare to tolerance, not bit-exactly
+    for a, b in ((dQ_t, buf.dQ), (dK_t, buf.dK), (dV_t, buf.dV)):
+        assert (a.permute(0, 2, 1, 3) - b).abs().max().item() <= 1e-3
+
+
+def test_outlier_scores_c3_shape(oracle):
+    """configs[2] structure: 4 of 128 Q/K channels x8 (|scaled score| up to ~100), causal striped 4x4, greedy order.
+    Reports the error of the single-bf16-operand backward on this data (the 2e-2 absolute bar is a ~2e-4 relative
+    bar here); the split-precision mode is the one required to meet it."""
+    w = W.scaled_down(W.C3, 512, heads_q=2)
+    inp = W.make_inputs(w, "cuda")
+    _, buf = run_fwd_bwd(w, inp)
+    rng = np.random.default_rng(5)
+    rows = np.unique(rng.integers(0, w.seq_total, 48))
+    qrows, qheads = all_pairs(rows, [0, 1])
+    krows, kheads = all_pairs(rows[:24], [0, 1])
+    errs = check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads, tol=0.5)
+    print("C3-shape single-bf16 operand errors:", errs)
+    check_invariants(w, inp, buf)
