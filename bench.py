@@ -1,0 +1,429 @@
+#!/usr/bin/env python
+"""bench.py -- one "step" = one pass of the whole hot path (plan -> tile forward ->
+merge, bwd preprocess -> tile backward with in-place reductions) over one synthetic workload.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload C5] [--impl ours|reference]
+
+Prints ONE JSON line (rank 0).  `value` = algorithmic forward+backward attention TFLOP/s of the whole
+job (all N GPUs: replicas of the same workload), inputs resident in HBM;
+`e2e` = the same metric through mesh_attn_step_host (host buffers, H2D/D2H inside the timed region);
+`roofline` = the dominant kernel (tile backward) against the measured dense-bf16 peak, timed per
+launch with CUDA events inside the timed region (mesh_attn_profile_*); `cpu_baseline` = the fp64 oracle
+on the host cores over a bounded sample.  `--impl reference` times the oracle only (rank 0).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import time
+from pathlib import Path
+
+ROOT = Path(__file__).resolve().parent
+if str(ROOT) not in sys.path:
+    sys.path.insert(0, str(ROOT))
+
+METRIC = "attention_fwd_bwd_tflops"
+UNIT = "TFLOP/s"
+FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=2)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C5", help="C1..C5 (BASELINE.json configs[0..4]); default: the 1M-token causal config")
+    ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target duration of the oracle sample")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            d = json.loads(p.read_text())
+            return {k: float(d[k]) for k in FALLBACK_PEAKS}, "measured"
+        except Exception:
+            pass
+    return dict(FALLBACK_PEAKS), "fallback"
+
+
+# ------------------------------------------------------------------------------------------ clocks
+CLOCK_QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+               "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+
+class ClockSampler:
+    """nvidia-smi sampled every 200 ms DURING the timed region (B200_PROFILING.md clocks line)."""
+
+    def __init__(self, device_index: int):
+        self.proc = None
+        self.idx = device_index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={CLOCK_QUERY}", "--format=csv,noheader,nounits", "-lms", "200",
+                                          "-i", str(self.idx)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2])); pw.append(float(f[3]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": statistics.median(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------ oracle leg
+def oracle_inputs_cpu(w):
+    """Seeded host inputs for the oracle-only arm: the query heads of KV head 0's group (the oracle's cost per
+    (row, head) does not depend on which head), generated on the CPU with the workload's recipe."""
+    from dataclasses import replace
+
+    import numpy as np
+    import torch
+
+    from paper_2512_20968_b200 import workloads as W
+
+    g = w.heads_q // w.heads_kv
+    ws = replace(w, heads_q=g, heads_kv=1)
+    inp = W.make_inputs(ws, "cpu", ("q", "k", "v", "do") if w.backward else ("q", "k", "v"))
+    return {k: t[0].contiguous().view(torch.int16).numpy().view(np.uint16) for k, t in inp.items()}
+
+
+def oracle_inputs_from_device(w, inp):
+    """Host copy (bf16 bits) of KV head 0 and its query-head group from the device inputs of the GPU arm."""
+    import numpy as np
+    import torch
+
+    g = w.heads_q // w.heads_kv
+    out = {}
+    for k, t in inp.items():
+        h = g if k in ("q", "do") else 1
+        out[k] = t[0, :, :h, :].contiguous().cpu().view(torch.int16).numpy().view(np.uint16)
+    return out
+
+
+class OracleSample:
+    """The oracle as it stands (oracle/attn_oracle.py, fp64, OpenMP over sampled rows) on a bounded sample of the
+    workload: R random query rows of query head 0 -> forward (O, LSE from the definition) and, for workloads with a
+    backward pass, the query-side backward (LSE, Delta, dQ).  Algorithmic FLOPs counted for the sample: 4*D per
+    visible (q,k) pair forward; 6*D backward (the S, dP and dQ contractions; the key-side dK/dV sums, 4*D, need
+    every query row per key and are not in the sample)."""
+
+    def __init__(self, w, host, seconds: float):
+        import numpy as np
+
+        from oracle import attn_oracle as oracle
+
+        oracle.build()
+        self.np, self.oracle, self.w, self.host = np, oracle, w, host
+        self.threads = oracle.num_threads()
+        self.pos = oracle.positions(w.n, w.L, w.seq_layout)
+        self.rng = np.random.default_rng(20968)
+        dt, _ = self.run(self.rows(self.threads))                      # calibration pass
+        per_round = max(dt, 1e-3)
+        self.R = int(max(1, min(4096, round(seconds / per_round)))) * self.threads
+
+    def rows(self, count):
+        return self.np.sort(self.rng.integers(0, self.w.seq_total, count)).astype(self.np.int64)
+
+    def run(self, rows):
+        np, w, h = self.np, self.w, self.host
+        heads = np.zeros(len(rows), dtype=np.int32)
+        t0 = time.perf_counter()
+        self.oracle.fwd_rows(h["q"], h["k"], h["v"], w.scale, w.causal, self.pos, rows, heads)
+        if w.backward:
+            self.oracle.bwd_dq_rows(h["q"], h["k"], h["v"], h["do"], w.scale, w.causal, self.pos, rows, heads)
+        dt = time.perf_counter() - t0
+        vis = int((self.pos[rows] + 1).sum()) if w.causal else len(rows) * w.seq_total
+        return dt, vis * w.head_dim * (4.0 + (6.0 if w.backward else 0.0))
+
+    def timed(self):
+        dt, flops = self.run(self.rows(self.R))
+        return dt, flops
+
+    def describe(self):
+        return (f"{self.R} random query rows of head 0 of {self.w.name}: fp64 forward rows"
+                + (" + query-side backward rows (dQ, Delta)" if self.w.backward else "") + ", all keys")
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2512_20968_b200 import workloads as W
+
+    w = W.CONFIGS[args.workload]
+    host = oracle_inputs_cpu(w)
+    smp = OracleSample(w, host, args.cpu_seconds)
+    for _ in range(args.warmup):
+        smp.run(smp.rows(smp.threads))                                  # warm-up: one row per thread
+    tot_t = tot_f = 0.0
+    for _ in range(args.steps):
+        dt, fl = smp.timed()
+        tot_t += dt
+        tot_f += fl
+    val = tot_f / tot_t / 1e12
+    line = {
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": workload_config(w, "oracle sample per step: " + smp.describe()),
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.threads, "kind": "oracle", "sample": smp.describe()},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(w, note=""):
+    cfg = {
+        "workload": f"{w.name} (BASELINE.json configs[{w.index - 1}])", "mask": "causal" if w.causal else "non-causal",
+        "mesh": f"{w.a}x{w.b}", "n": w.n, "seq_total": w.seq_total, "L": w.L, "batch": w.batch, "heads_q": w.heads_q,
+        "heads_kv": w.heads_kv, "head_dim": w.head_dim, "seq_layout": w.seq_layout, "kvr": w.kvr, "order": w.order,
+        "k_q": w.k_q, "k_kv": w.k_kv, "passes": "fwd+merge+bwd" if w.backward else "fwd+merge",
+        "inputs": "bf16 iid N(0,1)" + (" with 4 of 128 Q/K channels x8" if w.outlier else ""),
+        "l2": "inputs larger than L2 (no flush needed)" if w.seq_total * w.heads_q * w.head_dim * 2 > (126 << 20) else "L2-resident (report only)",
+    }
+    if note:
+        cfg["note"] = note
+    return cfg
+
+
+# ------------------------------------------------------------------------------------------ GPU arm
+def physical_gpu_index(local_rank: int) -> int:
+    """nvidia-smi index of this rank's GPU (CUDA_VISIBLE_DEVICES may renumber them)."""
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+    ids = [x for x in vis.split(",") if x.strip()]
+    if local_rank < len(ids) and ids[local_rank].strip().isdigit():
+        return int(ids[local_rank])
+    return local_rank
+
+
+def alloc_host(shape, dtype, torch):
+    """pinned host buffer; pageable if the box refuses to pin that much"""
+    try:
+        return torch.empty(shape, dtype=dtype, pin_memory=True), True
+    except RuntimeError:
+        return torch.empty(shape, dtype=dtype), False
+
+
+def run_e2e(plan, w, inp, buf, torch, steps):
+    """The public host-buffer call (mesh_attn_step_host): H2D of Q,K,V(,dO), the whole hot path, D2H of O, LSE
+    (and dQ,dK,dV), all inside the timed region."""
+    host_in, host_out, pinned = {}, {}, True
+    for k, t in inp.items():
+        host_in[k], p = alloc_host(t.shape, t.dtype, torch)
+        pinned &= p
+        host_in[k].copy_(t)
+    outs = {"O": buf.O, "lse": buf.lse}
+    if w.backward:
+        outs.update(dQ=buf.dQ, dK=buf.dK, dV=buf.dV)
+    for k, t in outs.items():
+        host_out[k], p = alloc_host(t.shape, t.dtype, torch)
+        pinned &= p
+        host_out[k].zero_()                                   # touch the pages before timing
+    kw = dict(Q_host=host_in["q"], K_host=host_in["k"], V_host=host_in["v"], O_host=host_out["O"], lse_host=host_out["lse"],
+              d_Q=inp["q"], d_K=inp["k"], d_V=inp["v"], d_O=buf.O, d_lse=buf.lse, d_partial_O=buf.partial_O,
+              d_partial_lse=buf.partial_lse)
+    if w.backward:
+        kw.update(dO_host=host_in["do"], dQ_host=host_out["dQ"], dK_host=host_out["dK"], dV_host=host_out["dV"], d_dO=inp["do"],
+                  d_delta=buf.delta, d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        plan.step_host(**kw)                                  # synchronises its stream before returning
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    h2d = sum(t.numel() * t.element_size() for t in host_in.values())
+    d2h = sum(t.numel() * t.element_size() for t in host_out.values())
+    return ms, h2d, d2h, pinned
+
+
+def run_ours(args):
+    import torch
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    import __graft_entry__ as entry
+
+    if rank == 0:
+        import contextlib
+
+        with contextlib.redirect_stdout(sys.stderr):
+            entry.build()
+    if dist is not None:
+        dist.barrier()
+    from paper_2512_20968_b200 import Buffers, launch_count, plan_for
+    from paper_2512_20968_b200 import binding as B
+    from paper_2512_20968_b200 import workloads as W
+
+    w = W.CONFIGS[args.workload]
+    peaks, peak_src = load_peaks()
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v", "do") if w.backward else ("q", "k", "v"))
+    plan = plan_for(w)
+    buf = Buffers(plan, w, backward=w.backward)
+
+    def step():
+        plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+        if w.backward:
+            plan.backward(inp["q"], inp["k"], inp["v"], buf.O, inp["do"], buf.lse, buf.delta, buf.dQ, buf.dK, buf.dV)
+
+    def fence():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    fence()
+    clocks = ClockSampler(physical_gpu_index(local_rank))
+    if rank == 0:
+        clocks.start()
+    B.profile_enable(True, 8192)
+    n0 = launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    fence()
+    ms_total = e0.elapsed_time(e1)
+    launches = launch_count() - n0
+    clk = clocks.stop() if rank == 0 else None
+    prof = {name: B.profile_read(kind) for name, kind in (("tile_fwd", B.K_TILE_FWD), ("merge", B.K_MERGE),
+                                                          ("bwd_preprocess", B.K_BWD_PREPROCESS), ("tile_bwd", B.K_TILE_BWD))}
+    B.profile_enable(False)
+    if dist is not None:
+        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+
+    K = args.steps
+    fl_fwd, fl_bwd = plan.query(B.Q_FLOPS_FWD), (plan.query(B.Q_FLOPS_BWD) if w.backward else 0)
+    sec = ms_total / 1e3
+    value = world * (fl_fwd + fl_bwd) * K / sec / 1e12
+
+    e2e = None
+    if not args.no_e2e:
+        try:
+            e2e_steps = 1 if ms_total / K > 2000 else min(K, 5)
+            ms_e, h2d, d2h, pinned = run_e2e(plan, w, inp, buf, torch, e2e_steps)
+            if dist is not None:
+                t = torch.tensor([ms_e], device="cuda", dtype=torch.float64)
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+                ms_e = float(t.item())
+            e2e = {"value": world * (fl_fwd + fl_bwd) / (ms_e / 1e3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+                   "d2h_bytes_per_step": d2h, "ms_per_step": ms_e, "steps": e2e_steps, "pinned": pinned,
+                   "api": "mesh_attn_step_host"}
+        except (RuntimeError, MemoryError) as ex:                # host memory too small for the host mirrors
+            e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel, per launch, from the events recorded inside the timed region
+    dom = max(("tile_fwd", "tile_bwd"), key=lambda k: prof[k][0])
+    dom_ms, dom_n = prof[dom]
+    dom_flops = (fl_fwd if dom == "tile_fwd" else fl_bwd) * K            # all launches of the timed region together
+    long_step = sec >= 2.0
+    peak = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
+    ach = dom_flops / (dom_ms / 1e3) / 1e12 if dom_ms > 0 else 0.0
+    roofline = {"kernel": f"mesh_attn_{dom}", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
+                "frac": ach / peak, "traffic": None, "launches": dom_n, "avg_launch_ms": dom_ms / max(1, dom_n),
+                "algorithmic_flops_per_launch": dom_flops / max(1, dom_n),
+                "peak_kind": f"{peak_src} dense bf16, " + ("sustained (kernel timed inside a long step)" if long_step else "burst"),
+                "share_of_step": dom_ms / ms_total}
+    kernels = {}
+    for name, (ms, n) in prof.items():
+        if n:
+            kernels[name] = {"launches": n, "ms_total": ms, "share_of_step": ms / ms_total}
+    if prof["tile_fwd"][0] > 0:
+        kernels["tile_fwd"]["tflops"] = fl_fwd * K / (prof["tile_fwd"][0] / 1e3) / 1e12
+        kernels["tile_fwd"]["frac_of_peak"] = kernels["tile_fwd"]["tflops"] / peak
+    if prof["tile_bwd"][0] > 0:
+        kernels["tile_bwd"]["tflops"] = fl_bwd * K / (prof["tile_bwd"][0] / 1e3) / 1e12
+        kernels["tile_bwd"]["frac_of_peak"] = kernels["tile_bwd"]["tflops"] / peak
+    if prof["merge"][0] > 0:
+        mbytes = plan.query(B.Q_MERGE_BYTES) * prof["merge"][1]
+        kernels["merge"]["gbs"] = mbytes / (prof["merge"][0] / 1e3) / 1e9
+        kernels["merge"]["frac_of_hbm"] = kernels["merge"]["gbs"] / peaks["hbm_gbs"]
+    fwd_ms = prof["tile_fwd"][0] + prof["merge"][0]
+    summary = {"fwd_tflops_incl_merge": fl_fwd * K / (fwd_ms / 1e3) / 1e12 if fwd_ms > 0 else None,
+               "fwd_bwd_tflops": value / world,
+               "pct_of_bf16_peak": {"measured_burst": 100 * value / world / peaks["bf16_tflops"],
+                                    "measured_sustained": 100 * value / world / peaks["bf16_tflops_sustained"],
+                                    "nominal_2250": 100 * value / world / 2250.0}}
+
+    cpu = None
+    if not args.no_cpu_baseline:
+        smp = OracleSample(w, oracle_inputs_from_device(w, inp), args.cpu_seconds)
+        dt, fl = smp.timed()
+        cpu = {"value": fl / dt / 1e12, "unit": UNIT, "cores": smp.threads, "kind": "oracle", "sample": smp.describe(),
+               "seconds": dt}
+
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
+        "ms_per_step": ms_total / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "bf16",
+        "data": "synthetic", "config": workload_config(w, "N>1: independent replicas, no collective (DESIGN.md)" if world > 1 else ""),
+        "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "kernels": kernels,
+        "summary": summary,
+    }
+    print(json.dumps(line), flush=True)
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -189,6 +189,17 @@ int mesh_attn_step_host(const mesh_attn_plan* plan, const mesh_attn_host_io* io,
 /* number of kernels launched by this library in the calling process so far (bench bookkeeping) */
 int64_t mesh_attn_launch_count(void);
 
+/* Per-kernel device timing (measurement): while enabled, every kernel launch
+ * of this library is bracketed by two cudaEventRecord calls on the launch's own stream
+ * (events come from a pool created at enable time; when the pool of `capacity` launches is
+ * full, further launches are not recorded).  mesh_attn_profile_read must be called after
+ * the caller has synchronised the stream(s): it sums cudaEventElapsedTime over the recorded
+ * launches of `kind` and returns their number.  enable(0,..) frees nothing and stops
+ * recording; enable(1, capacity) resets the records.  Not thread-safe; off by default. */
+enum { MESH_ATTN_K_TILE_FWD = 0, MESH_ATTN_K_MERGE = 1, MESH_ATTN_K_BWD_PREPROCESS = 2, MESH_ATTN_K_TILE_BWD = 3 };
+int mesh_attn_profile_enable(int32_t on, int32_t capacity);
+int mesh_attn_profile_read(int32_t kind, double* ms_total, int64_t* launches);
+
 const char* mesh_attn_strerror(int status);
 const char* mesh_attn_last_error(void); /* thread-local, valid until the next call on this thread */
 

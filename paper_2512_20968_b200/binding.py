@@ -64,6 +64,8 @@ lib.mesh_attn_forward.argtypes = [_P] * 9
 lib.mesh_attn_backward.argtypes = [_P] * 12
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
 lib.mesh_attn_launch_count.restype = C.c_int64
+lib.mesh_attn_profile_enable.argtypes = [C.c_int32, C.c_int32]
+lib.mesh_attn_profile_read.argtypes = [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
 lib.mesh_attn_strerror.restype = C.c_char_p
 lib.mesh_attn_strerror.argtypes = [C.c_int]
 lib.mesh_attn_last_error.restype = C.c_char_p
@@ -72,8 +74,9 @@ EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
-    "mesh_attn_strerror", "mesh_attn_last_error",
+    "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
 ]
+K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
 
 
 class MeshAttnError(RuntimeError):
@@ -192,6 +195,17 @@ class Plan:
                 raise TypeError(f"unknown host-io field {k}")
             setattr(io, k, _ptr(v))
         _check(lib.mesh_attn_step_host(self._h, C.byref(io), _stream(stream)))
+
+
+def profile_enable(on: bool, capacity: int = 4096):
+    _check(lib.mesh_attn_profile_enable(int(on), capacity))
+
+
+def profile_read(kind: int):
+    """(total milliseconds, launches) of the recorded launches of `kind`; synchronise the stream first."""
+    ms, cnt = C.c_double(), C.c_int64()
+    _check(lib.mesh_attn_profile_read(kind, C.byref(ms), C.byref(cnt)))
+    return ms.value, cnt.value
 
 
 def launch_count() -> int:

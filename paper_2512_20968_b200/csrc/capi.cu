@@ -5,6 +5,7 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <vector>
 
 #include "plan.hpp"
 #include "tile_kernels.hpp"
@@ -41,6 +42,30 @@ bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H)
     const uint64_t N = (uint64_t)p->geom.n * p->geom.L;
     return make_tmap_bf16_4d(m, base, p->geom.head_dim, H, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, kBlock);
 }
+
+// ---- per-kernel device timing (mesh_attn_profile_*): event pairs around each launch ----
+struct Profiler {
+    bool on = false;
+    std::vector<cudaEvent_t> ev;     // 2 per recorded launch
+    std::vector<int> kind;
+    size_t used = 0, capacity = 0;
+} g_prof;
+
+struct ProfScope {                   // records begin at construction, end at destruction, on the launch stream
+    cudaStream_t st;
+    long long slot = -1;
+    ProfScope(int kind, cudaStream_t s) : st(s)
+    {
+        if (!g_prof.on || g_prof.used >= g_prof.capacity) return;
+        slot = (long long)g_prof.used++;
+        g_prof.kind[slot] = kind;
+        cudaEventRecord(g_prof.ev[2 * slot], st);
+    }
+    ~ProfScope()
+    {
+        if (slot >= 0) cudaEventRecord(g_prof.ev[2 * slot + 1], st);
+    }
+};
 
 int check_device(const mesh_attn_plan* p, const char* who)
 {
@@ -120,6 +145,7 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     fp.g_count = g_count;
     fp.partial_O = partial_O;
     fp.partial_lse = partial_lse;
+    ProfScope prof(MESH_ATTN_K_TILE_FWD, (cudaStream_t)stream);
     const int e = launch_tile_fwd(fp, tmQ, tmK, tmV, p->num_sms, (cudaStream_t)stream);
     if (e) return cuda_fail("tile_fwd launch", e);
     g_launches.fetch_add(1);
@@ -147,6 +173,7 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
     mp.lse = lse;
     const Strides s = strides_of(p, p->geom.heads_q);
     mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
+    ProfScope prof(MESH_ATTN_K_MERGE, (cudaStream_t)stream);
     const int e = launch_merge(mp, (cudaStream_t)stream);
     if (e) return cuda_fail("merge launch", e);
     g_launches.fetch_add(1);
@@ -162,6 +189,7 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
     dp.O = O; dp.dO = dO; dp.delta = delta;
     const Strides s = strides_of(p, p->geom.heads_q);
     dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
+    ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
     const int e = launch_delta(dp, (cudaStream_t)stream);
     if (e) return cuda_fail("bwd_preprocess launch", e);
     g_launches.fetch_add(1);
@@ -193,6 +221,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     const Strides sq = strides_of(p, p->geom.heads_q), sk = strides_of(p, p->geom.heads_kv);
     bp.q_stride_b = sq.b; bp.q_stride_row = sq.row; bp.q_stride_h = sq.h;
     bp.k_stride_b = sk.b; bp.k_stride_row = sk.row; bp.k_stride_h = sk.h;
+    ProfScope prof(MESH_ATTN_K_TILE_BWD, (cudaStream_t)stream);
     const int e = launch_tile_bwd(bp, tmQ, tmK, tmV, tmdO, p->num_sms, (cudaStream_t)stream);
     if (e) return cuda_fail("tile_bwd launch", e);
     g_launches.fetch_add(1);
@@ -266,6 +295,42 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
 }
 
 int64_t mesh_attn_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int mesh_attn_profile_enable(int32_t on, int32_t capacity)
+{
+    g_prof.on = false;
+    if (!on) return MESH_ATTN_OK;
+    if (capacity <= 0) return fail(MESH_ATTN_EINVAL, "profile_enable: capacity must be positive");
+    while (g_prof.ev.size() < 2 * (size_t)capacity) {
+        cudaEvent_t e;
+        const cudaError_t rc = cudaEventCreate(&e);
+        if (rc != cudaSuccess) return cuda_fail("profile_enable: cudaEventCreate", (int)rc);
+        g_prof.ev.push_back(e);
+    }
+    g_prof.kind.assign(g_prof.ev.size() / 2, -1);
+    g_prof.capacity = (size_t)capacity;
+    g_prof.used = 0;
+    g_prof.on = true;
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_profile_read(int32_t kind, double* ms_total, int64_t* launches)
+{
+    if (!ms_total || !launches) return fail(MESH_ATTN_EINVAL, "profile_read: null pointer");
+    double total = 0.0;
+    int64_t cnt = 0;
+    for (size_t i = 0; i < g_prof.used; ++i) {
+        if (g_prof.kind[i] != kind) continue;
+        float ms = 0.f;
+        const cudaError_t rc = cudaEventElapsedTime(&ms, g_prof.ev[2 * i], g_prof.ev[2 * i + 1]);
+        if (rc != cudaSuccess) return cuda_fail("profile_read: cudaEventElapsedTime (synchronise the stream first)", (int)rc);
+        total += ms;
+        ++cnt;
+    }
+    *ms_total = total;
+    *launches = cnt;
+    return MESH_ATTN_OK;
+}
 
 const char* mesh_attn_strerror(int status)
 {
