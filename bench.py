@@ -257,7 +257,7 @@ def run_e2e(plan, w, inp, buf, torch, steps):
               d_partial_lse=buf.partial_lse)
     if w.backward:
         kw.update(dO_host=host_in["do"], dQ_host=host_out["dQ"], dK_host=host_out["dK"], dV_host=host_out["dV"], d_dO=inp["do"],
-                  d_delta=buf.delta, d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV)
+                  d_bwd_ws=buf.bwd_ws, d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV)
     torch.cuda.synchronize()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record()
@@ -309,7 +309,7 @@ def run_ours(args):
     def step():
         plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
         if w.backward:
-            plan.backward(inp["q"], inp["k"], inp["v"], buf.O, inp["do"], buf.lse, buf.delta, buf.dQ, buf.dK, buf.dV)
+            plan.backward(inp["q"], inp["k"], inp["v"], buf.O, inp["do"], buf.lse, buf.bwd_ws, buf.dQ, buf.dK, buf.dV)
 
     def fence():
         if dist is not None:

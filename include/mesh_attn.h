@@ -31,7 +31,7 @@
  *   Q, dO      bf16  [B, N, Hq,  D]   (tensor_layout 0)  or [B, Hq,  N, D] (tensor_layout 1)
  *   K, V       bf16  [B, N, Hkv, D]                      or [B, Hkv, N, D]
  *   O, dQ      fp32  same shape as Q;   dK, dV fp32 same shape as K
- *   lse, delta fp32  [B, Hq, N]   natural log of the sum of exp of the SCALED scores
+ *   lse        fp32  [B, Hq, N]   natural log of the sum of exp of the SCALED scores
  *   partial_O  fp32  [g_count][slots][B][L][Hq][D]   slots = a (partial_mode 0) or a*b (1)
  *   partial_lse fp32 [g_count][slots][B][Hq][L]
  * Token position of (p, s): seq_layout 0: p*L+s;  seq_layout 1 (striped): s*n+p.
@@ -89,7 +89,8 @@ enum {
     MESH_ATTN_Q_BWD_ITEMS_PER_GPU = 8, /* tile-backward work items per simulated GPU                      */
     MESH_ATTN_Q_BLOCKS_FWD = 9,        /* 128x128 score blocks the forward computes (all GPUs, heads)     */
     MESH_ATTN_Q_COMM_UNITS = 10,       /* paper's aggregate communication units of this AM   */
-    MESH_ATTN_Q_HAS_DEVICE = 11        /* 1 if the plan's work lists are resident on a CUDA device        */
+    MESH_ATTN_Q_HAS_DEVICE = 11,       /* 1 if the plan's work lists are resident on a CUDA device        */
+    MESH_ATTN_Q_BWD_WS_BYTES = 12      /* bytes of the backward workspace bwd_ws: 2*B*Hq*N*4               */
 };
 
 /* kinds in mesh_attn_plan_steps rows (step, kind, i, j) */
@@ -149,20 +150,24 @@ int mesh_attn_merge(const mesh_attn_plan* plan, int32_t q_group,
                     const float* partial_O, const float* partial_lse,
                     float* O, float* lse, void* stream);
 
-/* delta[b,h,row] = sum_d dO * O  (needed by every pair touching the row; the paper
- * passes O_i, dO_i to the backward kernel). All rows. */
+/* Backward workspace bwd_ws, fp32 [2][B][Hq][N] (MESH_ATTN_Q_BWD_WS_BYTES), all rows:
+ *   bwd_ws[0][b,h,row] = delta = sum_d dO * O  (needed by every pair touching the row; the
+ *                        paper passes O_i, dO_i to the backward kernel)
+ *   bwd_ws[1][b,h,row] = -lse * log2(e)  (exponent offset of P = exp(S - lse) in base 2;
+ *                        lse is the FINAL merged LSE, reading R8) */
 int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const float* O, const void* dO,
-                             float* delta, void* stream);
+                             const float* lse, float* bwd_ws, void* stream);
 
 /* Alg.3 l.3-5 for simulated GPUs g_first..: for each pair of the tile
  * recompute P = exp(S - lse) with the FINAL merged lse, dP = dO V^T, dS = P o (dP - delta),
  * and ACCUMULATE (atomic fp32 adds: the sums of Alg.3 l.6-7 and the GQA group sum)
  *   dV_v += P^T dO_u,  dK_v += scale dS^T Q_u,  dQ_u += scale dS K_v.
- * The caller zeroes dQ, dK, dV before the first call. */
+ * bwd_ws is what mesh_attn_bwd_preprocess wrote.  The caller zeroes dQ, dK, dV before the
+ * first call.  head_dim must be 128 (EUNSUPPORTED otherwise: the kernel's transposed dQ
+ * accumulator needs head_dim = 128 rows). */
 int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_count,
                        const void* Q, const void* K, const void* V, const void* dO,
-                       const float* lse, const float* delta,
-                       float* dQ, float* dK, float* dV, void* stream);
+                       const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream);
 
 /* All waves: for each Q group r: tile_fwd(g_first = r*a, a) then merge(r). partial_O /
  * partial_lse must hold `a` simulated GPUs (query PARTIAL_*_BYTES * a). */
@@ -171,7 +176,7 @@ int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, 
 
 /* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
 int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
-                       const float* O, const void* dO, const float* lse, float* delta,
+                       const float* O, const void* dO, const float* lse, float* bwd_ws,
                        float* dQ, float* dK, float* dV, void* stream);
 
 /* End-to-end step with HOST buffers (pinned or pageable): copies Q,K,V(,dO) host->device
@@ -182,7 +187,7 @@ typedef struct {
     const void *Q_host, *K_host, *V_host, *dO_host;      /* bf16 host inputs (dO_host may be NULL) */
     float *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* fp32 host outputs (any may be NULL = not copied back) */
     void *d_Q, *d_K, *d_V, *d_dO;                          /* device staging                         */
-    float *d_O, *d_lse, *d_delta, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;
+    float *d_O, *d_lse, *d_bwd_ws, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;
 } mesh_attn_host_io;
 int mesh_attn_step_host(const mesh_attn_plan* plan, const mesh_attn_host_io* io, void* stream);
 

@@ -23,7 +23,7 @@ lib = C.CDLL(str(_LIB_PATH))
 
 OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 (Q_PARTIAL_O_BYTES, Q_PARTIAL_LSE_BYTES, Q_SLOTS_PER_GPU, Q_FLOPS_FWD, Q_FLOPS_BWD, Q_WAVES, Q_MERGE_BYTES,
- Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE) = range(12)
+ Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE, Q_BWD_WS_BYTES) = range(13)
 TASK_AG_KV, TASK_AG_Q, TASK_RS_Q, TASK_C, TASK_RS_KV = range(5)
 
 
@@ -43,7 +43,7 @@ class PlanDesc(C.Structure):
 class HostIO(C.Structure):
     _fields_ = [(name, C.c_void_p) for name in (
         "Q_host", "K_host", "V_host", "dO_host", "O_host", "lse_host", "dQ_host", "dK_host", "dV_host",
-        "d_Q", "d_K", "d_V", "d_dO", "d_O", "d_lse", "d_delta", "d_dQ", "d_dK", "d_dV", "d_partial_O", "d_partial_lse")]
+        "d_Q", "d_K", "d_V", "d_dO", "d_O", "d_lse", "d_bwd_ws", "d_dQ", "d_dK", "d_dV", "d_partial_O", "d_partial_lse")]
 
 
 _P = C.c_void_p
@@ -58,8 +58,8 @@ lib.mesh_attn_plan_steps.argtypes = [_P, C.c_int32, _I32P, C.c_int32, _I32P]
 lib.mesh_attn_plan_query.argtypes = [_P, C.c_int32, C.POINTER(C.c_int64)]
 lib.mesh_attn_tile_fwd.argtypes = [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P, _P]
 lib.mesh_attn_merge.argtypes = [_P, C.c_int32, _P, _P, _P, _P, _P]
-lib.mesh_attn_bwd_preprocess.argtypes = [_P, _P, _P, _P, _P]
-lib.mesh_attn_tile_bwd.argtypes = [_P, C.c_int32, C.c_int32] + [_P] * 10
+lib.mesh_attn_bwd_preprocess.argtypes = [_P] * 6
+lib.mesh_attn_tile_bwd.argtypes = [_P, C.c_int32, C.c_int32] + [_P] * 9
 lib.mesh_attn_forward.argtypes = [_P] * 9
 lib.mesh_attn_backward.argtypes = [_P] * 12
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
@@ -174,18 +174,18 @@ class Plan:
     def merge(self, q_group, partial_O, partial_lse, O, lse, stream=None):
         _check(lib.mesh_attn_merge(self._h, q_group, _ptr(partial_O), _ptr(partial_lse), _ptr(O), _ptr(lse), _stream(stream)))
 
-    def bwd_preprocess(self, O, dO, delta, stream=None):
-        _check(lib.mesh_attn_bwd_preprocess(self._h, _ptr(O), _ptr(dO), _ptr(delta), _stream(stream)))
+    def bwd_preprocess(self, O, dO, lse, bwd_ws, stream=None):
+        _check(lib.mesh_attn_bwd_preprocess(self._h, _ptr(O), _ptr(dO), _ptr(lse), _ptr(bwd_ws), _stream(stream)))
 
-    def tile_bwd(self, g_first, g_count, Q, K, V, dO, lse, delta, dQ, dK, dV, stream=None):
-        _check(lib.mesh_attn_tile_bwd(self._h, g_first, g_count, _ptr(Q), _ptr(K), _ptr(V), _ptr(dO), _ptr(lse), _ptr(delta),
+    def tile_bwd(self, g_first, g_count, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream=None):
+        _check(lib.mesh_attn_tile_bwd(self._h, g_first, g_count, _ptr(Q), _ptr(K), _ptr(V), _ptr(dO), _ptr(bwd_ws),
                                       _ptr(dQ), _ptr(dK), _ptr(dV), _stream(stream)))
 
     def forward(self, Q, K, V, O, lse, partial_O, partial_lse, stream=None):
         _check(lib.mesh_attn_forward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _ptr(partial_O), _ptr(partial_lse), _stream(stream)))
 
-    def backward(self, Q, K, V, O, dO, lse, delta, dQ, dK, dV, stream=None):
-        _check(lib.mesh_attn_backward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(lse), _ptr(delta),
+    def backward(self, Q, K, V, O, dO, lse, bwd_ws, dQ, dK, dV, stream=None):
+        _check(lib.mesh_attn_backward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(lse), _ptr(bwd_ws),
                                       _ptr(dQ), _ptr(dK), _ptr(dV), _stream(stream)))
 
     def step_host(self, stream=None, **buffers):

@@ -1,7 +1,7 @@
 // aux_kernels.cu -- the two HBM-bound kernels of the hot path:
 //   merge_kernel   LSE-weighted merge of the partial outputs of a Q group (online-softmax
 //                  reducer of PAPER.md L77, Alg.2 l.6 L174; reading R4)
-//   delta_kernel   backward preprocess Delta = rowsum(dO o O)
+//   delta_kernel   backward preprocess Delta = rowsum(dO o O), plus -lse*log2e
 // Both are streaming kernels: 16-byte vector loads, many independent loads in flight per
 // thread, streaming cache hints, no shared-memory reuse of the bulk data.
 #include <cuda_bf16.h>
@@ -124,7 +124,14 @@ __global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) p.delta[((size_t)bt * gm.heads_q + h) * N + row] = acc;
+    if (lane == 0) {
+        const size_t at = ((size_t)bt * gm.heads_q + h) * N + row;
+        const float l = p.lse[at];
+        p.ws[at] = acc;
+        // exponent offset of the backward's P = exp2(S*scale*log2e - lse*log2e); a row without visible keys
+        // (lse = -inf) only ever meets masked positions: any finite value does
+        p.ws[(size_t)gm.batch * gm.heads_q * N + at] = (l == -INFINITY) ? 0.f : -l * 1.4426950408889634f;
+    }
 }
 
 }  // namespace

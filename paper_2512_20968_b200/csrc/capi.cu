@@ -180,13 +180,13 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
     return MESH_ATTN_OK;
 }
 
-int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void* dO, float* delta, void* stream)
+int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void* dO, const float* lse, float* bwd_ws, void* stream)
 {
     if (int rc = check_device(p, "bwd_preprocess")) return rc;
-    if (!O || !dO || !delta) return fail(MESH_ATTN_EINVAL, "bwd_preprocess: null pointer");
+    if (!O || !dO || !lse || !bwd_ws) return fail(MESH_ATTN_EINVAL, "bwd_preprocess: null pointer");
     DeltaParams dp;
     dp.gm = p->geom;
-    dp.O = O; dp.dO = dO; dp.delta = delta;
+    dp.O = O; dp.dO = dO; dp.lse = lse; dp.ws = bwd_ws;
     const Strides s = strides_of(p, p->geom.heads_q);
     dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
@@ -197,10 +197,11 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
 }
 
 int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
-                       const void* dO, const float* lse, const float* delta, float* dQ, float* dK, float* dV, void* stream)
+                       const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
 {
     if (int rc = check_device(p, "tile_bwd")) return rc;
-    if (!Q || !K || !V || !dO || !lse || !delta || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
+    if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
+    if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "tile_bwd: the backward kernel is built for head_dim 128 only");
     if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds");
     if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
     CUtensorMap tmQ, tmK, tmV, tmdO;
@@ -216,7 +217,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     bp.g_first = g_first;
     bp.g_count = g_count;
     bp.split = p->desc.precision;
-    bp.lse = lse; bp.delta = delta;
+    bp.ws = bwd_ws;
     bp.dQ = dQ; bp.dK = dK; bp.dV = dV;
     const Strides sq = strides_of(p, p->geom.heads_q), sk = strides_of(p, p->geom.heads_kv);
     bp.q_stride_b = sq.b; bp.q_stride_row = sq.row; bp.q_stride_h = sq.h;
@@ -240,9 +241,10 @@ int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, con
 }
 
 int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const float* O, const void* dO,
-                       const float* lse, float* delta, float* dQ, float* dK, float* dV, void* stream)
+                       const float* lse, float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
 {
     if (int rc = check_device(p, "backward")) return rc;
+    if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "backward: the backward kernel is built for head_dim 128 only");
     if (!dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward: null pointer");
     const Geom& gm = p->geom;
     const size_t N = (size_t)gm.n * gm.L;
@@ -251,10 +253,10 @@ int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, co
     if (e == cudaSuccess) e = cudaMemsetAsync(dK, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
     if (e == cudaSuccess) e = cudaMemsetAsync(dV, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
     if (e != cudaSuccess) return cuda_fail("backward memset", (int)e);
-    if (int rc = mesh_attn_bwd_preprocess(p, O, dO, delta, stream)) return rc;
+    if (int rc = mesh_attn_bwd_preprocess(p, O, dO, lse, bwd_ws, stream)) return rc;
     // keep each launch's work-item count below 2^31: one call per Q group
     for (int r = 0; r < gm.b; ++r)
-        if (int rc = mesh_attn_tile_bwd(p, r * gm.a, gm.a, Q, K, V, dO, lse, delta, dQ, dK, dV, stream)) return rc;
+        if (int rc = mesh_attn_tile_bwd(p, r * gm.a, gm.a, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream)) return rc;
     return MESH_ATTN_OK;
 }
 
@@ -274,13 +276,13 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
     if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, st);
     const bool bwd = io->dO_host != nullptr;
     if (bwd) {
-        if (!io->d_dO || !io->d_delta || !io->d_dQ || !io->d_dK || !io->d_dV) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
+        if (!io->d_dO || !io->d_bwd_ws || !io->d_dQ || !io->d_dK || !io->d_dV) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
         if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_dO, io->dO_host, nq * 2, cudaMemcpyHostToDevice, st);
     }
     if (e != cudaSuccess) return cuda_fail("step_host H2D", (int)e);
     if (int rc = mesh_attn_forward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_lse, io->d_partial_O, io->d_partial_lse, stream)) return rc;
     if (bwd)
-        if (int rc = mesh_attn_backward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_dO, io->d_lse, io->d_delta, io->d_dQ, io->d_dK, io->d_dV, stream))
+        if (int rc = mesh_attn_backward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_dO, io->d_lse, io->d_bwd_ws, io->d_dQ, io->d_dK, io->d_dV, stream))
             return rc;
     if (io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * 4, cudaMemcpyDeviceToHost, st);
     if (e == cudaSuccess && io->lse_host) e = cudaMemcpyAsync(io->lse_host, io->d_lse, nl * 4, cudaMemcpyDeviceToHost, st);

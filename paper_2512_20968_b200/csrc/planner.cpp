@@ -401,6 +401,7 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             break;
         }
         case MESH_ATTN_Q_HAS_DEVICE: *value = p->d_blob ? 1 : 0; break;
+        case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * gm.heads_q * (int64_t)gm.n * gm.L * 4; break;
         default: return fail(MESH_ATTN_EINVAL, "plan_query: unknown query");
     }
     return MESH_ATTN_OK;

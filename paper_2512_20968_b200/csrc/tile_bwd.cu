@@ -6,21 +6,32 @@
 // shared memory and dK, dV in TMEM, and streams 128-row Q / dO blocks of every Q partition
 // of the tile (and every query head of the GQA group).  Per Q block, five tcgen05 MMAs:
 //
-//   S^T  = K Q^T            (TMEM columns   0..127)      P^T = exp2(S^T*c - lse)  (bf16, over S^T)
-//   dP^T = V dO^T           (TMEM columns 128..255)      dS^T = P^T o (dP^T - delta) (bf16, smem)
+//   S^T  = K Q^T            (TMEM columns   0..127)      P^T = exp2(S^T*c - lse*log2e)  (bf16, over S^T)
+//   dP^T = V dO^T           (TMEM columns 128..255)      dS^T = P^T o (dP^T - delta)    (bf16, smem)
 //   dV  += P^T  dO          (TMEM columns 384..511)      A operand P^T straight from TMEM
 //   dK  += dS^T Q           (TMEM columns 256..383)      A operand dS^T from smem (K-major)
-//   dQ   = dS K             (TMEM columns 128..255, reusing dP^T once consumed)
-//                                                        A operand the same smem buffer read M-major
+//   dQ^T = K^T dS^T         (TMEM columns 128..255, reusing dP^T once consumed)
+//                                                        A = K tile read M-major, B = dS^T read N-major
 //
-//   warp 0      TMA producer: K,V per item; Q, dO, lse, delta per step through a 2-stage ring
+// dQ is produced TRANSPOSED (TMEM lane = head-dim index d, column = query) so that the drain's
+// `red.global.add.f32` has the 32 lanes of a warp on 32 consecutive floats of one dQ row: full
+// 128-byte lines per request.  (With lane = query row the same reduction is 32 scattered 16-byte
+// atomics per instruction and L2 tops out at 2.9 TB/s instead of 6.4 TB/s; profiles/r01_v1_README.md.)
+//
+//   warp 0      TMA producer: K,V per item; Q, dO, -lse*log2e, delta per step through a ring
 //   warp 1      MMA issuer (one thread)
 //   warp 2      TMEM allocator
-//   warps 4-7   one key row per thread: S^T -> P^T, dP^T -> dS^T; dK epilogue
-//   warps 8-11  one query row per thread: dQ drain (x scale, red.global.add); dV epilogue
+//   warps 4-7   compute group 0: key row = TMEM lane, query columns  0..63  of the block
+//   warps 8-11  compute group 1: key row = TMEM lane, query columns 64..127
+//               each: S^T -> P^T (regs + TMEM), dP^T -> dS^T (smem), dQ^T drain (x scale, atomics);
+//               epilogue: group 0 drains dK, group 1 drains dV
 //
-// dQ, dK, dV are accumulated into global fp32 with vector atomics: the sums over the Q group,
-// the KV group (Alg.3 l.6-7, L254-255) and the GQA head group all land in the same buffers.
+// dQ, dK, dV are accumulated into global fp32 with atomics: the sums over the Q group, the KV
+// group (Alg.3 l.6-7, L254-255) and the GQA head group all land in the same buffers.
+//
+// kSplit (plan precision = 1): P and dS are fed to the tensor core as hi + lo bf16 pairs (two
+// MMAs each for dV, dK, dQ^T), which brings the operand rounding from 2^-9 to 2^-17 relative;
+// needed when |dS| is large (outlier scores, BASELINE.json configs[2]).
 #include <cuda_bf16.h>
 
 #include "plan.hpp"
@@ -33,18 +44,19 @@ using namespace sm100;
 namespace {
 
 constexpr int kBwdThreads = 384;
-constexpr float kLog2e = 1.4426950408889634f;
 
-template <int D> struct BwdCfg {
+template <int D, bool kSplit> struct BwdCfg {
+    static_assert(D == 128, "backward kernel: dQ^T needs head_dim = UMMA M = 128");
     static constexpr int kBoxes = D / 64;
     static constexpr int kTileBytes = kBlock * D * 2;          // [128 x D] bf16
     static constexpr int kDsBytes = kBlock * kBlock * 2;        // dS^T [128 kv x 128 q] bf16
-    static constexpr int kStages = 2;
+    static constexpr int kNumDs = kSplit ? 2 : 1;               // hi (+ lo)
+    static constexpr int kStages = kSplit ? 1 : 2;              // split mode trades the second Q/dO stage for the dS lo tile
     static constexpr int kOffK = 0;
     static constexpr int kOffV = kTileBytes;
     static constexpr int kOffStage = 2 * kTileBytes;            // per stage: Q tile, dO tile
     static constexpr int kOffDs = kOffStage + kStages * 2 * kTileBytes;
-    static constexpr int kOffVec = kOffDs + kDsBytes;           // per stage: lse[128], delta[128] fp32
+    static constexpr int kOffVec = kOffDs + kNumDs * kDsBytes;  // per stage: -lse*log2e [128], delta[128] fp32
     static constexpr int kOffBars = kOffVec + kStages * 1024;
     static constexpr int kNumBars = 2 + 2 * kStages + 8;
     static constexpr int kSmemBytes = kOffBars + kNumBars * 8 + 16;
@@ -112,10 +124,19 @@ __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float 
 {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
-__device__ __forceinline__ float bf16lo(uint32_t w) { return __uint_as_float(w << 16); }
-__device__ __forceinline__ float bf16hi(uint32_t w) { return __uint_as_float(w & 0xffff0000u); }
+__device__ __forceinline__ void red_add(float* addr, float a)
+{
+    asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
+}
+// hi = bf16(x), lo = bf16(x - hi): packs two values' hi parts and lo parts
+__device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t& hi, uint32_t& lo)
+{
+    hi = pack_bf16x2(x0, x1);
+    lo = pack_bf16x2(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xffff0000u));
+}
 
 // TMEM accumulator [128 lanes x D columns] -> x scale -> atomic add into a global row of D floats
+// (item epilogue only: once per 128-key block)
 template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, float* grow, float scale)
 {
 #pragma unroll 1
@@ -130,12 +151,12 @@ template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, floa
     }
 }
 
-template <int D>
+template <int D, bool kSplit>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmdO, const BwdParams p)
 {
-    using Cfg = BwdCfg<D>;
+    using Cfg = BwdCfg<D, kSplit>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sK = smem + Cfg::kOffK;
     uint8_t* sV = smem + Cfg::kOffV;
@@ -163,6 +184,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const Geom& gm = p.gm;
     const int total_items = p.items_per_gpu * p.g_count;
     const long long N = (long long)gm.n * gm.L;
+    constexpr int kCompute = 2 * kBlock;                // threads of the two compute groups
 
     if (threadIdx.x == 0) {
         if (smem_u32(smem) & 1023u) { printf("mesh_attn tile_bwd: dynamic smem base not 1024-byte aligned\n"); __trap(); }
@@ -171,13 +193,13 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(kv_empty, 1);
         for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&qd_full[s], 1); mbar_init(&qd_empty[s], 1); }
         mbar_init(s_full, 1);
-        mbar_init(p_full, kBlock);
+        mbar_init(p_full, kCompute);
         mbar_init(dp_full, 1);
-        mbar_init(ds_full, kBlock);
+        mbar_init(ds_full, kCompute);
         mbar_init(dq_full, 1);
-        mbar_init(dq_empty, kBlock);
+        mbar_init(dq_empty, kCompute);
         mbar_init(dkv_full, 1);
-        mbar_init(dkv_empty, 2 * kBlock);
+        mbar_init(dkv_empty, kCompute);
         fence_mbar_init();
     }
     if (warp == 2) tmem_alloc<512>(tmem_slot);
@@ -190,6 +212,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // =============================== TMA producer ===============================
         if (lane == 0) {
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0;
+            const float* nlse = p.ws + (size_t)gm.batch * gm.heads_q * N;      // ws[1] = -lse*log2e
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
@@ -214,8 +237,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         tma_load_4d(sdO(stage) + bx * (kBlock * 128), &tmdO, &qd_full[stage], bx * 64, h, row, c.it.batch, kEvictLast);
                     }
                     const size_t vec = ((size_t)c.it.batch * gm.heads_q + h) * N + row;
-                    bulk_load(sLse(stage), p.lse + vec, 512, &qd_full[stage]);
-                    bulk_load(sDelta(stage), p.delta + vec, 512, &qd_full[stage]);
+                    bulk_load(sLse(stage), nlse + vec, 512, &qd_full[stage]);
+                    bulk_load(sDelta(stage), p.ws + vec, 512, &qd_full[stage]);
                     if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
                 }
             }
@@ -223,9 +246,9 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else if (warp == 1) {
         // =============================== MMA issuer ===============================
         if (lane == 0) {
-            constexpr uint32_t idesc_kk = umma_idesc(kBlock, kBlock, false, false);   // S^T, dP^T
-            constexpr uint32_t idesc_tn = umma_idesc(kBlock, D, false, true);         // dV (A in TMEM), dK (A smem K-major)
-            constexpr uint32_t idesc_nn = umma_idesc(kBlock, D, true, true);          // dQ (A smem M-major)
+            constexpr uint32_t idesc_kk = umma_idesc(kBlock, kBlock, false, false);   // S^T, dP^T: both operands K-major over head_dim
+            constexpr uint32_t idesc_tn = umma_idesc(kBlock, D, false, true);         // dV (A in TMEM), dK (A smem K-major); B row-major [q x d]
+            constexpr uint32_t idesc_nn = umma_idesc(D, kBlock, true, true);          // dQ^T: A = K tile M-major, B = dS^T N-major
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0, p_ph = 0, ds_ph = 0, dqe_ph = 0, dkve_ph = 0;
             const uint32_t aK = smem_u32(sK), aV = smem_u32(sV), aDs = smem_u32(sDs);
             auto mma_kmajor = [&](uint32_t dcol, uint32_t a, uint32_t b) {          // D = A B^T, both K-major over head_dim
@@ -235,61 +258,71 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     umma_ss(tmem + dcol, umma_desc(a + o, 16, 1024), umma_desc(b + o, 16, 1024), idesc_kk, kk > 0);
                 }
             };
+            auto next_stage = [&]() {                                                // wait for the next Q/dO stage, return its slot
+                mbar_wait(&qd_full[stage], ring_phase);
+                tc_fence_after();
+                const uint32_t st = stage;
+                if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
+                return st;
+            };
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
                 int u, h, s0, off, i = 0;
-                uint32_t st_cur = 0;
                 bool have = walk.next(u, h, s0, off);
                 if (!have) continue;
                 mbar_wait(kv_full, kv_phase);
                 kv_phase ^= 1;
                 mbar_wait(dkv_empty, dkve_ph ^ 1);      // previous item's dK/dV drained from TMEM
                 dkve_ph ^= 1;
-                // prologue: S^T(0), dP^T(0)
-                mbar_wait(&qd_full[stage], ring_phase);
-                tc_fence_after();
-                st_cur = stage;
+                uint32_t st_cur = next_stage();         // prologue: S^T(0), dP^T(0)
                 mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_cur)));
                 umma_commit(s_full);
                 mma_kmajor(Cfg::kColDP, aV, smem_u32(sdO(st_cur)));
                 umma_commit(dp_full);
-                if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
                 while (have) {
                     const bool more = walk.next(u, h, s0, off);
                     const uint32_t aQ = smem_u32(sQ(st_cur)), adO = smem_u32(sdO(st_cur));
-                    // dV += P^T dO
+                    // dV += P^T dO   (P^T bf16 in TMEM: group w's 64 queries at columns 64w.. (hi) and 64w+32.. (lo))
                     mbar_wait(p_full, p_ph);
                     p_ph ^= 1;
                     tc_fence_after();
 #pragma unroll
-                    for (int kk = 0; kk < kBlock / 16; ++kk)
-                        umma_ts(tmem + Cfg::kColDV, tmem + Cfg::kColS + kk * 8, umma_desc(adO + kk * 2048, kBlock * 128, 1024), idesc_tn,
-                                (i > 0 || kk > 0) ? 1u : 0u);
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
+#pragma unroll
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ts(tmem + Cfg::kColDV, tmem + Cfg::kColS + (kk >> 2) * 64 + x * 32 + (kk & 3) * 8,
+                                    umma_desc(adO + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
                     uint32_t st_next = 0;
-                    if (more) {                          // S^T(i+1) as early as possible
-                        mbar_wait(&qd_full[stage], ring_phase);
-                        tc_fence_after();
-                        st_next = stage;
-                        if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
+                    if (Cfg::kStages > 1 && more) {      // S^T(i+1) as early as possible
+                        st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
                         umma_commit(s_full);
                     }
-                    // dK += dS^T Q ; dQ = dS K
+                    // dQ^T = K^T dS^T (first: its drain overlaps the dK MMA) ; dK += dS^T Q
                     mbar_wait(ds_full, ds_ph);
                     ds_ph ^= 1;
                     tc_fence_after();
 #pragma unroll
-                    for (int kk = 0; kk < kBlock / 16; ++kk)
-                        umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
-                                umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0) ? 1u : 0u);
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
-                    for (int kk = 0; kk < kBlock / 16; ++kk)
-                        umma_ss(tmem + Cfg::kColDP, umma_desc(aDs + kk * 2048, kBlock * 128, 1024), umma_desc(aK + kk * 2048, kBlock * 128, 1024),
-                                idesc_nn, kk > 0);
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
+                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
                     umma_commit(dq_full);
+#pragma unroll
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
+#pragma unroll
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
+                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
                     umma_commit(&qd_empty[st_cur]);
-                    if (more) {                          // dP^T(i+1) once dQ(i) has left TMEM
+                    if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
+                        st_next = next_stage();
+                        mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
+                        umma_commit(s_full);
+                    }
+                    if (more) {                          // dP^T(i+1) once dQ^T(i) has left TMEM
                         mbar_wait(dq_empty, dqe_ph);
                         dqe_ph ^= 1;
                         tc_fence_after();
@@ -307,134 +340,155 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 }
             }
         }
-    } else if (warp >= 4 && warp < 8) {
-        // =============================== S^T -> P^T, dP^T -> dS^T (one key row per thread) ===============================
-        const int row = threadIdx.x - 128;
+    } else if (warp >= 4) {
+        // =============================== compute groups ===============================
+        // thread = (key row `row` = TMEM lane, query-column half `wg`): 64 elements of S^T / dP^T per step
+        const int wg = (warp - 4) >> 2;
+        const int row = ((warp & 3) << 5) | lane;
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t tS = tmem + lane_base + Cfg::kColS, tDP = tmem + lane_base + Cfg::kColDP, tDK = tmem + lane_base + Cfg::kColDK;
+        const uint32_t tS = tmem + lane_base + Cfg::kColS + wg * 64;      // S^T columns of this half; P^T (bf16) is written over them
+        const uint32_t tDP = tmem + lane_base + Cfg::kColDP + wg * 64;    // dP^T columns of this half; later dQ^T (lane = d, column = query)
+        uint8_t* sDsHalf = sDs + wg * (kBlock * 128);                     // [128 key rows][64 queries] bf16, 128-byte swizzled rows
         uint32_t stage = 0, ring_phase = 0, s_ph = 0, dp_ph = 0, dq_ph = 0, dkv_ph = 0;
-        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
-            const BwdItemCtx c = load_bwd_item(p, idx);
-            QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-            int u, h, s0, off, i = 0;
-            while (walk.next(u, h, s0, off)) {
-                mbar_wait(&qd_full[stage], ring_phase);   // lse / delta of this step landed (bulk copies on the same barrier)
-                const float* lse = sLse(stage);
-                const float* delta = sDelta(stage);
-                // query column cq of this block is visible to key row `row` iff cq >= cmin
-                const int cmin = c.it.t0 + row - off - s0;
-                const bool masked = gm.causal && (c.it.t0 + kBlock - 1 - off - s0 > 0);
-                uint32_t pk[kBlock / 2];
-                mbar_wait(s_full, s_ph);
-                s_ph ^= 1;
-                tc_fence_after();
-#pragma unroll
-                for (int ch = 0; ch < kBlock / 32; ++ch) {
-                    uint32_t r[32];
-                    tmem_ld_x32(tS + ch * 32, r);
-                    tmem_ld_wait();
-#pragma unroll
-                    for (int q4 = 0; q4 < 32; q4 += 4) {
-                        const float4 l4 = *reinterpret_cast<const float4*>(lse + ch * 32 + q4);
-                        float p0 = ex2(fmaf(__uint_as_float(r[q4 + 0]), gm.scale_log2, -l4.x * kLog2e));
-                        float p1 = ex2(fmaf(__uint_as_float(r[q4 + 1]), gm.scale_log2, -l4.y * kLog2e));
-                        float p2 = ex2(fmaf(__uint_as_float(r[q4 + 2]), gm.scale_log2, -l4.z * kLog2e));
-                        float p3 = ex2(fmaf(__uint_as_float(r[q4 + 3]), gm.scale_log2, -l4.w * kLog2e));
-                        if (masked) {
-                            const int cq = ch * 32 + q4;
-                            if (cq + 0 < cmin) p0 = 0.f;
-                            if (cq + 1 < cmin) p1 = 0.f;
-                            if (cq + 2 < cmin) p2 = 0.f;
-                            if (cq + 3 < cmin) p3 = 0.f;
-                        }
-                        pk[ch * 16 + q4 / 2] = pack_bf16x2(p0, p1);
-                        pk[ch * 16 + q4 / 2 + 1] = pack_bf16x2(p2, p3);
-                    }
-                    tmem_st_x16(tS + ch * 16, *reinterpret_cast<uint32_t(*)[16]>(&pk[ch * 16]));
-                }
-                tmem_st_wait();
-                tc_fence_before();
-                mbar_arrive(p_full);
+        float pr[64];                                                     // P^T of the current step (fp32), reused for dS^T
 
-                mbar_wait(dp_full, dp_ph);
-                dp_ph ^= 1;
-                if (i > 0) { mbar_wait(dq_full, dq_ph); dq_ph ^= 1; }     // dS buffer free: dK/dQ MMAs of the previous step done
-                tc_fence_after();
+        auto next_stage = [&]() {
+            mbar_wait(&qd_full[stage], ring_phase);                       // Q/dO tiles and the -lse*log2e / delta vectors landed
+            const uint32_t st = stage;
+            if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
+            return st;
+        };
+        // P^T = exp2(S^T * scale*log2e - lse*log2e), causal mask on blocks that straddle the diagonal only
+        auto compute_P = [&](uint32_t st, int t0, int s0, int off) {
+            const float4* nl4 = reinterpret_cast<const float4*>(sLse(st) + wg * 64);
+            const bool masked = gm.causal && (t0 + kBlock - 1 - off - s0 > 0);     // block-uniform
+            mbar_wait(s_full, s_ph);
+            s_ph ^= 1;
+            tc_fence_after();
 #pragma unroll
-                for (int ch = 0; ch < kBlock / 32; ++ch) {
-                    uint32_t r[32];
-                    tmem_ld_x32(tDP + ch * 32, r);
-                    tmem_ld_wait();
-                    uint8_t* half = sDs + (ch / 2) * (kBlock * 128);
+            for (int ch = 0; ch < 2; ++ch) {
+                uint32_t r[32];
+                tmem_ld_x32(tS + ch * 32, r);
+                tmem_ld_wait();
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {                          // 8 columns = one 16-byte chunk
-                        uint32_t w[4];
+                for (int q4 = 0; q4 < 32; q4 += 4) {
+                    const float4 l4 = nl4[ch * 8 + q4 / 4];
+                    pr[ch * 32 + q4 + 0] = ex2(fmaf(__uint_as_float(r[q4 + 0]), gm.scale_log2, l4.x));
+                    pr[ch * 32 + q4 + 1] = ex2(fmaf(__uint_as_float(r[q4 + 1]), gm.scale_log2, l4.y));
+                    pr[ch * 32 + q4 + 2] = ex2(fmaf(__uint_as_float(r[q4 + 2]), gm.scale_log2, l4.z));
+                    pr[ch * 32 + q4 + 3] = ex2(fmaf(__uint_as_float(r[q4 + 3]), gm.scale_log2, l4.w));
+                }
+            }
+            if (masked) {
+                const int cmin = t0 + row - off - s0 - wg * 64;            // local query column c visible to this key iff c >= cmin
 #pragma unroll
-                        for (int j = 0; j < 4; ++j) {
-                            const int cq = ch * 32 + k * 8 + j * 2;
-                            const uint32_t pw = pk[cq / 2];
-                            const float d0 = bf16lo(pw) * (__uint_as_float(r[k * 8 + j * 2]) - delta[cq]);
-                            const float d1 = bf16hi(pw) * (__uint_as_float(r[k * 8 + j * 2 + 1]) - delta[cq + 1]);
-                            w[j] = pack_bf16x2(d0, d1);
-                        }
-                        *reinterpret_cast<uint4*>(half + sw128_offset(row, (ch & 1) * 4 + k)) = make_uint4(w[0], w[1], w[2], w[3]);
+                for (int c = 0; c < 64; ++c) if (c < cmin) pr[c] = 0.f;
+            }
+            // all 64 S^T columns of this half are in registers: P^T may now overwrite them
+            if constexpr (!kSplit) {
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    uint32_t pk[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) pk[j] = pack_bf16x2(pr[hf * 32 + 2 * j], pr[hf * 32 + 2 * j + 1]);
+                    tmem_st_x16(tS + hf * 16, pk);
+                }
+            } else {
+#pragma unroll
+                for (int hf = 0; hf < 2; ++hf) {
+                    uint32_t hi[16], lo[16];
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) split_bf16x2(pr[hf * 32 + 2 * j], pr[hf * 32 + 2 * j + 1], hi[j], lo[j]);
+                    tmem_st_x16(tS + hf * 16, hi);
+                    tmem_st_x16(tS + 32 + hf * 16, lo);
+                }
+            }
+            tmem_st_wait();
+            tc_fence_before();
+            mbar_arrive(p_full);
+        };
+        // dS^T = P^T o (dP^T - delta) -> bf16 -> smem (K-major rows for dK, read N-major for dQ^T)
+        auto compute_dS = [&](uint32_t st) {
+            const float4* dl4 = reinterpret_cast<const float4*>(sDelta(st) + wg * 64);
+            mbar_wait(dp_full, dp_ph);           // also: dQ^T / dK of the previous step have finished reading the dS tile
+            dp_ph ^= 1;
+            tc_fence_after();
+#pragma unroll
+            for (int ch = 0; ch < 2; ++ch) {
+                uint32_t r[32];
+                tmem_ld_x32(tDP + ch * 32, r);
+                tmem_ld_wait();
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {                              // 8 columns = one 16-byte chunk of the row
+                    const float4 da = dl4[ch * 8 + k * 2], db = dl4[ch * 8 + k * 2 + 1];
+                    const int c = ch * 32 + k * 8;
+                    const float d0 = pr[c + 0] * (__uint_as_float(r[k * 8 + 0]) - da.x), d1 = pr[c + 1] * (__uint_as_float(r[k * 8 + 1]) - da.y);
+                    const float d2 = pr[c + 2] * (__uint_as_float(r[k * 8 + 2]) - da.z), d3 = pr[c + 3] * (__uint_as_float(r[k * 8 + 3]) - da.w);
+                    const float d4 = pr[c + 4] * (__uint_as_float(r[k * 8 + 4]) - db.x), d5 = pr[c + 5] * (__uint_as_float(r[k * 8 + 5]) - db.y);
+                    const float d6 = pr[c + 6] * (__uint_as_float(r[k * 8 + 6]) - db.z), d7 = pr[c + 7] * (__uint_as_float(r[k * 8 + 7]) - db.w);
+                    const uint32_t o = sw128_offset(row, ch * 4 + k);
+                    if constexpr (!kSplit) {
+                        *reinterpret_cast<uint4*>(sDsHalf + o) =
+                            make_uint4(pack_bf16x2(d0, d1), pack_bf16x2(d2, d3), pack_bf16x2(d4, d5), pack_bf16x2(d6, d7));
+                    } else {
+                        uint32_t h0, h1, h2, h3, l0, l1, l2, l3;
+                        split_bf16x2(d0, d1, h0, l0); split_bf16x2(d2, d3, h1, l1);
+                        split_bf16x2(d4, d5, h2, l2); split_bf16x2(d6, d7, h3, l3);
+                        *reinterpret_cast<uint4*>(sDsHalf + o) = make_uint4(h0, h1, h2, h3);
+                        *reinterpret_cast<uint4*>(sDsHalf + Cfg::kDsBytes + o) = make_uint4(l0, l1, l2, l3);
                     }
                 }
-                fence_proxy_async_smem();
-                tc_fence_before();
-                mbar_arrive(ds_full);
-                if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
-                ++i;
             }
-            if (i == 0) continue;
-            mbar_wait(dq_full, dq_ph);           // last step's dq_full (not consumed above)
-            dq_ph ^= 1;
-            // epilogue: dK rows (x softmax scale)
-            mbar_wait(dkv_full, dkv_ph);
-            dkv_ph ^= 1;
-            tc_fence_after();
-            float* grow = p.dK + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
-                          (size_t)c.it.head_kv * p.k_stride_h;
-            drain_rows<D>(tDK, grow, gm.scale);
+            fence_proxy_async_smem();
             tc_fence_before();
-            mbar_arrive(dkv_empty);
-        }
-    } else if (warp >= 8) {
-        // =============================== dQ drain (one query row per thread); dV epilogue ===============================
-        const int row = threadIdx.x - 256;
-        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
-        const uint32_t tDQ = tmem + lane_base + Cfg::kColDP, tDV = tmem + lane_base + Cfg::kColDV;
-        uint32_t dq_ph = 0, dkv_ph = 0;
+            mbar_arrive(ds_full);
+        };
+        // dQ^T (lane = d, columns = the 64 queries of this half) -> x scale -> one coalesced atomic per (query, 32 d's)
+        auto drain_dQ = [&](int batch, int u, int h, int s0) {
+            float* base = p.dQ + (size_t)batch * p.q_stride_b + ((size_t)u * gm.L + s0 + wg * 64) * p.q_stride_row + (size_t)h * p.q_stride_h + row;
+            mbar_wait(dq_full, dq_ph);
+            dq_ph ^= 1;
+            tc_fence_after();
+            uint32_t r[32];                      // two 32-column halves in turn: P^T of the next step is live in registers
+            tmem_ld_x32(tDP, r);
+            tmem_ld_wait();
+#pragma unroll
+            for (int j = 0; j < 32; ++j) red_add(base + (size_t)j * p.q_stride_row, __uint_as_float(r[j]) * gm.scale);
+            tmem_ld_x32(tDP + 32, r);
+            tmem_ld_wait();
+            tc_fence_before();
+            mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
+#pragma unroll
+            for (int j = 0; j < 32; ++j) red_add(base + (size_t)(32 + j) * p.q_stride_row, __uint_as_float(r[j]) * gm.scale);
+        };
+
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-            int u, h, s0, off, i = 0;
-            while (walk.next(u, h, s0, off)) {
-                float* grow = p.dQ + (size_t)c.it.batch * p.q_stride_b + ((size_t)u * gm.L + s0 + row) * p.q_stride_row + (size_t)h * p.q_stride_h;
-                mbar_wait(dq_full, dq_ph);
-                dq_ph ^= 1;
-                tc_fence_after();
-                uint32_t r[D / 32][32];
-#pragma unroll
-                for (int ch = 0; ch < D / 32; ++ch) tmem_ld_x32(tDQ + ch * 32, r[ch]);
-                tmem_ld_wait();
-                tc_fence_before();
-                mbar_arrive(dq_empty);           // TMEM columns free again: dP^T of the next step may start
-#pragma unroll
-                for (int ch = 0; ch < D / 32; ++ch)
-#pragma unroll
-                    for (int k = 0; k < 32; k += 4)
-                        red_add_v4(grow + ch * 32 + k, __uint_as_float(r[ch][k]) * gm.scale, __uint_as_float(r[ch][k + 1]) * gm.scale,
-                                   __uint_as_float(r[ch][k + 2]) * gm.scale, __uint_as_float(r[ch][k + 3]) * gm.scale);
-                ++i;
+            int u, h, s0, off;
+            bool have = walk.next(u, h, s0, off);
+            if (!have) continue;
+            uint32_t st_cur = next_stage();
+            compute_P(st_cur, c.it.t0, s0, off);
+            while (have) {
+                int un, hn, s0n, offn;
+                const bool more = walk.next(un, hn, s0n, offn);
+                compute_dS(st_cur);
+                if (more) {
+                    st_cur = next_stage();
+                    compute_P(st_cur, c.it.t0, s0n, offn);
+                }
+                drain_dQ(c.it.batch, u, h, s0);
+                u = un; h = hn; s0 = s0n; off = offn;
+                have = more;
             }
-            if (i == 0) continue;
+            // epilogue: group 0 drains dK (x softmax scale), group 1 drains dV
             mbar_wait(dkv_full, dkv_ph);
             dkv_ph ^= 1;
             tc_fence_after();
-            float* grow = p.dV + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
+            float* grow = (wg == 0 ? p.dK : p.dV) + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
                           (size_t)c.it.head_kv * p.k_stride_h;
-            drain_rows<D>(tDV, grow, 1.0f);
+            drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? gm.scale : 1.0f);
             tc_fence_before();
             mbar_arrive(dkv_empty);
         }
@@ -445,26 +499,28 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == 2) tmem_dealloc<512>(tmem);
 }
 
+template <int D, bool kSplit>
+int launch_one(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmdO, int grid,
+               cudaStream_t stream)
+{
+    using Cfg = BwdCfg<D, kSplit>;
+    static_assert(Cfg::kSmemBytes <= 227 * 1024, "tile_bwd shared memory over the 227 KB CTA limit");
+    cudaError_t e = cudaFuncSetAttribute(tile_bwd_kernel<D, kSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
+    if (e != cudaSuccess) return (int)e;
+    tile_bwd_kernel<D, kSplit><<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(tmQ, tmK, tmV, tmdO, p);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace
 
 int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmdO,
                     int num_sms, cudaStream_t stream)
 {
-    if (p.split) return (int)cudaErrorNotSupported;
+    if (p.gm.head_dim != 128) return (int)cudaErrorNotSupported;     // capi.cu reports EUNSUPPORTED before getting here
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
-    cudaError_t e;
-    if (p.gm.head_dim == 128) {
-        e = cudaFuncSetAttribute(tile_bwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<128>::kSmemBytes);
-        if (e != cudaSuccess) return (int)e;
-        tile_bwd_kernel<128><<<grid, kBwdThreads, BwdCfg<128>::kSmemBytes, stream>>>(tmQ, tmK, tmV, tmdO, p);
-    } else {
-        e = cudaFuncSetAttribute(tile_bwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, BwdCfg<64>::kSmemBytes);
-        if (e != cudaSuccess) return (int)e;
-        tile_bwd_kernel<64><<<grid, kBwdThreads, BwdCfg<64>::kSmemBytes, stream>>>(tmQ, tmK, tmV, tmdO, p);
-    }
-    return (int)cudaGetLastError();
+    return p.split ? launch_one<128, true>(p, tmQ, tmK, tmV, tmdO, grid, stream) : launch_one<128, false>(p, tmQ, tmK, tmV, tmdO, grid, stream);
 }
 
 }  // namespace mesh_attn
