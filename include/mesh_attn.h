@@ -72,7 +72,8 @@ typedef struct {
     int32_t tensor_layout;    /* 0: [B,N,H,D], 1: [B,H,N,D]                                            */
     int32_t partial_mode;     /* 0: one partial per (g,u), fused over I_g^KV (Alg.2 l.5);
                                  1: one partial per pair (u,v): literal O_ij, lse_ij           */
-    int32_t precision;        /* backward MMA operands P, dS: 0 single bf16, 1 split hi+lo bf16        */
+    int32_t precision;        /* P (forward and backward) and dS as tensor-core operands: 0 one bf16,
+                                 1 split hi+lo bf16 pairs (two MMAs each; needed for outlier scores)    */
     int32_t reserved[5];      /* must be 0                                                             */
 } mesh_attn_plan_desc;
 

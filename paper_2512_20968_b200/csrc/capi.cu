@@ -143,6 +143,7 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     fp.items_per_gpu = (int)p->fwd_items.size();
     fp.g_first = g_first;
     fp.g_count = g_count;
+    fp.split = p->desc.precision;
     fp.partial_O = partial_O;
     fp.partial_lse = partial_lse;
     ProfScope prof(MESH_ATTN_K_TILE_FWD, (cudaStream_t)stream);

@@ -44,6 +44,10 @@ using namespace sm100;
 namespace {
 
 constexpr int kBwdThreads = 384;
+// register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs <= 65536
+constexpr int kCtrlRegs = 152, kComputeRegs = 176;
+template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
 template <int D, bool kSplit> struct BwdCfg {
     static_assert(D == 128, "backward kernel: dQ^T needs head_dim = UMMA M = 128");
@@ -208,6 +212,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
+    if (warp < 4) reg_dealloc<kCtrlRegs>();
     if (warp == 0) {
         // =============================== TMA producer ===============================
         if (lane == 0) {
@@ -343,6 +348,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     } else if (warp >= 4) {
         // =============================== compute groups ===============================
         // thread = (key row `row` = TMEM lane, query-column half `wg`): 64 elements of S^T / dP^T per step
+        reg_alloc<kComputeRegs>();
         const int wg = (warp - 4) >> 2;
         const int row = ((warp & 3) << 5) | lane;
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;

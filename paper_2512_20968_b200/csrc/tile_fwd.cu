@@ -29,6 +29,36 @@ namespace {
 
 constexpr int kThreads = 384;
 constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
+// register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kSoftmaxRegs <= 65536
+constexpr int kCtrlRegs = 72, kSoftmaxRegs = 216;
+constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
+#ifndef MESH_ATTN_POLY_OF_8
+#define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU
+#endif
+
+template <int N> struct IntTag { static constexpr int value = N; };
+template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
+
+// 2^x for x <= ~8 on the FMA/ALU pipes: round to nearest integer n with the 1.5*2^23 trick, degree-3 minimax
+// polynomial of 2^f on f = x - n in [-0.5, 0.5] (max relative error 7.5e-5, below the 2^-9 rounding of the bf16
+// P operand), then add n to the exponent field.  Inputs below -126 give ~2^-126 instead of 0.
+__device__ __forceinline__ float ex2_poly(float x)
+{
+    x = fmaxf(x, -126.f);
+    const float xr = x + 12582912.f;
+    const float f = x - (xr - 12582912.f);
+    float q = fmaf(0.0551716648f, f, 0.2426111251f);
+    q = fmaf(q, f, 0.6932609677f);
+    q = fmaf(q, f, 0.9999280572f);
+    return __int_as_float(__float_as_int(q) + (__float_as_int(xr) << 23));
+}
+// hi = bf16(x), lo = bf16(x - hi) for two values
+__device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t& hi, uint32_t& lo)
+{
+    hi = pack_bf16x2(x0, x1);
+    lo = pack_bf16x2(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xffff0000u));
+}
 
 template <int D> struct FwdCfg {
     static constexpr int kBoxes = D / 64;                  // 64-element (128-byte) TMA boxes per row
@@ -95,7 +125,7 @@ __device__ __forceinline__ ItemCtx load_item(const FwdParams& p, int idx)
     return c;
 }
 
-template <int D>
+template <int D, bool kSplit>
 __global__ void __launch_bounds__(kThreads, 1)
 tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const FwdParams p)
@@ -133,6 +163,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
+    if (warp < kSoftmaxWarp0) reg_dealloc<kCtrlRegs>();
     if (warp == kLoaderWarp) {
         // =============================== TMA producer ===============================
         if (lane == 0) {
@@ -184,12 +215,14 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     umma_ss(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc_qk, kk > 0);
                 }
             };
-            auto issue_pv = [&](int t, uint32_t vslot, bool acc) {
+            auto issue_pv = [&](int t, uint32_t vslot, bool acc) {      // P (bf16) in TMEM over S: hi at columns 0..63, lo at 64..127
                 const uint32_t va = smem_u32(sRing + vslot * Cfg::kTileBytes);
 #pragma unroll
-                for (int kk = 0; kk < kBlock / 16; ++kk)
-                    umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + kk * 8,
-                            umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || kk > 0) ? 1u : 0u);
+                for (int x = 0; x < (kSplit ? 2 : 1); ++x)
+#pragma unroll
+                    for (int kk = 0; kk < kBlock / 16; ++kk)
+                        umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + x * 64 + kk * 8,
+                                umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || kk > 0 || x > 0) ? 1u : 0u);
             };
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const ItemCtx c = load_item(p, idx);
@@ -223,11 +256,13 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
     } else if (warp >= kSoftmaxWarp0) {
         // =============================== softmax / epilogue ===============================
+        reg_alloc<kSoftmaxRegs>();
         const int t = (warp - kSoftmaxWarp0) >> 2;              // sub-tile of this warpgroup
         const int row = threadIdx.x - kSoftmaxWarp0 * 32 - t * kBlock;   // 0..127 = TMEM lane
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;
         const uint32_t tS = tmem + lane_base + Cfg::kColS + t * kBlock;
         const uint32_t tO = tmem + lane_base + Cfg::kColO + t * D;
+        const float c2 = gm.scale_log2;
         uint32_t s_phase = 0, o_phase = 0;
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const ItemCtx c = load_item(p, idx);
@@ -237,35 +272,43 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             float* out = p.partial_O + ((slot * gm.L + srow) * gm.heads_q + c.it.head) * (size_t)D;
             float* out_lse = p.partial_lse + (slot * gm.heads_q + c.it.head) * (size_t)gm.L + srow;
             KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
-            float m = -INFINITY, l = 0.f;     // running max (log2 domain, scaled) and running sum
+            // m: the reference max the exponentials are taken against (log2 domain, scaled).  It only follows the true
+            // running max when that has moved by more than kRescaleStep: P then stays <= 2^kRescaleStep, and the
+            // accumulator rescale (a TMEM round trip) is rare.  O / l is exact for any reference.
+            float m = -INFINITY, l = 0.f;
             int v, t0, off, j = 0;
             while (walk.next(v, t0, off)) {
                 mbar_wait(&s_full[t], s_phase);
                 s_phase ^= 1;
                 tc_fence_after();
-                // key column c of this block is visible iff c <= row + dlt
+                uint32_t s[kBlock];                                 // the whole score row of this thread
+#pragma unroll
+                for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tS + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[ch * 32]));
+                tmem_ld_wait();
+                // key column c of this block is visible iff c <= row + dlt; only blocks that straddle the diagonal mask
                 const int dlt = c.it.q0 + t * kBlock + off - t0;
                 const bool masked = gm.causal && dlt < kBlock - 1;
-                // pass 1: row max
-                float mx = -INFINITY;
-#pragma unroll 1
-                for (int ch = 0; ch < kBlock / 32; ++ch) {
-                    uint32_t r[32];
-                    tmem_ld_x32(tS + ch * 32, r);
-                    tmem_ld_wait();
-                    if (masked) {
+                if (masked) {
+                    const int lim = row + dlt;
 #pragma unroll
-                        for (int i = 0; i < 32; ++i) if (ch * 32 + i <= row + dlt) mx = fmaxf(mx, __uint_as_float(r[i]));
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 32; ++i) mx = fmaxf(mx, __uint_as_float(r[i]));
-                    }
+                    for (int i = 0; i < kBlock; ++i) if (i > lim) s[i] = 0xff800000u;   // -inf
                 }
-                const float m_new = fmaxf(m, mx * gm.scale_log2);
-                // rescale the accumulator when the running max moved (warp-uniform decision: TMEM ops are warp-collective)
-                if (j > 0 && __any_sync(0xffffffffu, m_new > m)) {
+                float mx0 = -INFINITY, mx1 = -INFINITY, mx2 = -INFINITY, mx3 = -INFINITY;
+#pragma unroll
+                for (int i = 0; i < kBlock; i += 8) {
+                    mx0 = fmaxf(mx0, fmaxf(__uint_as_float(s[i + 0]), __uint_as_float(s[i + 1])));
+                    mx1 = fmaxf(mx1, fmaxf(__uint_as_float(s[i + 2]), __uint_as_float(s[i + 3])));
+                    mx2 = fmaxf(mx2, fmaxf(__uint_as_float(s[i + 4]), __uint_as_float(s[i + 5])));
+                    mx3 = fmaxf(mx3, fmaxf(__uint_as_float(s[i + 6]), __uint_as_float(s[i + 7])));
+                }
+                const float m_blk = fmaxf(fmaxf(mx0, mx1), fmaxf(mx2, mx3)) * c2;
+                if (j == 0) {
+                    m = m_blk;
+                } else if (__any_sync(0xffffffffu, m_blk > m + kRescaleStep)) {   // warp-uniform: TMEM ops are warp-collective
+                    const float m_new = fmaxf(m, m_blk);
                     const float alpha = (m_new == -INFINITY) ? 1.f : ex2(m - m_new);   // m = -inf -> 0
                     l *= alpha;
+                    m = m_new;
 #pragma unroll 1
                     for (int ch = 0; ch < D / 32; ++ch) {
                         uint32_t r[32];
@@ -276,31 +319,33 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         tmem_st_x32(tO + ch * 32, r);
                     }
                 }
-                m = m_new;
-                const float m_safe = (m == -INFINITY) ? 0.f : m;
-                // pass 2: p = exp2(s*scale_log2 - m), row sum, P (bf16) into TMEM over S
-                float lsum = 0.f;
-#pragma unroll 1
-                for (int ch = 0; ch < kBlock / 32; ++ch) {
-                    uint32_t r[32], pk[16];
-                    tmem_ld_x32(tS + ch * 32, r);
-                    tmem_ld_wait();
+                const float neg_m = (m == -INFINITY) ? 0.f : -m;
+                // p = exp2(s*c2 - m).  Unmasked blocks: kPolyOf8 of every 8 on the FMA pipe (degree-3 polynomial), the
+                // rest on the MUFU; diagonal blocks: all on the MUFU (exp2(-inf) must be exactly 0 there).
+                float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+                auto exp_row = [&](auto poly_tag) {
+                    constexpr int kPoly = decltype(poly_tag)::value;
 #pragma unroll
-                    for (int i = 0; i < 32; i += 2) {
-                        float p0 = ex2(fmaf(__uint_as_float(r[i]), gm.scale_log2, -m_safe));
-                        float p1 = ex2(fmaf(__uint_as_float(r[i + 1]), gm.scale_log2, -m_safe));
-                        if (masked) {
-                            if (ch * 32 + i > row + dlt) p0 = 0.f;
-                            if (ch * 32 + i + 1 > row + dlt) p1 = 0.f;
+                    for (int ch = 0; ch < kBlock / 32; ++ch) {
+                        uint32_t hi[16], lo[16];
+#pragma unroll
+                        for (int i = 0; i < 32; i += 2) {
+                            const float x0 = fmaf(__uint_as_float(s[ch * 32 + i]), c2, neg_m);
+                            const float x1 = fmaf(__uint_as_float(s[ch * 32 + i + 1]), c2, neg_m);
+                            const float p0 = ((i & 7) < kPoly) ? ex2_poly(x0) : ex2(x0);
+                            const float p1 = (((i + 1) & 7) < kPoly) ? ex2_poly(x1) : ex2(x1);
+                            if ((i & 2) == 0) { l0 += p0; l1 += p1; } else { l2 += p0; l3 += p1; }
+                            if constexpr (kSplit) split_bf16x2(p0, p1, hi[i / 2], lo[i / 2]);
+                            else hi[i / 2] = pack_bf16x2(p0, p1);
                         }
-                        lsum += p0 + p1;
-                        pk[i / 2] = pack_bf16x2(p0, p1);
+                        // the whole S row is in registers: P (bf16) may overwrite any of its columns
+                        tmem_st_x16(tS + ch * 16, hi);
+                        if constexpr (kSplit) tmem_st_x16(tS + 64 + ch * 16, lo);
                     }
-                    // chunk ch of S (32 fp32 columns) was fully read above; P chunk ch occupies 16 columns
-                    // [16*ch, 16*ch+16) which only overlaps S columns this thread has already consumed
-                    tmem_st_x16(tS + ch * 16, pk);
-                }
-                l += lsum;
+                };
+                if (masked) exp_row(IntTag<0>{});
+                else exp_row(IntTag<MESH_ATTN_POLY_OF_8>{});
+                l += (l0 + l1) + (l2 + l3);
                 tmem_st_wait();
                 tc_fence_before();
                 mbar_arrive(&p_full[t]);
@@ -336,6 +381,15 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == kAllocWarp) tmem_dealloc<512>(tmem);
 }
 
+template <int D, bool kSplit>
+int launch_fwd_one(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int grid, cudaStream_t stream)
+{
+    cudaError_t e = cudaFuncSetAttribute(tile_fwd_kernel<D, kSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes);
+    if (e != cudaSuccess) return (int)e;
+    tile_fwd_kernel<D, kSplit><<<grid, kThreads, FwdCfg<D>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
+    return (int)cudaGetLastError();
+}
+
 }  // namespace
 
 int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int num_sms,
@@ -344,17 +398,9 @@ int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
-    cudaError_t e;
-    if (p.gm.head_dim == 128) {
-        e = cudaFuncSetAttribute(tile_fwd_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<128>::kSmemBytes);
-        if (e != cudaSuccess) return (int)e;
-        tile_fwd_kernel<128><<<grid, kThreads, FwdCfg<128>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
-    } else {
-        e = cudaFuncSetAttribute(tile_fwd_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<64>::kSmemBytes);
-        if (e != cudaSuccess) return (int)e;
-        tile_fwd_kernel<64><<<grid, kThreads, FwdCfg<64>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
-    }
-    return (int)cudaGetLastError();
+    if (p.gm.head_dim == 128)
+        return p.split ? launch_fwd_one<128, true>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<128, false>(p, tmQ, tmK, tmV, grid, stream);
+    return p.split ? launch_fwd_one<64, true>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<64, false>(p, tmQ, tmK, tmV, grid, stream);
 }
 
 }  // namespace mesh_attn

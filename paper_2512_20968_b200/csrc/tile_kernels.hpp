@@ -14,6 +14,7 @@ struct FwdParams {
     const SegList* seglists;
     int items_per_gpu;
     int g_first, g_count;
+    int split;                 // precision: 1 = P fed to the PV MMA as hi + lo bf16
     float* partial_O;          // [g_count][slots][B][L][Hq][D]
     float* partial_lse;        // [g_count][slots][B][Hq][L]
 };
