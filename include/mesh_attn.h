@@ -154,8 +154,9 @@ int mesh_attn_merge(const mesh_attn_plan* plan, int32_t q_group,
 /* Backward workspace bwd_ws, fp32 [2][B][Hq][N] (MESH_ATTN_Q_BWD_WS_BYTES), all rows:
  *   bwd_ws[0][b,h,row] = delta = sum_d dO * O  (needed by every pair touching the row; the
  *                        paper passes O_i, dO_i to the backward kernel)
- *   bwd_ws[1][b,h,row] = -lse * log2(e)  (exponent offset of P = exp(S - lse) in base 2;
- *                        lse is the FINAL merged LSE, reading R8) */
+ *   bwd_ws[1][b,h,row] = log2(softmax_scale) - lse * log2(e)  (exponent offset, in base 2, of
+ *                        scale * P = scale * exp(S - lse); lse is the FINAL merged LSE,
+ *                        DESIGN.md reading R8) */
 int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const float* O, const void* dO,
                              const float* lse, float* bwd_ws, void* stream);
 

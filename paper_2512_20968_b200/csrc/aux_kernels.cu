@@ -128,9 +128,9 @@ __global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
         const size_t at = ((size_t)bt * gm.heads_q + h) * N + row;
         const float l = p.lse[at];
         p.ws[at] = acc;
-        // exponent offset of the backward's P = exp2(S*scale*log2e - lse*log2e); a row without visible keys
-        // (lse = -inf) only ever meets masked positions: any finite value does
-        p.ws[(size_t)gm.batch * gm.heads_q * N + at] = (l == -INFINITY) ? 0.f : -l * 1.4426950408889634f;
+        // exponent offset of the backward's P' = scale * exp(S - lse) = exp2(S*scale*log2e + log2(scale) - lse*log2e); a row
+        // without visible keys (lse = -inf) only ever meets masked positions: any finite value does
+        p.ws[(size_t)gm.batch * gm.heads_q * N + at] = (l == -INFINITY) ? 0.f : fmaf(-l, 1.4426950408889634f, log2f(gm.scale));
     }
 }
 

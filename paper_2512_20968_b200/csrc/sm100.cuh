@@ -35,13 +35,15 @@ __device__ __forceinline__ void mbar_arrive(uint64_t* bar)
 {
     asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// One try_wait: the thread is suspended by the hardware until the phase completes or a time limit (at most the
+// suspend-time hint, in ns) expires -- a waiting warp does not compete for issue slots with the compute warps.
 __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
 {
     uint32_t ok;
     asm volatile(
-        "{\n.reg .pred P;\nmbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2;\nselp.b32 %0, 1, 0, P;\n}"
+        "{\n.reg .pred P;\nmbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2, %3;\nselp.b32 %0, 1, 0, P;\n}"
         : "=r"(ok)
-        : "r"(smem_u32(bar)), "r"(parity)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(10000000u)
         : "memory");
     return ok != 0;
 }
@@ -50,9 +52,8 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 #if MESH_ATTN_WATCHDOG
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
-    uint32_t spins = 0;
     while (!mbar_try_wait(bar, parity)) {
-        if ((++spins & 0x3ff) == 0 && clock64() - t0 > 8000000000ll) {   // ~4 s: certainly a deadlock
+        if (clock64() - t0 > 8000000000ll) {   // ~4 s: certainly a deadlock
             printf("mesh_attn watchdog: mbarrier wait timed out (block %d thread %d bar 0x%x parity %u)\n", blockIdx.x,
                    threadIdx.x, smem_u32(bar), parity);
             __trap();

@@ -6,7 +6,7 @@
 // shared memory and dK, dV in TMEM, and streams 128-row Q / dO blocks of every Q partition
 // of the tile (and every query head of the GQA group).  Per Q block, five tcgen05 MMAs:
 //
-//   S^T  = K Q^T            (TMEM columns   0..127)      P^T = exp2(S^T*c - lse*log2e)  (bf16, over S^T)
+//   S^T  = K Q^T            (TMEM columns   0..127)      P^T = scale * exp2(S^T*c - lse*log2e)  (bf16, over S^T)
 //   dP^T = V dO^T           (TMEM columns 128..255)      dS^T = P^T o (dP^T - delta)    (bf16, smem)
 //   dV  += P^T  dO          (TMEM columns 384..511)      A operand P^T straight from TMEM
 //   dK  += dS^T Q           (TMEM columns 256..383)      A operand dS^T from smem (K-major)
@@ -25,6 +25,9 @@
 //   warps 8-11  compute group 1: key row = TMEM lane, query columns 64..127
 //               each: S^T -> P^T (regs + TMEM), dP^T -> dS^T (smem), dQ^T drain (x scale, atomics);
 //               epilogue: group 0 drains dK, group 1 drains dV
+//
+// The softmax scale is folded into P^T (its log2 is part of the exponent offset the preprocess kernel wrote), so
+// dS^T, dQ^T and dK come out already scaled and only dV is divided by it, once per item in the epilogue.
 //
 // dQ, dK, dV are accumulated into global fp32 with atomics: the sums over the Q group, the KV
 // group (Alg.3 l.6-7, L254-255) and the GQA head group all land in the same buffers.
@@ -217,7 +220,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // =============================== TMA producer ===============================
         if (lane == 0) {
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0;
-            const float* nlse = p.ws + (size_t)gm.batch * gm.heads_q * N;      // ws[1] = -lse*log2e
+            const float* nlse = p.ws + (size_t)gm.batch * gm.heads_q * N;      // ws[1] = log2(scale) - lse*log2e
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
@@ -364,7 +367,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
             return st;
         };
-        // P^T = exp2(S^T * scale*log2e - lse*log2e), causal mask on blocks that straddle the diagonal only
+        // P^T = scale * exp2(S^T * scale*log2e - lse*log2e) (the offset in smem is log2(scale) - lse*log2e), causal mask on
+        // blocks that straddle the diagonal only
         auto compute_P = [&](uint32_t st, int t0, int s0, int off) {
             const float4* nl4 = reinterpret_cast<const float4*>(sLse(st) + wg * 64);
             const bool masked = gm.causal && (t0 + kBlock - 1 - off - s0 > 0);     // block-uniform
@@ -451,7 +455,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         };
         // dQ^T (lane = d, columns = the 64 queries of this half) -> x scale -> one coalesced atomic per (query, 32 d's)
         auto drain_dQ = [&](int batch, int u, int h, int s0) {
-            float* base = p.dQ + (size_t)batch * p.q_stride_b + ((size_t)u * gm.L + s0 + wg * 64) * p.q_stride_row + (size_t)h * p.q_stride_h + row;
+            float* ptr = p.dQ + (size_t)batch * p.q_stride_b + ((size_t)u * gm.L + s0 + wg * 64) * p.q_stride_row + (size_t)h * p.q_stride_h + row;
+            const size_t rs = (size_t)p.q_stride_row;
             mbar_wait(dq_full, dq_ph);
             dq_ph ^= 1;
             tc_fence_after();
@@ -459,13 +464,13 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tmem_ld_x32(tDP, r);
             tmem_ld_wait();
 #pragma unroll
-            for (int j = 0; j < 32; ++j) red_add(base + (size_t)j * p.q_stride_row, __uint_as_float(r[j]) * gm.scale);
+            for (int j = 0; j < 32; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
             tmem_ld_x32(tDP + 32, r);
             tmem_ld_wait();
             tc_fence_before();
             mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
 #pragma unroll
-            for (int j = 0; j < 32; ++j) red_add(base + (size_t)(32 + j) * p.q_stride_row, __uint_as_float(r[j]) * gm.scale);
+            for (int j = 0; j < 32; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
         };
 
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
@@ -494,7 +499,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_after();
             float* grow = (wg == 0 ? p.dK : p.dV) + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
                           (size_t)c.it.head_kv * p.k_stride_h;
-            drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? gm.scale : 1.0f);
+            drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? 1.0f : 1.0f / gm.scale);
             tc_fence_before();
             mbar_arrive(dkv_empty);
         }

@@ -30,7 +30,7 @@ namespace {
 constexpr int kThreads = 384;
 constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
 // register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kSoftmaxRegs <= 65536
-constexpr int kCtrlRegs = 72, kSoftmaxRegs = 216;
+constexpr int kCtrlRegs = 88, kSoftmaxRegs = 208;
 constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
 #ifndef MESH_ATTN_POLY_OF_8
 #define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU

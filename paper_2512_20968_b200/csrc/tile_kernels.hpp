@@ -27,7 +27,7 @@ struct BwdParams {
     int items_per_gpu;
     int g_first, g_count;
     int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
-    const float* ws;           // [2][B][Hq][N]: delta, -lse*log2e (written by bwd_preprocess)
+    const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess)
     float *dQ, *dK, *dV;       // fp32 accumulators
     // element strides of dQ (query-shaped) and dK/dV (key-shaped) tensors
     long long q_stride_b, q_stride_row, q_stride_h;
@@ -52,7 +52,7 @@ struct DeltaParams {
     const float* O;
     const void* dO;            // bf16
     const float* lse;          // [B][Hq][N] final merged LSE (natural log)
-    float* ws;                 // [2][B][Hq][N]: delta, -lse*log2e
+    float* ws;                 // [2][B][Hq][N]: delta, log2(scale) - lse*log2e
     long long stride_b, stride_row, stride_h;   // element strides shared by O and dO
 };
 

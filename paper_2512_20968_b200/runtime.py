@@ -30,7 +30,7 @@ class Buffers:
         self.O = torch.empty((B, N, Hq, D), **f32)
         self.lse = torch.empty((B, Hq, N), **f32)
         if backward:
-            self.bwd_ws = torch.empty((2, B, Hq, N), **f32)      # [0] = delta, [1] = -lse*log2(e)  (Q_BWD_WS_BYTES)
+            self.bwd_ws = torch.empty((2, B, Hq, N), **f32)      # [0] = delta, [1] = log2(scale) - lse*log2(e)  (Q_BWD_WS_BYTES)
             self.delta = self.bwd_ws[0]
             self.dQ = torch.empty((B, N, Hq, D), **f32)
             self.dK = torch.empty((B, N, Hkv, D), **f32)
