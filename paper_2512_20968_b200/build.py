@@ -45,9 +45,11 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     OBJ.mkdir(exist_ok=True)
     nvcc = _nvcc()
 
+    extra = os.environ.get("MESH_ATTN_NVCC_EXTRA", "").split()      # e.g. -DMESH_ATTN_POLY_OF_8=1 for tuning builds
+
     def compile_one(src: str):
         obj = OBJ / (src.rsplit(".", 1)[0] + ".o")
-        cmd = [nvcc, *NVCC_FLAGS, "-x", "cu", "-c", str(CSRC / src), "-o", str(obj)]
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-x", "cu", "-c", str(CSRC / src), "-o", str(obj)]
         r = subprocess.run(cmd, capture_output=True, text=True)
         (OBJ / (src + ".log")).write_text(r.stdout + r.stderr)
         if r.returncode != 0:

@@ -218,7 +218,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp < 4) reg_dealloc<kCtrlRegs>();
     if (warp == 0) {
         // =============================== TMA producer ===============================
-        if (lane == 0) {
+        if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0;
             const float* nlse = p.ws + (size_t)gm.batch * gm.heads_q * N;      // ws[1] = log2(scale) - lse*log2e
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
@@ -253,7 +253,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         }
     } else if (warp == 1) {
         // =============================== MMA issuer ===============================
-        if (lane == 0) {
+        if (elect_one()) {
             constexpr uint32_t idesc_kk = umma_idesc(kBlock, kBlock, false, false);   // S^T, dP^T: both operands K-major over head_dim
             constexpr uint32_t idesc_tn = umma_idesc(kBlock, D, false, true);         // dV (A in TMEM), dK (A smem K-major); B row-major [q x d]
             constexpr uint32_t idesc_nn = umma_idesc(D, kBlock, true, true);          // dQ^T: A = K tile M-major, B = dS^T N-major

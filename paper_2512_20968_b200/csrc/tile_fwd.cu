@@ -36,6 +36,17 @@ constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is resc
 #define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU
 #endif
 
+// optional per-phase clock accounting of one softmax thread (tuning builds only: -DMESH_ATTN_PHASE_TIMING)
+#ifdef MESH_ATTN_PHASE_TIMING
+#define PT_DECL long long pt_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long pt_last = clock64(); long long pt_n = 0
+#define PT_MARK(k) do { const long long pt_now = clock64(); pt_acc[k] += pt_now - pt_last; pt_last = pt_now; if ((k) == 0) ++pt_n; } while (0)
+#define PT_REPORT(what) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && pt_n) printf("%s | thread %d blocks %lld: %lld %lld %lld %lld %lld (loop-back %lld)\n", what, threadIdx.x, pt_n, pt_acc[1] / pt_n, pt_acc[2] / pt_n, pt_acc[3] / pt_n, pt_acc[4] / pt_n, pt_acc[5] / pt_n, pt_acc[0] / pt_n); } while (0)
+#else
+#define PT_DECL
+#define PT_MARK(k)
+#define PT_REPORT(what)
+#endif
+
 template <int N> struct IntTag { static constexpr int value = N; };
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
@@ -71,39 +82,41 @@ template <int D> struct FwdCfg {
     static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
 };
 
-// Walks the 128-key KV blocks of a work item in plan order; every role runs the same walk.
-struct KvWalk {
-    const Geom& gm;
-    const Seg* segs;
-    int nseg, g, u, q_last;   // q_last = last local query row of the item
-    int si = -1, t = 0, t_hi = 0, v = 0, off = 0;
-    __device__ KvWalk(const Geom& gm_, const Seg* segs_, int nseg_, int g_, int u_, int q_last_)
-        : gm(gm_), segs(segs_), nseg(nseg_), g(g_), u(u_), q_last(q_last_) {}
-    // next block: KV partition v, first local key row t0, causal offset off (key t visible to row s iff t <= s + off)
-    __device__ bool next(int& v_out, int& t0_out, int& off_out)
-    {
-        while (true) {
-            if (si >= 0 && t < t_hi) { v_out = v; t0_out = t; off_out = off; t += kBlock; return true; }
-            if (++si >= nseg) return false;
-            const Seg sg = segs[si];
-            v = kv_partition(gm, g, sg.part_local);
-            t = sg.begin;
-            t_hi = sg.end;
-            off = 0x20000000;
-            if (gm.causal) {
-                off = causal_off(gm, u, v);
-                const int lim = q_last + off;                 // last visible key row for the item's last query row
-                t_hi = lim < sg.begin ? sg.begin : min(sg.end, (lim / kBlock + 1) * kBlock);
-            }
-        }
+// The 128-key KV blocks of a work item in plan order: segment by segment (KV partition v, local key rows
+// [begin, end) clipped to the rows visible to the item's last query row), block by block.  Every role runs the same
+// nest; f(v, t0, off): KV partition, first local key row, causal offset (key t visible to row s iff t <= s + off).
+struct KvRange { int v, off, t_lo, t_hi; };
+__device__ __forceinline__ KvRange kv_range(const Geom& gm, const Seg sg, int g, int u, int q_last)
+{
+    KvRange r;
+    r.v = kv_partition(gm, g, sg.part_local);
+    r.t_lo = sg.begin;
+    r.t_hi = sg.end;
+    r.off = 0x20000000;
+    if (gm.causal) {
+        r.off = causal_off(gm, u, r.v);
+        const int lim = q_last + r.off;                 // last visible key row for the item's last query row
+        r.t_hi = lim < sg.begin ? sg.begin : min(sg.end, (lim / kBlock + 1) * kBlock);
     }
-    __device__ int count()
-    {
-        int n = 0, a, b, c;
-        while (next(a, b, c)) ++n;
-        return n;
+    return r;
+}
+template <class F>
+__device__ __forceinline__ void for_each_kv_block(const Geom& gm, const Seg* segs, int nseg, int g, int u, int q_last, F&& f)
+{
+    for (int si = 0; si < nseg; ++si) {
+        const KvRange r = kv_range(gm, segs[si], g, u, q_last);
+        for (int t0 = r.t_lo; t0 < r.t_hi; t0 += kBlock) f(r.v, t0, r.off);
     }
-};
+}
+__device__ __forceinline__ int count_kv_blocks(const Geom& gm, const Seg* segs, int nseg, int g, int u, int q_last)
+{
+    int n = 0;
+    for (int si = 0; si < nseg; ++si) {
+        const KvRange r = kv_range(gm, segs[si], g, u, q_last);
+        n += (r.t_hi - r.t_lo) / kBlock;
+    }
+    return n;
+}
 
 struct ItemCtx {
     FwdItem it;
@@ -166,14 +179,12 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp < kSoftmaxWarp0) reg_dealloc<kCtrlRegs>();
     if (warp == kLoaderWarp) {
         // =============================== TMA producer ===============================
-        if (lane == 0) {
+        if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, q_phase = 0;
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const ItemCtx c = load_item(p, idx);
-                KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
-                int v, t0, off;
                 bool first = true;
-                while (walk.next(v, t0, off)) {
+                for_each_kv_block(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1, [&](int v, int t0, int) {
                     if (first) {
                         first = false;
                         mbar_wait(q_empty, q_phase ^ 1);
@@ -193,15 +204,16 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                                         bx * 64, hk, v * gm.L + t0, c.it.batch, kEvictLast);
                         if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
                     }
-                }
+                });
             }
         }
     } else if (warp == kMmaWarp) {
         // =============================== MMA issuer ===============================
-        if (lane == 0) {
+        if (elect_one()) {
             constexpr uint32_t idesc_qk = umma_idesc(kBlock, kBlock, false, false);
             constexpr uint32_t idesc_pv = umma_idesc(kBlock, D, false, true);
             uint32_t stage = 0, ring_phase = 0, q_phase = 0, p_phase[2] = {0, 0};
+            PT_DECL;
             auto ring_wait = [&](uint32_t& slot) {
                 mbar_wait(&kv_full[stage], ring_phase);
                 slot = stage;
@@ -226,8 +238,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             };
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const ItemCtx c = load_item(p, idx);
-                KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
-                const int nb = walk.count();
+                const int nb = count_kv_blocks(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
                 if (nb == 0) continue;
                 mbar_wait(q_full, q_phase);
                 q_phase ^= 1;
@@ -238,21 +249,26 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 umma_commit(&kv_empty[kslot]);
                 for (int j = 0; j < nb; ++j) {
                     const bool more = j + 1 < nb;
+                    PT_MARK(0);
                     ring_wait(vslot);
                     if (more) ring_wait(kslot);
+                    PT_MARK(1);
                     for (int t = 0; t < c.nt; ++t) {
                         mbar_wait(&p_full[t], p_phase[t]);
                         p_phase[t] ^= 1;
                         tc_fence_after();
+                        PT_MARK(2 + 2 * t);
                         issue_pv(t, vslot, j > 0);
                         if (more) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
                         else umma_commit(&o_full[t]);
+                        PT_MARK(3 + 2 * t);
                     }
                     umma_commit(&kv_empty[vslot]);
                     if (more) umma_commit(&kv_empty[kslot]);
                 }
                 umma_commit(q_empty);
             }
+            PT_REPORT("fwd MMA thread clocks per block: ring_wait, wait_p0, issue0, wait_p1, issue1");
         }
     } else if (warp >= kSoftmaxWarp0) {
         // =============================== softmax / epilogue ===============================
@@ -264,6 +280,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const uint32_t tO = tmem + lane_base + Cfg::kColO + t * D;
         const float c2 = gm.scale_log2;
         uint32_t s_phase = 0, o_phase = 0;
+        PT_DECL;
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const ItemCtx c = load_item(p, idx);
             if (t >= c.nt) continue;
@@ -271,20 +288,22 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             const size_t slot = ((size_t)c.g_local * gm.slots_per_gpu + c.it.slot) * gm.batch + c.it.batch;
             float* out = p.partial_O + ((slot * gm.L + srow) * gm.heads_q + c.it.head) * (size_t)D;
             float* out_lse = p.partial_lse + (slot * gm.heads_q + c.it.head) * (size_t)gm.L + srow;
-            KvWalk walk(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
             // m: the reference max the exponentials are taken against (log2 domain, scaled).  It only follows the true
             // running max when that has moved by more than kRescaleStep: P then stays <= 2^kRescaleStep, and the
             // accumulator rescale (a TMEM round trip) is rare.  O / l is exact for any reference.
             float m = -INFINITY, l = 0.f;
-            int v, t0, off, j = 0;
-            while (walk.next(v, t0, off)) {
+            int j = 0;
+            for_each_kv_block(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1, [&](int, int t0, int off) {
+                PT_MARK(0);
                 mbar_wait(&s_full[t], s_phase);
                 s_phase ^= 1;
                 tc_fence_after();
                 uint32_t s[kBlock];                                 // the whole score row of this thread
 #pragma unroll
                 for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tS + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[ch * 32]));
+                PT_MARK(1);
                 tmem_ld_wait();
+                PT_MARK(2);
                 // key column c of this block is visible iff c <= row + dlt; only blocks that straddle the diagonal mask
                 const int dlt = c.it.q0 + t * kBlock + off - t0;
                 const bool masked = gm.causal && dlt < kBlock - 1;
@@ -319,6 +338,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         tmem_st_x32(tO + ch * 32, r);
                     }
                 }
+                PT_MARK(3);
                 const float neg_m = (m == -INFINITY) ? 0.f : -m;
                 // p = exp2(s*c2 - m).  Unmasked blocks: kPolyOf8 of every 8 on the FMA pipe (degree-3 polynomial), the
                 // rest on the MUFU; diagonal blocks: all on the MUFU (exp2(-inf) must be exactly 0 there).
@@ -346,11 +366,13 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (masked) exp_row(IntTag<0>{});
                 else exp_row(IntTag<MESH_ATTN_POLY_OF_8>{});
                 l += (l0 + l1) + (l2 + l3);
+                PT_MARK(4);
                 tmem_st_wait();
                 tc_fence_before();
                 mbar_arrive(&p_full[t]);
+                PT_MARK(5);
                 ++j;
-            }
+            });
             if (j == 0) {                      // no visible key for the whole item (reading R5)
 #pragma unroll 4
                 for (int d = 0; d < D; d += 4) *reinterpret_cast<float4*>(out + d) = make_float4(0.f, 0.f, 0.f, 0.f);
@@ -374,6 +396,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             }
             *out_lse = l > 0.f ? (m + lg2(l)) * 0.6931471805599453f : -INFINITY;
         }
+        PT_REPORT("fwd softmax clocks per block: wait_s+issue_ld, wait_ld, mask+max+rescale, exp+st, st_wait+arrive");
     }
 
     tc_fence_before();
