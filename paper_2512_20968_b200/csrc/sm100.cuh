@@ -10,6 +10,17 @@
 #define MESH_ATTN_WATCHDOG 1   // bounded mbarrier waits: a protocol bug traps instead of hanging the GPU
 #endif
 
+// optional per-phase clock accounting of one thread per role (tuning builds only: -DMESH_ATTN_PHASE_TIMING)
+#ifdef MESH_ATTN_PHASE_TIMING
+#define PT_DECL long long pt_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long pt_last = clock64(); long long pt_n = 0
+#define PT_MARK(k) do { const long long pt_now = clock64(); pt_acc[k] += pt_now - pt_last; pt_last = pt_now; if ((k) == 0) ++pt_n; } while (0)
+#define PT_REPORT(what) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && pt_n) printf("%s | thread %d blocks %lld: %lld %lld %lld %lld %lld (loop-back %lld)\n", what, threadIdx.x, pt_n, pt_acc[1] / pt_n, pt_acc[2] / pt_n, pt_acc[3] / pt_n, pt_acc[4] / pt_n, pt_acc[5] / pt_n, pt_acc[0] / pt_n); } while (0)
+#else
+#define PT_DECL
+#define PT_MARK(k)
+#define PT_REPORT(what)
+#endif
+
 namespace sm100 {
 
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -216,6 +227,35 @@ __device__ __forceinline__ float lg2(float x)
     float y;
     asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
     return y;
+}
+
+// ---------------------------------------------------------------------------------- packed fp32 pairs (sm_100: FFMA2/FADD2/FMUL2)
+// two independent fp32 operations per instruction: halves the issue slots of the element-wise softmax arithmetic
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 mul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
 }
 
 // byte offset of (row, 16-byte chunk) inside a 128B-swizzled tile whose rows are 128 bytes and

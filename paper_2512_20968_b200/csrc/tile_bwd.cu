@@ -23,8 +23,8 @@
 //   warp 2      TMEM allocator
 //   warps 4-7   compute group 0: key row = TMEM lane, query columns  0..63  of the block
 //   warps 8-11  compute group 1: key row = TMEM lane, query columns 64..127
-//               each: S^T -> P^T (regs + TMEM), dP^T -> dS^T (smem), dQ^T drain (x scale, atomics);
-//               epilogue: group 0 drains dK, group 1 drains dV
+//               each: S^T -> P^T (regs + TMEM), dP^T -> dS^T (smem); epilogue: group 0 drains dK, group 1 drains dV
+//   warps 12-15 dQ drain group: dQ^T row d = TMEM lane -> registers -> atomics, overlapping the next step's MMAs
 //
 // The softmax scale is folded into P^T (its log2 is part of the exponent offset the preprocess kernel wrote), so
 // dS^T, dQ^T and dK come out already scaled and only dV is divided by it, once per item in the epilogue.
@@ -46,9 +46,9 @@ using namespace sm100;
 
 namespace {
 
-constexpr int kBwdThreads = 384;
-// register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs <= 65536
-constexpr int kCtrlRegs = 152, kComputeRegs = 176;
+constexpr int kBwdThreads = 512;
+// register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs + 128 x kDrainRegs <= 65536
+constexpr int kCtrlRegs = 72, kComputeRegs = 136, kDrainRegs = 160;
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
@@ -204,7 +204,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(dp_full, 1);
         mbar_init(ds_full, kCompute);
         mbar_init(dq_full, 1);
-        mbar_init(dq_empty, kCompute);
+        mbar_init(dq_empty, kBlock);
         mbar_init(dkv_full, 1);
         mbar_init(dkv_empty, kCompute);
         fence_mbar_init();
@@ -258,6 +258,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             constexpr uint32_t idesc_tn = umma_idesc(kBlock, D, false, true);         // dV (A in TMEM), dK (A smem K-major); B row-major [q x d]
             constexpr uint32_t idesc_nn = umma_idesc(D, kBlock, true, true);          // dQ^T: A = K tile M-major, B = dS^T N-major
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0, p_ph = 0, ds_ph = 0, dqe_ph = 0, dkve_ph = 0;
+            PT_DECL;
             const uint32_t aK = smem_u32(sK), aV = smem_u32(sV), aDs = smem_u32(sDs);
             auto mma_kmajor = [&](uint32_t dcol, uint32_t a, uint32_t b) {          // D = A B^T, both K-major over head_dim
 #pragma unroll
@@ -291,10 +292,12 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 while (have) {
                     const bool more = walk.next(u, h, s0, off);
                     const uint32_t aQ = smem_u32(sQ(st_cur)), adO = smem_u32(sdO(st_cur));
+                    PT_MARK(0);
                     // dV += P^T dO   (P^T bf16 in TMEM: group w's 64 queries at columns 64w.. (hi) and 64w+32.. (lo))
                     mbar_wait(p_full, p_ph);
                     p_ph ^= 1;
                     tc_fence_after();
+                    PT_MARK(1);
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
@@ -302,22 +305,18 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             umma_ts(tmem + Cfg::kColDV, tmem + Cfg::kColS + (kk >> 2) * 64 + x * 32 + (kk & 3) * 8,
                                     umma_desc(adO + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
                     uint32_t st_next = 0;
-                    if (Cfg::kStages > 1 && more) {      // S^T(i+1) as early as possible
+                    if (Cfg::kStages > 1 && more) {      // S^T(i+1) as early as possible: P^T(i+1) is computed under this step's MMAs
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
                         umma_commit(s_full);
                     }
-                    // dQ^T = K^T dS^T (first: its drain overlaps the dK MMA) ; dK += dS^T Q
+                    // dK += dS^T Q first (it releases the Q/dO stage: the next load gets the longest possible lead), then
+                    // dQ^T = K^T dS^T, emptied by the drain group
+                    PT_MARK(2);
                     mbar_wait(ds_full, ds_ph);
                     ds_ph ^= 1;
                     tc_fence_after();
-#pragma unroll
-                    for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
-                        for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
-                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(dq_full);
+                    PT_MARK(3);
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
@@ -325,15 +324,24 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
                                     umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
                     umma_commit(&qd_empty[st_cur]);
+#pragma unroll
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
+#pragma unroll
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
+                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
+                    umma_commit(dq_full);
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
                         umma_commit(s_full);
                     }
+                    PT_MARK(4);
                     if (more) {                          // dP^T(i+1) once dQ^T(i) has left TMEM
                         mbar_wait(dq_empty, dqe_ph);
                         dqe_ph ^= 1;
                         tc_fence_after();
+                        PT_MARK(5);
                         mma_kmajor(Cfg::kColDP, aV, smem_u32(sdO(st_next)));
                         umma_commit(dp_full);
                     } else {
@@ -347,8 +355,9 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     ++i;
                 }
             }
+            PT_REPORT("bwd MMA thread clocks per step: wait_p, issue dV+S(next), wait_ds, issue dK+dQ, wait_dq_empty (loop-back = issue dP)");
         }
-    } else if (warp >= 4) {
+    } else if (warp >= 4 && warp < 12) {
         // =============================== compute groups ===============================
         // thread = (key row `row` = TMEM lane, query-column half `wg`): 64 elements of S^T / dP^T per step
         reg_alloc<kComputeRegs>();
@@ -360,6 +369,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         uint8_t* sDsHalf = sDs + wg * (kBlock * 128);                     // [128 key rows][64 queries] bf16, 128-byte swizzled rows
         uint32_t stage = 0, ring_phase = 0, s_ph = 0, dp_ph = 0, dq_ph = 0, dkv_ph = 0;
         float pr[64];                                                     // P^T of the current step (fp32), reused for dS^T
+        PT_DECL;
 
         auto next_stage = [&]() {
             mbar_wait(&qd_full[stage], ring_phase);                       // Q/dO tiles and the -lse*log2e / delta vectors landed
@@ -375,6 +385,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mbar_wait(s_full, s_ph);
             s_ph ^= 1;
             tc_fence_after();
+            PT_MARK(3);
 #pragma unroll
             for (int ch = 0; ch < 2; ++ch) {
                 uint32_t r[32];
@@ -423,6 +434,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mbar_wait(dp_full, dp_ph);           // also: dQ^T / dK of the previous step have finished reading the dS tile
             dp_ph ^= 1;
             tc_fence_after();
+            PT_MARK(1);
 #pragma unroll
             for (int ch = 0; ch < 2; ++ch) {
                 uint32_t r[32];
@@ -453,26 +465,6 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             mbar_arrive(ds_full);
         };
-        // dQ^T (lane = d, columns = the 64 queries of this half) -> x scale -> one coalesced atomic per (query, 32 d's)
-        auto drain_dQ = [&](int batch, int u, int h, int s0) {
-            float* ptr = p.dQ + (size_t)batch * p.q_stride_b + ((size_t)u * gm.L + s0 + wg * 64) * p.q_stride_row + (size_t)h * p.q_stride_h + row;
-            const size_t rs = (size_t)p.q_stride_row;
-            mbar_wait(dq_full, dq_ph);
-            dq_ph ^= 1;
-            tc_fence_after();
-            uint32_t r[32];                      // two 32-column halves in turn: P^T of the next step is live in registers
-            tmem_ld_x32(tDP, r);
-            tmem_ld_wait();
-#pragma unroll
-            for (int j = 0; j < 32; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
-            tmem_ld_x32(tDP + 32, r);
-            tmem_ld_wait();
-            tc_fence_before();
-            mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
-#pragma unroll
-            for (int j = 0; j < 32; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
-        };
-
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
@@ -484,12 +476,14 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             while (have) {
                 int un, hn, s0n, offn;
                 const bool more = walk.next(un, hn, s0n, offn);
+                PT_MARK(0);
                 compute_dS(st_cur);
+                PT_MARK(2);
                 if (more) {
                     st_cur = next_stage();
                     compute_P(st_cur, c.it.t0, s0n, offn);
                 }
-                drain_dQ(c.it.batch, u, h, s0);
+                PT_MARK(4);
                 u = un; h = hn; s0 = s0n; off = offn;
                 have = more;
             }
@@ -503,6 +497,45 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             mbar_arrive(dkv_empty);
         }
+        PT_REPORT("bwd compute clocks per step: wait dP, dS, wait S, P, 0");
+    }
+    else if (warp >= 12) {
+        // =============================== dQ drain group ===============================
+        // thread = head-dim index d (TMEM lane): dQ^T row d, all 128 queries of the step -> registers (the TMEM columns are
+        // released at once) -> one line-coalesced atomic per (query, 32 consecutive d) while the next step's MMAs run
+        reg_alloc<kDrainRegs>();
+        const int d = ((warp & 3) << 5) | lane;
+        const uint32_t tDQ = tmem + ((uint32_t)((warp & 3) * 32) << 16) + Cfg::kColDP;
+        const size_t rs = (size_t)p.q_stride_row;
+        uint32_t dq_ph = 0;
+        PT_DECL;
+        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            const BwdItemCtx c = load_bwd_item(p, idx);
+            QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
+            int u, h, s0, off;
+            while (walk.next(u, h, s0, off)) {
+                float* ptr = p.dQ + (size_t)c.it.batch * p.q_stride_b + ((size_t)u * gm.L + s0) * p.q_stride_row + (size_t)h * p.q_stride_h + d;
+                PT_MARK(0);
+                mbar_wait(dq_full, dq_ph);
+                dq_ph ^= 1;
+                tc_fence_after();
+                uint32_t r[kBlock];
+#pragma unroll
+                for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tDQ + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[ch * 32]));
+                tmem_ld_wait();
+                tc_fence_before();
+                mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
+                PT_MARK(1);
+#pragma unroll
+#ifdef MESH_ATTN_EXPERIMENT_NO_DQ_RED
+                if (__uint_as_float(r[5]) == 123.456f) red_add(ptr, __uint_as_float(r[7]));
+#else
+                for (int j = 0; j < kBlock; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
+#endif
+                PT_MARK(2);
+            }
+        }
+        PT_REPORT("bwd drain clocks per step: wait dQ + ld, reds, 0, 0, 0");
     }
 
     tc_fence_before();

@@ -33,18 +33,8 @@ constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
 constexpr int kCtrlRegs = 88, kSoftmaxRegs = 208;
 constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
 #ifndef MESH_ATTN_POLY_OF_8
-#define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU
-#endif
-
-// optional per-phase clock accounting of one softmax thread (tuning builds only: -DMESH_ATTN_PHASE_TIMING)
-#ifdef MESH_ATTN_PHASE_TIMING
-#define PT_DECL long long pt_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long pt_last = clock64(); long long pt_n = 0
-#define PT_MARK(k) do { const long long pt_now = clock64(); pt_acc[k] += pt_now - pt_last; pt_last = pt_now; if ((k) == 0) ++pt_n; } while (0)
-#define PT_REPORT(what) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && pt_n) printf("%s | thread %d blocks %lld: %lld %lld %lld %lld %lld (loop-back %lld)\n", what, threadIdx.x, pt_n, pt_acc[1] / pt_n, pt_acc[2] / pt_n, pt_acc[3] / pt_n, pt_acc[4] / pt_n, pt_acc[5] / pt_n, pt_acc[0] / pt_n); } while (0)
-#else
-#define PT_DECL
-#define PT_MARK(k)
-#define PT_REPORT(what)
+#define MESH_ATTN_POLY_OF_8 0            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU (measured: 0 is fastest,
+                                         // the softmax warps are issue-bound, not MUFU-bound; profiles/r01_v3_README.md)
 #endif
 
 template <int N> struct IntTag { static constexpr int value = N; };
@@ -342,7 +332,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 const float neg_m = (m == -INFINITY) ? 0.f : -m;
                 // p = exp2(s*c2 - m).  Unmasked blocks: kPolyOf8 of every 8 on the FMA pipe (degree-3 polynomial), the
                 // rest on the MUFU; diagonal blocks: all on the MUFU (exp2(-inf) must be exactly 0 there).
-                float l0 = 0.f, l1 = 0.f, l2 = 0.f, l3 = 0.f;
+                f32x2 lacc0 = 0ull, lacc1 = 0ull;                    // two (even, odd) partial row sums
+                const f32x2 c22 = pack2(c2, c2), nm2 = pack2(neg_m, neg_m);
                 auto exp_row = [&](auto poly_tag) {
                     constexpr int kPoly = decltype(poly_tag)::value;
 #pragma unroll
@@ -350,11 +341,12 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         uint32_t hi[16], lo[16];
 #pragma unroll
                         for (int i = 0; i < 32; i += 2) {
-                            const float x0 = fmaf(__uint_as_float(s[ch * 32 + i]), c2, neg_m);
-                            const float x1 = fmaf(__uint_as_float(s[ch * 32 + i + 1]), c2, neg_m);
+                            float x0, x1;
+                            unpack2(fma2(pack2(__uint_as_float(s[ch * 32 + i]), __uint_as_float(s[ch * 32 + i + 1])), c22, nm2), x0, x1);
                             const float p0 = ((i & 7) < kPoly) ? ex2_poly(x0) : ex2(x0);
                             const float p1 = (((i + 1) & 7) < kPoly) ? ex2_poly(x1) : ex2(x1);
-                            if ((i & 2) == 0) { l0 += p0; l1 += p1; } else { l2 += p0; l3 += p1; }
+                            if ((i & 2) == 0) lacc0 = add2(lacc0, pack2(p0, p1));
+                            else lacc1 = add2(lacc1, pack2(p0, p1));
                             if constexpr (kSplit) split_bf16x2(p0, p1, hi[i / 2], lo[i / 2]);
                             else hi[i / 2] = pack_bf16x2(p0, p1);
                         }
@@ -365,7 +357,9 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 };
                 if (masked) exp_row(IntTag<0>{});
                 else exp_row(IntTag<MESH_ATTN_POLY_OF_8>{});
-                l += (l0 + l1) + (l2 + l3);
+                float l0, l1;
+                unpack2(add2(lacc0, lacc1), l0, l1);
+                l += l0 + l1;
                 PT_MARK(4);
                 tmem_st_wait();
                 tc_fence_before();
