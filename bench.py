@@ -219,6 +219,23 @@ def workload_config(w, note=""):
     return cfg
 
 
+# ------------------------------------------------------------------------------------------ multi-rank bookkeeping
+def max_over_ranks(ms: float, dist, device) -> float:
+    """Timing of the whole job = the slowest rank (replicas run independently)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return float(ms)
+    import torch
+
+    t = torch.tensor([ms], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_tflops(flops_per_rank_step: float, world: int, steps: int, ms_total: float) -> float:
+    """value = units all ranks processed / max-over-ranks time (weak scaling: every rank runs the full workload)."""
+    return world * flops_per_rank_step * steps / (ms_total / 1e3) / 1e12
+
+
 # ------------------------------------------------------------------------------------------ GPU arm
 def physical_gpu_index(local_rank: int) -> int:
     """nvidia-smi index of this rank's GPU (CUDA_VISIBLE_DEVICES may renumber them)."""
@@ -336,26 +353,20 @@ def run_ours(args):
     prof = {name: B.profile_read(kind) for name, kind in (("tile_fwd", B.K_TILE_FWD), ("merge", B.K_MERGE),
                                                           ("bwd_preprocess", B.K_BWD_PREPROCESS), ("tile_bwd", B.K_TILE_BWD))}
     B.profile_enable(False)
-    if dist is not None:
-        t = torch.tensor([ms_total], device="cuda", dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
 
     K = args.steps
     fl_fwd, fl_bwd = plan.query(B.Q_FLOPS_FWD), (plan.query(B.Q_FLOPS_BWD) if w.backward else 0)
     sec = ms_total / 1e3
-    value = world * (fl_fwd + fl_bwd) * K / sec / 1e12
+    value = whole_job_tflops(fl_fwd + fl_bwd, world, K, ms_total)
 
     e2e = None
     if not args.no_e2e:
         try:
             e2e_steps = 1 if ms_total / K > 2000 else min(K, 5)
             ms_e, h2d, d2h, pinned = run_e2e(plan, w, inp, buf, torch, e2e_steps)
-            if dist is not None:
-                t = torch.tensor([ms_e], device="cuda", dtype=torch.float64)
-                dist.all_reduce(t, op=dist.ReduceOp.MAX)
-                ms_e = float(t.item())
-            e2e = {"value": world * (fl_fwd + fl_bwd) / (ms_e / 1e3) / 1e12, "unit": UNIT, "h2d_bytes_per_step": h2d,
+            ms_e = max_over_ranks(ms_e, dist, "cuda")
+            e2e = {"value": whole_job_tflops(fl_fwd + fl_bwd, world, 1, ms_e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "ms_per_step": ms_e, "steps": e2e_steps, "pinned": pinned,
                    "api": "mesh_attn_step_host"}
         except (RuntimeError, MemoryError) as ex:                # host memory too small for the host mirrors
