@@ -29,6 +29,9 @@ if str(ROOT) not in sys.path:
 METRIC = "attention_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one ncu capture of this command
+# (profiles/r01_v3_traffic_c5_tile_bwd.csv; profiles/r01_v3_ncu_c2_bwd.txt): workload -> kernel -> bytes
+NCU_TRAFFIC = {"C5": {"tile_bwd": 3720749815296 + 1899515161600}, "C2": {"tile_bwd": 4042925000 + 2411813000, "tile_fwd": 921501440 + 571924992}}
 
 
 def parse_args():
@@ -384,7 +387,7 @@ def run_ours(args):
     peak = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
     ach = dom_flops / (dom_ms / 1e3) / 1e12 if dom_ms > 0 else 0.0
     roofline = {"kernel": f"mesh_attn_{dom}", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": None, "launches": dom_n, "avg_launch_ms": dom_ms / max(1, dom_n),
+                "frac": ach / peak, "traffic": NCU_TRAFFIC.get(w.name, {}).get(dom), "launches": dom_n, "avg_launch_ms": dom_ms / max(1, dom_n),
                 "algorithmic_flops_per_launch": dom_flops / max(1, dom_n),
                 "peak_kind": f"{peak_src} dense bf16, " + ("sustained (kernel timed inside a long step)" if long_step else "burst"),
                 "share_of_step": dom_ms / ms_total}

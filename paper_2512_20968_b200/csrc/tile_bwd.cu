@@ -47,6 +47,10 @@ using namespace sm100;
 namespace {
 
 constexpr int kBwdThreads = 512;
+#ifndef MESH_ATTN_BWD_POLY_OF_4
+#define MESH_ATTN_BWD_POLY_OF_4 0        // exponentials per 4 evaluated on the FMA pipe instead of the MUFU
+#endif
+constexpr int kBwdPolyOf4 = MESH_ATTN_BWD_POLY_OF_4;
 // register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs + 128 x kDrainRegs <= 65536
 constexpr int kCtrlRegs = 72, kComputeRegs = 136, kDrainRegs = 160;
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
@@ -135,13 +139,6 @@ __device__ __forceinline__ void red_add(float* addr, float a)
 {
     asm volatile("red.global.add.f32 [%0], %1;" ::"l"(addr), "f"(a) : "memory");
 }
-// hi = bf16(x), lo = bf16(x - hi): packs two values' hi parts and lo parts
-__device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t& hi, uint32_t& lo)
-{
-    hi = pack_bf16x2(x0, x1);
-    lo = pack_bf16x2(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xffff0000u));
-}
-
 // TMEM accumulator [128 lanes x D columns] -> x scale -> atomic add into a global row of D floats
 // (item epilogue only: once per 128-key block)
 template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, float* grow, float scale)
@@ -317,6 +314,22 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     ds_ph ^= 1;
                     tc_fence_after();
                     PT_MARK(3);
+#ifdef MESH_ATTN_BWD_DQ_FIRST
+#pragma unroll
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
+#pragma unroll
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
+                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
+                    umma_commit(dq_full);
+#pragma unroll
+                    for (int x = 0; x < Cfg::kNumDs; ++x)
+#pragma unroll
+                        for (int kk = 0; kk < kBlock / 16; ++kk)
+                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
+                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
+                    umma_commit(&qd_empty[st_cur]);
+#else
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
@@ -331,6 +344,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
                                     umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
                     umma_commit(dq_full);
+#endif
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
@@ -369,6 +383,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         uint8_t* sDsHalf = sDs + wg * (kBlock * 128);                     // [128 key rows][64 queries] bf16, 128-byte swizzled rows
         uint32_t stage = 0, ring_phase = 0, s_ph = 0, dp_ph = 0, dq_ph = 0, dkv_ph = 0;
         float pr[64];                                                     // P^T of the current step (fp32), reused for dS^T
+        const f32x2 c22 = pack2(gm.scale_log2, gm.scale_log2);
         PT_DECL;
 
         auto next_stage = [&]() {
@@ -394,10 +409,14 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 #pragma unroll
                 for (int q4 = 0; q4 < 32; q4 += 4) {
                     const float4 l4 = nl4[ch * 8 + q4 / 4];
-                    pr[ch * 32 + q4 + 0] = ex2(fmaf(__uint_as_float(r[q4 + 0]), gm.scale_log2, l4.x));
-                    pr[ch * 32 + q4 + 1] = ex2(fmaf(__uint_as_float(r[q4 + 1]), gm.scale_log2, l4.y));
-                    pr[ch * 32 + q4 + 2] = ex2(fmaf(__uint_as_float(r[q4 + 2]), gm.scale_log2, l4.z));
-                    pr[ch * 32 + q4 + 3] = ex2(fmaf(__uint_as_float(r[q4 + 3]), gm.scale_log2, l4.w));
+                    float x0, x1, x2, x3;
+                    unpack2(fma2(pack2(__uint_as_float(r[q4 + 0]), __uint_as_float(r[q4 + 1])), c22, pack2(l4.x, l4.y)), x0, x1);
+                    unpack2(fma2(pack2(__uint_as_float(r[q4 + 2]), __uint_as_float(r[q4 + 3])), c22, pack2(l4.z, l4.w)), x2, x3);
+                    // kBwdPolyOf4 of every 4 exponentials on the FMA pipe, the rest on the MUFU (x <= 0 here: P <= scale)
+                    pr[ch * 32 + q4 + 0] = (0 < kBwdPolyOf4) ? ex2_poly(x0) : ex2(x0);
+                    pr[ch * 32 + q4 + 1] = (1 < kBwdPolyOf4) ? ex2_poly(x1) : ex2(x1);
+                    pr[ch * 32 + q4 + 2] = (2 < kBwdPolyOf4) ? ex2_poly(x2) : ex2(x2);
+                    pr[ch * 32 + q4 + 3] = (3 < kBwdPolyOf4) ? ex2_poly(x3) : ex2(x3);
                 }
             }
             if (masked) {
@@ -444,10 +463,11 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 for (int k = 0; k < 4; ++k) {                              // 8 columns = one 16-byte chunk of the row
                     const float4 da = dl4[ch * 8 + k * 2], db = dl4[ch * 8 + k * 2 + 1];
                     const int c = ch * 32 + k * 8;
-                    const float d0 = pr[c + 0] * (__uint_as_float(r[k * 8 + 0]) - da.x), d1 = pr[c + 1] * (__uint_as_float(r[k * 8 + 1]) - da.y);
-                    const float d2 = pr[c + 2] * (__uint_as_float(r[k * 8 + 2]) - da.z), d3 = pr[c + 3] * (__uint_as_float(r[k * 8 + 3]) - da.w);
-                    const float d4 = pr[c + 4] * (__uint_as_float(r[k * 8 + 4]) - db.x), d5 = pr[c + 5] * (__uint_as_float(r[k * 8 + 5]) - db.y);
-                    const float d6 = pr[c + 6] * (__uint_as_float(r[k * 8 + 6]) - db.z), d7 = pr[c + 7] * (__uint_as_float(r[k * 8 + 7]) - db.w);
+                    float d0, d1, d2, d3, d4, d5, d6, d7;        // dS = P o (dP - delta), two elements per instruction
+                    unpack2(mul2(pack2(pr[c + 0], pr[c + 1]), add2(pack2(__uint_as_float(r[k * 8 + 0]), __uint_as_float(r[k * 8 + 1])), pack2(-da.x, -da.y))), d0, d1);
+                    unpack2(mul2(pack2(pr[c + 2], pr[c + 3]), add2(pack2(__uint_as_float(r[k * 8 + 2]), __uint_as_float(r[k * 8 + 3])), pack2(-da.z, -da.w))), d2, d3);
+                    unpack2(mul2(pack2(pr[c + 4], pr[c + 5]), add2(pack2(__uint_as_float(r[k * 8 + 4]), __uint_as_float(r[k * 8 + 5])), pack2(-db.x, -db.y))), d4, d5);
+                    unpack2(mul2(pack2(pr[c + 6], pr[c + 7]), add2(pack2(__uint_as_float(r[k * 8 + 6]), __uint_as_float(r[k * 8 + 7])), pack2(-db.z, -db.w))), d6, d7);
                     const uint32_t o = sw128_offset(row, ch * 4 + k);
                     if constexpr (!kSplit) {
                         *reinterpret_cast<uint4*>(sDsHalf + o) =

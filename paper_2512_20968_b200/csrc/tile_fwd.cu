@@ -41,26 +41,6 @@ template <int N> struct IntTag { static constexpr int value = N; };
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
-// 2^x for x <= ~8 on the FMA/ALU pipes: round to nearest integer n with the 1.5*2^23 trick, degree-3 minimax
-// polynomial of 2^f on f = x - n in [-0.5, 0.5] (max relative error 7.5e-5, below the 2^-9 rounding of the bf16
-// P operand), then add n to the exponent field.  Inputs below -126 give ~2^-126 instead of 0.
-__device__ __forceinline__ float ex2_poly(float x)
-{
-    x = fmaxf(x, -126.f);
-    const float xr = x + 12582912.f;
-    const float f = x - (xr - 12582912.f);
-    float q = fmaf(0.0551716648f, f, 0.2426111251f);
-    q = fmaf(q, f, 0.6932609677f);
-    q = fmaf(q, f, 0.9999280572f);
-    return __int_as_float(__float_as_int(q) + (__float_as_int(xr) << 23));
-}
-// hi = bf16(x), lo = bf16(x - hi) for two values
-__device__ __forceinline__ void split_bf16x2(float x0, float x1, uint32_t& hi, uint32_t& lo)
-{
-    hi = pack_bf16x2(x0, x1);
-    lo = pack_bf16x2(x0 - __uint_as_float(hi << 16), x1 - __uint_as_float(hi & 0xffff0000u));
-}
-
 template <int D> struct FwdCfg {
     static constexpr int kBoxes = D / 64;                  // 64-element (128-byte) TMA boxes per row
     static constexpr int kTileBytes = kBlock * D * 2;      // one [128 x D] bf16 tile
