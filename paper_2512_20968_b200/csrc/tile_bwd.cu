@@ -401,23 +401,21 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             s_ph ^= 1;
             tc_fence_after();
             PT_MARK(3);
+            uint32_t(&pu)[64] = reinterpret_cast<uint32_t(&)[64]>(pr);      // S^T lands in the registers P^T is computed in
+            tmem_ld_x32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pu[0]));
+            tmem_ld_x32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pu[32]));
+            tmem_ld_wait();
 #pragma unroll
-            for (int ch = 0; ch < 2; ++ch) {
-                uint32_t r[32];
-                tmem_ld_x32(tS + ch * 32, r);
-                tmem_ld_wait();
-#pragma unroll
-                for (int q4 = 0; q4 < 32; q4 += 4) {
-                    const float4 l4 = nl4[ch * 8 + q4 / 4];
-                    float x0, x1, x2, x3;
-                    unpack2(fma2(pack2(__uint_as_float(r[q4 + 0]), __uint_as_float(r[q4 + 1])), c22, pack2(l4.x, l4.y)), x0, x1);
-                    unpack2(fma2(pack2(__uint_as_float(r[q4 + 2]), __uint_as_float(r[q4 + 3])), c22, pack2(l4.z, l4.w)), x2, x3);
-                    // kBwdPolyOf4 of every 4 exponentials on the FMA pipe, the rest on the MUFU (x <= 0 here: P <= scale)
-                    pr[ch * 32 + q4 + 0] = (0 < kBwdPolyOf4) ? ex2_poly(x0) : ex2(x0);
-                    pr[ch * 32 + q4 + 1] = (1 < kBwdPolyOf4) ? ex2_poly(x1) : ex2(x1);
-                    pr[ch * 32 + q4 + 2] = (2 < kBwdPolyOf4) ? ex2_poly(x2) : ex2(x2);
-                    pr[ch * 32 + q4 + 3] = (3 < kBwdPolyOf4) ? ex2_poly(x3) : ex2(x3);
-                }
+            for (int q4 = 0; q4 < 64; q4 += 4) {
+                const float4 l4 = nl4[q4 / 4];
+                float x0, x1, x2, x3;
+                unpack2(fma2(pack2(pr[q4 + 0], pr[q4 + 1]), c22, pack2(l4.x, l4.y)), x0, x1);
+                unpack2(fma2(pack2(pr[q4 + 2], pr[q4 + 3]), c22, pack2(l4.z, l4.w)), x2, x3);
+                // kBwdPolyOf4 of every 4 exponentials on the FMA pipe, the rest on the MUFU (x <= 0 here: P <= scale)
+                pr[q4 + 0] = (0 < kBwdPolyOf4) ? ex2_poly(x0) : ex2(x0);
+                pr[q4 + 1] = (1 < kBwdPolyOf4) ? ex2_poly(x1) : ex2(x1);
+                pr[q4 + 2] = (2 < kBwdPolyOf4) ? ex2_poly(x2) : ex2(x2);
+                pr[q4 + 3] = (3 < kBwdPolyOf4) ? ex2_poly(x3) : ex2(x3);
             }
             if (masked) {
                 const int cmin = t0 + row - off - s0 - wg * 64;            // local query column c visible to this key iff c >= cmin
@@ -454,21 +452,18 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             dp_ph ^= 1;
             tc_fence_after();
             PT_MARK(1);
+            uint32_t ra[16], rb[16];             // 16-column chunks: chunk c+1 is in flight while chunk c is processed
+            auto ds_chunk = [&](int c16, const uint32_t (&r)[16]) {
 #pragma unroll
-            for (int ch = 0; ch < 2; ++ch) {
-                uint32_t r[32];
-                tmem_ld_x32(tDP + ch * 32, r);
-                tmem_ld_wait();
-#pragma unroll
-                for (int k = 0; k < 4; ++k) {                              // 8 columns = one 16-byte chunk of the row
-                    const float4 da = dl4[ch * 8 + k * 2], db = dl4[ch * 8 + k * 2 + 1];
-                    const int c = ch * 32 + k * 8;
+                for (int k = 0; k < 2; ++k) {                              // 8 columns = one 16-byte chunk of the row
+                    const float4 da = dl4[c16 * 4 + k * 2], db = dl4[c16 * 4 + k * 2 + 1];
+                    const int c = c16 * 16 + k * 8;
                     float d0, d1, d2, d3, d4, d5, d6, d7;        // dS = P o (dP - delta), two elements per instruction
                     unpack2(mul2(pack2(pr[c + 0], pr[c + 1]), add2(pack2(__uint_as_float(r[k * 8 + 0]), __uint_as_float(r[k * 8 + 1])), pack2(-da.x, -da.y))), d0, d1);
                     unpack2(mul2(pack2(pr[c + 2], pr[c + 3]), add2(pack2(__uint_as_float(r[k * 8 + 2]), __uint_as_float(r[k * 8 + 3])), pack2(-da.z, -da.w))), d2, d3);
                     unpack2(mul2(pack2(pr[c + 4], pr[c + 5]), add2(pack2(__uint_as_float(r[k * 8 + 4]), __uint_as_float(r[k * 8 + 5])), pack2(-db.x, -db.y))), d4, d5);
                     unpack2(mul2(pack2(pr[c + 6], pr[c + 7]), add2(pack2(__uint_as_float(r[k * 8 + 6]), __uint_as_float(r[k * 8 + 7])), pack2(-db.z, -db.w))), d6, d7);
-                    const uint32_t o = sw128_offset(row, ch * 4 + k);
+                    const uint32_t o = sw128_offset(row, c16 * 2 + k);
                     if constexpr (!kSplit) {
                         *reinterpret_cast<uint4*>(sDsHalf + o) =
                             make_uint4(pack_bf16x2(d0, d1), pack_bf16x2(d2, d3), pack_bf16x2(d4, d5), pack_bf16x2(d6, d7));
@@ -480,7 +475,19 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         *reinterpret_cast<uint4*>(sDsHalf + Cfg::kDsBytes + o) = make_uint4(l0, l1, l2, l3);
                     }
                 }
-            }
+            };
+            tmem_ld_x16(tDP, ra);
+            tmem_ld_wait();
+            tmem_ld_x16(tDP + 16, rb);
+            ds_chunk(0, ra);
+            tmem_ld_wait();
+            tmem_ld_x16(tDP + 32, ra);
+            ds_chunk(1, rb);
+            tmem_ld_wait();
+            tmem_ld_x16(tDP + 48, rb);
+            ds_chunk(2, ra);
+            tmem_ld_wait();
+            ds_chunk(3, rb);
             fence_proxy_async_smem();
             tc_fence_before();
             mbar_arrive(ds_full);
