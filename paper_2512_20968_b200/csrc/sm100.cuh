@@ -14,7 +14,7 @@
 #ifdef MESH_ATTN_PHASE_TIMING
 #define PT_DECL long long pt_acc[8] = {0, 0, 0, 0, 0, 0, 0, 0}; long long pt_last = clock64(); long long pt_n = 0
 #define PT_MARK(k) do { const long long pt_now = clock64(); pt_acc[k] += pt_now - pt_last; pt_last = pt_now; if ((k) == 0) ++pt_n; } while (0)
-#define PT_REPORT(what) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && pt_n) printf("%s | thread %d blocks %lld: %lld %lld %lld %lld %lld (loop-back %lld)\n", what, threadIdx.x, pt_n, pt_acc[1] / pt_n, pt_acc[2] / pt_n, pt_acc[3] / pt_n, pt_acc[4] / pt_n, pt_acc[5] / pt_n, pt_acc[0] / pt_n); } while (0)
+#define PT_REPORT(what) do { if (blockIdx.x == 0 && (threadIdx.x & 31) == 0 && pt_n) printf("%s | thread %d blocks %lld: %lld %lld %lld %lld %lld %lld %lld (loop-back %lld)\n", what, threadIdx.x, pt_n, pt_acc[1] / pt_n, pt_acc[2] / pt_n, pt_acc[3] / pt_n, pt_acc[4] / pt_n, pt_acc[5] / pt_n, pt_acc[6] / pt_n, pt_acc[7] / pt_n, pt_acc[0] / pt_n); } while (0)
 #else
 #define PT_DECL
 #define PT_MARK(k)

@@ -314,22 +314,6 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     ds_ph ^= 1;
                     tc_fence_after();
                     PT_MARK(3);
-#ifdef MESH_ATTN_BWD_DQ_FIRST
-#pragma unroll
-                    for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
-                        for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
-                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(dq_full);
-#pragma unroll
-                    for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
-                        for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
-                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(&qd_empty[st_cur]);
-#else
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
@@ -344,7 +328,6 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                             umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
                                     umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
                     umma_commit(dq_full);
-#endif
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
@@ -478,6 +461,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             };
             tmem_ld_x16(tDP, ra);
             tmem_ld_wait();
+            PT_MARK(5);
             tmem_ld_x16(tDP + 16, rb);
             ds_chunk(0, ra);
             tmem_ld_wait();
@@ -488,6 +472,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             ds_chunk(2, ra);
             tmem_ld_wait();
             ds_chunk(3, rb);
+            PT_MARK(6);
             fence_proxy_async_smem();
             tc_fence_before();
             mbar_arrive(ds_full);
@@ -524,7 +509,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             mbar_arrive(dkv_empty);
         }
-        PT_REPORT("bwd compute clocks per step: wait dP, dS, wait S, P, 0");
+        PT_REPORT("bwd compute clocks per step: wait dP, fence+arrive(ds), wait S, P, first dP ld, dS chunks, 0");
     }
     else if (warp >= 12) {
         // =============================== dQ drain group ===============================
@@ -554,11 +539,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
                 PT_MARK(1);
 #pragma unroll
-#ifdef MESH_ATTN_EXPERIMENT_NO_DQ_RED
-                if (__uint_as_float(r[5]) == 123.456f) red_add(ptr, __uint_as_float(r[7]));
-#else
                 for (int j = 0; j < kBlock; ++j) { red_add(ptr, __uint_as_float(r[j])); ptr += rs; }
-#endif
                 PT_MARK(2);
             }
         }
