@@ -33,8 +33,8 @@ constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
 constexpr int kCtrlRegs = 88, kSoftmaxRegs = 208;
 constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
 #ifndef MESH_ATTN_POLY_OF_8
-#define MESH_ATTN_POLY_OF_8 0            // exponentials per 8 evaluated on the FMA pipe instead of the MUFU (measured: 0 is fastest,
-                                         // the softmax warps are issue-bound, not MUFU-bound; profiles/r01_v3_README.md)
+#define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe (packed fp32x2 polynomial) instead of the
+                                         // MUFU: measured 0 / 2 / 4 of 8 -> 6.08 / 5.89 / 6.19 ms per C2 launch (profiles/r01_v3_README.md)
 #endif
 
 template <int N> struct IntTag { static constexpr int value = N; };
@@ -323,8 +323,9 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         for (int i = 0; i < 32; i += 2) {
                             float x0, x1;
                             unpack2(fma2(pack2(__uint_as_float(s[ch * 32 + i]), __uint_as_float(s[ch * 32 + i + 1])), c22, nm2), x0, x1);
-                            const float p0 = ((i & 7) < kPoly) ? ex2_poly(x0) : ex2(x0);
-                            const float p1 = (((i + 1) & 7) < kPoly) ? ex2_poly(x1) : ex2(x1);
+                            float p0, p1;
+                            if ((i & 7) < kPoly) ex2_poly2(x0, x1, p0, p1);       // pairs: kPoly of every 8 elements
+                            else { p0 = ex2(x0); p1 = ex2(x1); }
                             if ((i & 2) == 0) lacc0 = add2(lacc0, pack2(p0, p1));
                             else lacc1 = add2(lacc1, pack2(p0, p1));
                             if constexpr (kSplit) split_bf16x2(p0, p1, hi[i / 2], lo[i / 2]);
