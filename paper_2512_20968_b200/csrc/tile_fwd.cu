@@ -47,7 +47,7 @@ template <int D> struct FwdCfg {
     static constexpr int kStages = D == 128 ? 5 : 8;       // K/V ring slots (each one tile)
     static constexpr int kSmemQ = 2 * kTileBytes;
     static constexpr int kSmemRing = kStages * kTileBytes;
-    static constexpr int kNumBars = 2 + 2 * kStages + 6;
+    static constexpr int kNumBars = 2 + 2 * kStages + 8;
     static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 1024;   // + alignment slack
     static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
 };
@@ -124,8 +124,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* kv_full = bars + 2;
     uint64_t* kv_empty = kv_full + Cfg::kStages;
     uint64_t* s_full = kv_empty + Cfg::kStages;   // [2]
-    uint64_t* p_full = s_full + 2;                // [2]
-    uint64_t* o_full = p_full + 2;                // [2]
+    uint64_t* p_half = s_full + 2;                // [2 sub-tiles][2 column halves]: P is handed to the PV MMA in two halves
+    uint64_t* o_full = p_half + 4;                // [2]
     uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_full + 2);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -137,7 +137,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(q_full, 1);
         mbar_init(q_empty, 1);
         for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
-        for (int t = 0; t < 2; ++t) { mbar_init(&s_full[t], 1); mbar_init(&p_full[t], kBlock); mbar_init(&o_full[t], 1); }
+        for (int t = 0; t < 2; ++t) { mbar_init(&s_full[t], 1); mbar_init(&o_full[t], 1); }
+        for (int t = 0; t < 4; ++t) mbar_init(&p_half[t], kBlock);
         fence_mbar_init();
     }
     if (warp == kAllocWarp) tmem_alloc<512>(tmem_slot);
@@ -197,14 +198,17 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     umma_ss(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc_qk, kk > 0);
                 }
             };
-            auto issue_pv = [&](int t, uint32_t vslot, bool acc) {      // P (bf16) in TMEM over S: hi at columns 0..63, lo at 64..127
+            // P (bf16) in TMEM over S: hi at columns 0..63, lo at 64..127; `half` = keys 0..63 or 64..127 of the block
+            auto issue_pv = [&](int t, uint32_t vslot, int half, bool acc) {
                 const uint32_t va = smem_u32(sRing + vslot * Cfg::kTileBytes);
 #pragma unroll
                 for (int x = 0; x < (kSplit ? 2 : 1); ++x)
 #pragma unroll
-                    for (int kk = 0; kk < kBlock / 16; ++kk)
+                    for (int k4 = 0; k4 < kBlock / 32; ++k4) {
+                        const int kk = half * (kBlock / 32) + k4;
                         umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + x * 64 + kk * 8,
-                                umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || kk > 0 || x > 0) ? 1u : 0u);
+                                umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || k4 > 0 || x > 0) ? 1u : 0u);
+                    }
             };
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const ItemCtx c = load_item(p, idx);
@@ -224,11 +228,14 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     if (more) ring_wait(kslot);
                     PT_MARK(1);
                     for (int t = 0; t < c.nt; ++t) {
-                        mbar_wait(&p_full[t], p_phase[t]);
+                        mbar_wait(&p_half[2 * t], p_phase[t]);       // the PV MMA starts on the first 64 keys while the softmax
+                        tc_fence_after();                             // group is still exponentiating the other 64
+                        PT_MARK(2 + 2 * t);
+                        issue_pv(t, vslot, 0, j > 0);
+                        mbar_wait(&p_half[2 * t + 1], p_phase[t]);
                         p_phase[t] ^= 1;
                         tc_fence_after();
-                        PT_MARK(2 + 2 * t);
-                        issue_pv(t, vslot, j > 0);
+                        issue_pv(t, vslot, 1, true);
                         if (more) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
                         else umma_commit(&o_full[t]);
                         PT_MARK(3 + 2 * t);
@@ -334,6 +341,11 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         // the whole S row is in registers: P (bf16) may overwrite any of its columns
                         tmem_st_x16(tS + ch * 16, hi);
                         if constexpr (kSplit) tmem_st_x16(tS + 64 + ch * 16, lo);
+                        if (ch & 1) {                                 // half of the keys done: hand it to the PV MMA
+                            tmem_st_wait();
+                            tc_fence_before();
+                            mbar_arrive(&p_half[2 * t + (ch >> 1)]);
+                        }
                     }
                 };
                 if (masked) exp_row(IntTag<0>{});
@@ -342,9 +354,6 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 unpack2(add2(lacc0, lacc1), l0, l1);
                 l += l0 + l1;
                 PT_MARK(4);
-                tmem_st_wait();
-                tc_fence_before();
-                mbar_arrive(&p_full[t]);
                 PT_MARK(5);
                 ++j;
             });
