@@ -52,7 +52,7 @@ constexpr int kBwdThreads = 512;
 #endif
 constexpr int kBwdPolyOf4 = MESH_ATTN_BWD_POLY_OF_4;
 // register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs + 128 x kDrainRegs <= 65536
-constexpr int kCtrlRegs = 72, kComputeRegs = 136, kDrainRegs = 160;
+constexpr int kCtrlRegs = 80, kComputeRegs = 136, kDrainRegs = 160;
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
@@ -74,22 +74,26 @@ template <int D, bool kSplit> struct BwdCfg {
     static constexpr uint32_t kColS = 0, kColDP = 128, kColDK = 256, kColDV = 384;
 };
 
-// Walks the 128-row Q blocks of a backward work item in plan order: for every segment
-// (Q partition u, local rows [begin, end)), every query head of the GQA group, every block with
-// at least one visible (query, key) pair.  Every role runs the same walk.
+// The 128-row Q blocks of a backward work item in plan order, as RUNS: for every segment (Q partition u, local rows
+// [begin, end)) and every query head of the GQA group, the consecutive blocks with at least one visible (query, key)
+// pair.  Every role iterates the same runs; inside a run a step is just s0 += 128, so the per-step state is two
+// registers and the segment bookkeeping (which may live in local memory) is touched once per run.
 struct QWalk {
     const Geom& gm;
     const Seg* segs;
     int nseg, g, v, t0, head_kv;
-    int si = -1, hh = 0, s = 0, s_lo = 0, s_hi = 0, u = 0, off = 0;
-    __device__ QWalk(const Geom& gm_, const Seg* segs_, int nseg_, int g_, int v_, int t0_, int head_kv_)
+    int si = -1, hh = 0, s_lo = 0, s_hi = 0, u = 0, off = 0;
+    __device__ __forceinline__ QWalk(const Geom& gm_, const Seg* segs_, int nseg_, int g_, int v_, int t0_, int head_kv_)
         : gm(gm_), segs(segs_), nseg(nseg_), g(g_), v(v_), t0(t0_), head_kv(head_kv_) {}
-    // next block: Q partition u, query head h, first local query row s0, causal offset off
-    __device__ bool next(int& u_out, int& h_out, int& s0_out, int& off_out)
+    // next run: Q partition u, query head h, first local query row s0, number of blocks n >= 1, causal offset off
+    __device__ bool next_run(int& u_out, int& h_out, int& s0_out, int& n_out, int& off_out)
     {
         while (true) {
-            if (si >= 0 && s < s_hi) { u_out = u; h_out = head_kv * gm.group + hh; s0_out = s; off_out = off; s += kBlock; return true; }
-            if (si >= 0 && s_lo < s_hi && ++hh < gm.group) { s = s_lo; continue; }
+            if (si >= 0 && s_lo < s_hi && hh < gm.group) {
+                u_out = u; h_out = head_kv * gm.group + hh; s0_out = s_lo; n_out = (s_hi - s_lo) / kBlock; off_out = off;
+                ++hh;
+                return true;
+            }
             if (++si >= nseg) return false;
             const Seg sg = segs[si];
             u = (g / gm.a) * gm.a + sg.part_local;
@@ -102,8 +106,26 @@ struct QWalk {
                 const int x = t0 - off - (kBlock - 1);          // first query row that sees key t0 is t0 - off
                 if (x > s_lo) s_lo = min(s_hi, ((x + kBlock - 1) / kBlock) * kBlock);
             }
-            s = s_lo;
         }
+    }
+    // total number of steps of the item (consumes the walk)
+    __device__ int count_steps()
+    {
+        int total = 0, a, b, c, n, d;
+        while (next_run(a, b, c, n, d)) total += n;
+        return total;
+    }
+};
+// One step forward over the runs: (u, h, off) change once per run, s0 advances by 128 inside it.
+struct QStep {
+    int u = 0, h = 0, s0 = 0, off = 0, left = 0;
+    __device__ __forceinline__ bool next(QWalk& w)
+    {
+        if (left > 0) { s0 += kBlock; --left; return true; }
+        int n;
+        if (!w.next_run(u, h, s0, n, off)) return false;
+        left = n - 1;
+        return true;
     }
 };
 
@@ -221,9 +243,10 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-                int u, h, s0, off;
+                QStep q;
                 bool first = true;
-                while (walk.next(u, h, s0, off)) {
+                while (q.next(walk)) {
+                    const int u = q.u, h = q.h, s0 = q.s0;
                     if (first) {
                         first = false;
                         mbar_wait(kv_empty, kv_phase ^ 1);
@@ -274,9 +297,10 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-                int u, h, s0, off, i = 0;
-                bool have = walk.next(u, h, s0, off);
-                if (!have) continue;
+                const int nsteps = walk.count_steps();
+                if (nsteps == 0) continue;
+                int i = 0;
+                bool have = true;
                 mbar_wait(kv_full, kv_phase);
                 kv_phase ^= 1;
                 mbar_wait(dkv_empty, dkve_ph ^ 1);      // previous item's dK/dV drained from TMEM
@@ -287,7 +311,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mma_kmajor(Cfg::kColDP, aV, smem_u32(sdO(st_cur)));
                 umma_commit(dp_full);
                 while (have) {
-                    const bool more = walk.next(u, h, s0, off);
+                    const bool more = i + 1 < nsteps;
                     const uint32_t aQ = smem_u32(sQ(st_cur)), adO = smem_u32(sdO(st_cur));
                     PT_MARK(0);
                     // dV += P^T dO   (P^T bf16 in TMEM: group w's 64 queries at columns 64w.. (hi) and 64w+32.. (lo))
@@ -480,23 +504,21 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-            int u, h, s0, off;
-            bool have = walk.next(u, h, s0, off);
+            QStep q;
+            bool have = q.next(walk);
             if (!have) continue;
             uint32_t st_cur = next_stage();
-            compute_P(st_cur, c.it.t0, s0, off);
+            compute_P(st_cur, c.it.t0, q.s0, q.off);
             while (have) {
-                int un, hn, s0n, offn;
-                const bool more = walk.next(un, hn, s0n, offn);
+                const bool more = q.next(walk);              // q now describes step i+1 (dS^T(i) needs nothing of step i)
                 PT_MARK(0);
                 compute_dS(st_cur);
                 PT_MARK(2);
                 if (more) {
                     st_cur = next_stage();
-                    compute_P(st_cur, c.it.t0, s0n, offn);
+                    compute_P(st_cur, c.it.t0, q.s0, q.off);
                 }
                 PT_MARK(4);
-                u = un; h = hn; s0 = s0n; off = offn;
                 have = more;
             }
             // epilogue: group 0 drains dK (x softmax scale), group 1 drains dV
@@ -524,9 +546,12 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
-            int u, h, s0, off;
-            while (walk.next(u, h, s0, off)) {
-                float* ptr = p.dQ + (size_t)c.it.batch * p.q_stride_b + ((size_t)u * gm.L + s0) * p.q_stride_row + (size_t)h * p.q_stride_h + d;
+            QStep q;
+            float* ptr = nullptr;
+            while (true) {
+                const bool in_run = q.left > 0;               // inside a run the next block's rows follow the previous one's
+                if (!q.next(walk)) break;
+                if (!in_run) ptr = p.dQ + (size_t)c.it.batch * p.q_stride_b + ((size_t)q.u * gm.L + q.s0) * p.q_stride_row + (size_t)q.h * p.q_stride_h + d;
                 PT_MARK(0);
                 mbar_wait(dq_full, dq_ph);
                 dq_ph ^= 1;
