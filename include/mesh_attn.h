@@ -91,7 +91,12 @@ enum {
     MESH_ATTN_Q_BLOCKS_FWD = 9,        /* 128x128 score blocks the forward computes (all GPUs, heads)     */
     MESH_ATTN_Q_COMM_UNITS = 10,       /* paper's aggregate communication units of this AM   */
     MESH_ATTN_Q_HAS_DEVICE = 11,       /* 1 if the plan's work lists are resident on a CUDA device        */
-    MESH_ATTN_Q_BWD_WS_BYTES = 12      /* bytes of the backward workspace bwd_ws: 2*B*Hq*N*4               */
+    MESH_ATTN_Q_BWD_WS_BYTES = 12,     /* bytes of the backward workspace bwd_ws: 2*B*Hq*N*4               */
+    /* planner analytics (what the paper's cluster would move; nothing here is executed): */
+    MESH_ATTN_Q_MESH_COMM_BYTES_FWD = 13,  /* per-GPU forward volume of this a x b tiling, closed form
+                                              2(a+b-2) N d / n elements x 2 bytes (bf16), d = Hq*head_dim */
+    MESH_ATTN_Q_MESH_COMM_BYTES_BWD = 14,  /* backward: twice the forward volume (Q,O,dO in, dQ out; K,V in, dK,dV out; Table 5) */
+    MESH_ATTN_Q_RING_COMM_BYTES_FWD = 15   /* Ring-Attention on the same n GPUs: (2 - 2/n) N d elements x 2 bytes */
 };
 
 /* kinds in mesh_attn_plan_steps rows (step, kind, i, j) */
@@ -131,6 +136,15 @@ int mesh_attn_plan_tiles(const mesh_attn_plan* plan, int32_t g, int32_t* tiles, 
 int mesh_attn_plan_steps(const mesh_attn_plan* plan, int32_t pass, int32_t* steps, int32_t capacity, int32_t* count);
 
 int mesh_attn_plan_query(const mesh_attn_plan* plan, int32_t what, int64_t* value);
+
+/* Topology-aware mapping: an alpha-wide, (gpus_per_node/alpha)-tall tile of the logical a x b mesh
+ * (rows = Q groups, columns = position inside the Q group) is placed on each node.  Returns the inter-node traffic of
+ * node `node` in units of one partition: q_units = 2 per remote member of every Q group the node intersects (Q in,
+ * partial O out), kv_units = 2 per remote member of every KV group it intersects (K and V).  alpha == a with
+ * gpus_per_node == a is the row-major mapping.  EINVAL unless alpha divides a and gpus_per_node, and
+ * gpus_per_node/alpha divides b. */
+int mesh_attn_plan_tam_units(const mesh_attn_plan* plan, int32_t gpus_per_node, int32_t alpha, int32_t node,
+                             int64_t* q_units, int64_t* kv_units);
 
 /* ---- hot path (device pointers; enqueued on stream) -------------------------------------- */
 

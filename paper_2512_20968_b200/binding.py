@@ -23,7 +23,8 @@ lib = C.CDLL(str(_LIB_PATH))
 
 OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 (Q_PARTIAL_O_BYTES, Q_PARTIAL_LSE_BYTES, Q_SLOTS_PER_GPU, Q_FLOPS_FWD, Q_FLOPS_BWD, Q_WAVES, Q_MERGE_BYTES,
- Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE, Q_BWD_WS_BYTES) = range(13)
+ Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE, Q_BWD_WS_BYTES,
+ Q_MESH_COMM_BYTES_FWD, Q_MESH_COMM_BYTES_BWD, Q_RING_COMM_BYTES_FWD) = range(16)
 TASK_AG_KV, TASK_AG_Q, TASK_RS_Q, TASK_C, TASK_RS_KV = range(5)
 
 
@@ -56,6 +57,7 @@ lib.mesh_attn_plan_footprint.argtypes = [_P, C.c_int32, _I32P, _I32P]
 lib.mesh_attn_plan_tiles.argtypes = [_P, C.c_int32, _I32P, C.c_int32, _I32P]
 lib.mesh_attn_plan_steps.argtypes = [_P, C.c_int32, _I32P, C.c_int32, _I32P]
 lib.mesh_attn_plan_query.argtypes = [_P, C.c_int32, C.POINTER(C.c_int64)]
+lib.mesh_attn_plan_tam_units.argtypes = [_P, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 lib.mesh_attn_tile_fwd.argtypes = [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P, _P]
 lib.mesh_attn_merge.argtypes = [_P, C.c_int32, _P, _P, _P, _P, _P]
 lib.mesh_attn_bwd_preprocess.argtypes = [_P] * 6
@@ -72,7 +74,7 @@ lib.mesh_attn_last_error.restype = C.c_char_p
 
 EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
-    "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
+    "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
 ]
@@ -136,6 +138,12 @@ class Plan:
         v = C.c_int64()
         _check(lib.mesh_attn_plan_query(self._h, what, C.byref(v)))
         return v.value
+
+    def tam_units(self, gpus_per_node: int, alpha: int, node: int = 0):
+        """(Q-dimension, KV-dimension) inter-node units of `node` under the alpha-wide node tile"""
+        q, kv = C.c_int64(), C.c_int64()
+        _check(lib.mesh_attn_plan_tam_units(self._h, gpus_per_node, alpha, node, C.byref(q), C.byref(kv)))
+        return q.value, kv.value
 
     def am(self) -> np.ndarray:
         n = self.desc.n

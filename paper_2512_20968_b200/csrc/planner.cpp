@@ -358,6 +358,33 @@ extern "C" int mesh_attn_plan_steps(const mesh_attn_plan* p, int32_t pass, int32
     return MESH_ATTN_OK;
 }
 
+extern "C" int mesh_attn_plan_tam_units(const mesh_attn_plan* p, int32_t gpus_per_node, int32_t alpha, int32_t node, int64_t* q_units,
+                             int64_t* kv_units)
+{
+    if (!p || !q_units || !kv_units) return fail(MESH_ATTN_EINVAL, "plan_tam_units: null pointer");
+    const Geom& gm = p->geom;
+    if (gpus_per_node <= 0 || alpha <= 0 || gm.a % alpha || gpus_per_node % alpha || gm.b % (gpus_per_node / alpha))
+        return fail(MESH_ATTN_EINVAL, "plan_tam_units: alpha must divide a and gpus_per_node, gpus_per_node/alpha must divide b");
+    const int rows_per_node = gpus_per_node / alpha, tiles_per_row = gm.a / alpha;
+    const int nodes = gm.n / gpus_per_node;
+    if (node < 0 || node >= nodes) return fail(MESH_ATTN_EINVAL, "plan_tam_units: node out of range");
+    // logical GPU g sits at mesh row r = g / a (its Q group) and column c = g mod a (its KV group)
+    auto node_of = [&](int g) { return ((g / gm.a) / rows_per_node) * tiles_per_row + (g % gm.a) / alpha; };
+    std::set<int> rows, cols;
+    for (int g = 0; g < gm.n; ++g)
+        if (node_of(g) == node) { rows.insert(g / gm.a); cols.insert(g % gm.a); }
+    int64_t q = 0, kv = 0;
+    for (int r : rows)                                     // Q group r = {r a .. r a + a - 1}
+        for (int x = r * gm.a; x < (r + 1) * gm.a; ++x)
+            if (node_of(x) != node) q += 2;
+    for (int c : cols)                                     // KV group c = {c, c + a, c + 2a, ...}
+        for (int x = c; x < gm.n; x += gm.a)
+            if (node_of(x) != node) kv += 2;
+    *q_units = q;
+    *kv_units = kv;
+    return MESH_ATTN_OK;
+}
+
 extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64_t* value)
 {
     if (!p || !value) return fail(MESH_ATTN_EINVAL, "plan_query: null argument");
@@ -401,6 +428,20 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             break;
         }
         case MESH_ATTN_Q_HAS_DEVICE: *value = p->d_blob ? 1 : 0; break;
+        case MESH_ATTN_Q_MESH_COMM_BYTES_FWD:
+        case MESH_ATTN_Q_MESH_COMM_BYTES_BWD: {
+            // each GPU gathers (a-1) remote Q and returns as many partial O, and gathers (b-1) remote
+            // K and V: 2(a-1) + 2(b-1) units of N d / n elements; the backward moves twice that (Table 5)
+            const long double unit = (long double)gm.batch * gm.n * gm.L * gm.heads_q * gm.head_dim / gm.n * 2.0L;
+            const long double fwd = 2.0L * (gm.a + gm.b - 2) * unit;
+            *value = (int64_t)(what == MESH_ATTN_Q_MESH_COMM_BYTES_FWD ? fwd : 2.0L * fwd);
+            break;
+        }
+        case MESH_ATTN_Q_RING_COMM_BYTES_FWD: {
+            const long double Nd = (long double)gm.batch * gm.n * gm.L * gm.heads_q * gm.head_dim * 2.0L;
+            *value = (int64_t)((2.0L - 2.0L / gm.n) * Nd);
+            break;
+        }
         case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * gm.heads_q * (int64_t)gm.n * gm.L * 4; break;
         default: return fail(MESH_ATTN_EINVAL, "plan_query: unknown query");
     }

@@ -1,5 +1,7 @@
 """C++ planner (through the C ABI, host only) against oracle/plan_oracle.py, the paper's printed
 examples and structural invariants.  No GPU needed."""
+from pathlib import Path
+
 import numpy as np
 import pytest
 
@@ -150,3 +152,32 @@ def test_compute_calls_fail_loudly_without_gpu():
     with pytest.raises(MeshAttnError) as e:
         p.tile_fwd(0, 1, 16, 16, 16, 16, 16, stream=0)
     assert e.value.status == B.ECUDA
+
+
+def test_planner_analytics_against_paper_numbers():
+    """S8(f).1: closed-form per-GPU volumes (Table 1 / Table 5) and the topology-aware mapping traffic (Section 3.6),
+    against the values the paper prints (tests/golden) and the independent planner oracle."""
+    from oracle import plan_oracle as po
+
+    gold = {}
+    for line in (Path(__file__).parent / "golden" / "paper_planner_examples.txt").read_text().splitlines():
+        if "=" in line and not line.startswith("#"):
+            k, v = line.split("#")[0].split("=")
+            gold[k.strip()] = v.strip()
+    gib = 2.0 ** 30
+    # 256 GPUs (16 x 16), 512K tokens, hidden 8192 = 64 heads x 128, BF16 (PAPER.md L300, Table 5)
+    p = B.Plan(a=16, b=16, batch=1, seq_total=524288, heads_q=64, heads_kv=64, head_dim=128)
+    fwd, bwd, ring = (p.query(x) for x in (B.Q_MESH_COMM_BYTES_FWD, B.Q_MESH_COMM_BYTES_BWD, B.Q_RING_COMM_BYTES_FWD))
+    assert round(fwd / gib, 1) == float(gold["mesh_16x16_fwd_gib"]) and round(bwd / gib, 1) == float(gold["mesh_16x16_bwd_gib"])
+    assert round(ring / gib, 1) == float(gold["ring_fwd_gib"])
+    assert fwd == int(po.mesh_volume_fwd(16, 16, 524288 * 8192) * 2)
+    # 64 GPUs, a = b = 8, 8 GPUs per node: row-major mapping (alpha = 8) vs 4-wide node tiles (P:L259-261)
+    p = B.Plan(a=8, b=8, batch=1, seq_total=8 * 8 * 128, heads_q=1, heads_kv=1, head_dim=128)
+    q, kv = p.tam_units(8, 8)
+    assert q == 0 and q + kv == int(gold["tam_alpha8_node0_units"])
+    assert p.tam_units(8, 4) == (int(gold["tam_alpha4_node0_q_units"]), int(gold["tam_alpha4_node0_kv_units"]))
+    for alpha in (1, 2, 4, 8):
+        for node in range(8):
+            assert p.tam_units(8, alpha, node) == po.tam_internode_units(8, 8, 8, alpha, node)
+    with pytest.raises(B.MeshAttnError):
+        p.tam_units(8, 3)
