@@ -137,6 +137,15 @@ int mesh_attn_plan_steps(const mesh_attn_plan* plan, int32_t pass, int32_t* step
 
 int mesh_attn_plan_query(const mesh_attn_plan* plan, int32_t what, int64_t* value);
 
+/* Timeline of the step list under the paper's execution model: in every step one collective runs
+ * concurrently with the step's compute tasks, which run one after the other; a step lasts
+ * max(T_comm, sum of T_compute) with the plan's task costs (the descriptor's, or the built-in model).
+ * Returns, in the cost unit: makespan = sum of step durations; serial = every task back to back (no overlap);
+ * exposed_comm = makespan - total compute time (the communication that compute does not hide, cf. Fig.7).
+ * With order == 0 (row-major, no overlap scheduled) makespan == serial.
+ * pass: 0 forward, 1 backward (backward costs: AG of Q,O,dO = 3 x t_ag_q, compute = 2.5 x t_c; reading R12). */
+int mesh_attn_plan_timeline(const mesh_attn_plan* plan, int32_t pass, double* makespan, double* serial, double* exposed_comm);
+
 /* Topology-aware mapping: an alpha-wide, (gpus_per_node/alpha)-tall tile of the logical a x b mesh
  * (rows = Q groups, columns = position inside the Q group) is placed on each node.  Returns the inter-node traffic of
  * node `node` in units of one partition: q_units = 2 per remote member of every Q group the node intersects (Q in,

@@ -57,6 +57,7 @@ lib.mesh_attn_plan_footprint.argtypes = [_P, C.c_int32, _I32P, _I32P]
 lib.mesh_attn_plan_tiles.argtypes = [_P, C.c_int32, _I32P, C.c_int32, _I32P]
 lib.mesh_attn_plan_steps.argtypes = [_P, C.c_int32, _I32P, C.c_int32, _I32P]
 lib.mesh_attn_plan_query.argtypes = [_P, C.c_int32, C.POINTER(C.c_int64)]
+lib.mesh_attn_plan_timeline.argtypes = [_P, C.c_int32] + [C.POINTER(C.c_double)] * 3
 lib.mesh_attn_plan_tam_units.argtypes = [_P, C.c_int32, C.c_int32, C.c_int32, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
 lib.mesh_attn_tile_fwd.argtypes = [_P, C.c_int32, C.c_int32, _P, _P, _P, _P, _P, _P]
 lib.mesh_attn_merge.argtypes = [_P, C.c_int32, _P, _P, _P, _P, _P]
@@ -74,7 +75,7 @@ lib.mesh_attn_last_error.restype = C.c_char_p
 
 EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
-    "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
+    "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
 ]
@@ -138,6 +139,12 @@ class Plan:
         v = C.c_int64()
         _check(lib.mesh_attn_plan_query(self._h, what, C.byref(v)))
         return v.value
+
+    def timeline(self, backward: bool = False):
+        """(makespan, serial time, exposed communication) of the step list in the plan's cost units"""
+        m, s, e = C.c_double(), C.c_double(), C.c_double()
+        _check(lib.mesh_attn_plan_timeline(self._h, int(backward), C.byref(m), C.byref(s), C.byref(e)))
+        return m.value, s.value, e.value
 
     def tam_units(self, gpus_per_node: int, alpha: int, node: int = 0):
         """(Q-dimension, KV-dimension) inter-node units of `node` under the alpha-wide node tile"""

@@ -358,6 +358,42 @@ extern "C" int mesh_attn_plan_steps(const mesh_attn_plan* p, int32_t pass, int32
     return MESH_ATTN_OK;
 }
 
+extern "C" int mesh_attn_plan_timeline(const mesh_attn_plan* p, int32_t pass, double* makespan, double* serial, double* exposed_comm)
+{
+    if (!p || !makespan || !serial || !exposed_comm) return fail(MESH_ATTN_EINVAL, "plan_timeline: null pointer");
+    if (pass != 0 && pass != 1) return fail(MESH_ATTN_EINVAL, "plan_timeline: pass must be 0 or 1");
+    const std::vector<int32_t>& rows = pass == 0 ? p->steps_fwd : p->steps_bwd;
+    // the same task costs goo_schedule was given for this pass
+    const double t_c = pass == 0 ? p->t_c : 2.5 * p->t_c;
+    auto cost = [&](int kind) -> double {
+        switch (kind) {
+            case MESH_ATTN_TASK_AG_KV: return p->t_ag_kv;
+            case MESH_ATTN_TASK_AG_Q: return pass == 0 ? p->t_ag_q : 3.0 * p->t_ag_q;
+            case MESH_ATTN_TASK_RS_Q: return p->t_rs_q;
+            case MESH_ATTN_TASK_RS_KV: return p->t_rs_kv;
+            default: return t_c;
+        }
+    };
+    double total = 0.0, ser = 0.0, compute = 0.0;
+    for (size_t r = 0; r < rows.size();) {                 // rows (step, kind, i, j), grouped by step
+        const int step = rows[r];
+        double comm = 0.0, comp = 0.0;
+        for (; r < rows.size() && rows[r] == step; r += 4) {
+            const int kind = rows[r + 1];
+            if (kind == MESH_ATTN_TASK_C) comp += cost(kind);
+            else comm += cost(kind);
+        }
+        total += comm > comp ? comm : comp;
+        ser += comm + comp;
+        compute += comp;
+    }
+    if (p->desc.order == 0) total = ser;                   // row-major order schedules no overlap: gather, compute, reduce
+    *makespan = total;
+    *serial = ser;
+    *exposed_comm = total - compute;
+    return MESH_ATTN_OK;
+}
+
 extern "C" int mesh_attn_plan_tam_units(const mesh_attn_plan* p, int32_t gpus_per_node, int32_t alpha, int32_t node, int64_t* q_units,
                              int64_t* kv_units)
 {

@@ -69,6 +69,13 @@ def test_goo_fig4_example():
     assert comm[:6] == [(B.TASK_AG_KV, 0), (B.TASK_AG_Q, 0), (B.TASK_AG_Q, 1), (B.TASK_AG_KV, 1), (B.TASK_AG_Q, 2), (B.TASK_AG_KV, 2)]
     assert steps[2][1] == [(0, 0)] and steps[5][1] == [(1, 1), (2, 0)]
     assert [k + 1 for k, c in enumerate(comm) if c is None] == [7, 10] and len(steps) == 11
+    # timeline of that printed schedule, by hand: steps last 1, .5, .5, 1, .5, 1 (AG-KV-2 || C-1-1 + C-2-0), .5, .5, .5, .5, .5
+    makespan, serial, exposed = p.timeline()
+    assert (makespan, serial, exposed) == (7.0, 3 * 1.0 + 6 * 0.5 + 9 * 0.5, 7.0 - 9 * 0.5)
+    # row-major order has a single step: all communication first, nothing hidden
+    q = mk(2, 2, L=384, order=0, k_q=3, k_kv=3, t_ag_kv=1.0, t_ag_q=0.5, t_rs_q=0.5, t_c=0.5)
+    m2, s2, e2 = q.timeline()
+    assert s2 == serial and m2 >= makespan and e2 >= exposed
 
 
 @pytest.mark.parametrize("kq,kkv", [(1, 1), (2, 2), (4, 4), (2, 8), (8, 2), (1, 16), (16, 1), (3, 5)])
@@ -78,6 +85,11 @@ def test_goo_matches_oracle_and_tile_lists(kq, kkv, costs):
     p = mk(2, 3, L=L, kvr=1, order=1, k_q=kq, k_kv=kkv, t_ag_kv=costs[0], t_ag_q=costs[1], t_rs_q=costs[2], t_c=costs[3])
     ref = po.goo_forward(kq, kkv, *costs, gamma=1.05)
     assert _steps_to_oracle_form(p.steps()) == ref
+    # timeline invariants: never longer than serial execution, never shorter than either lane alone
+    makespan, serial, exposed = p.timeline()
+    comm_total = kkv * costs[0] + kq * costs[1] + kq * costs[2]
+    assert max(comm_total, kq * kkv * costs[3]) - 1e-9 <= makespan <= serial + 1e-9
+    assert abs(serial - (comm_total + kq * kkv * costs[3])) < 1e-6 and abs(exposed - (makespan - kq * kkv * costs[3])) < 1e-6
     order = po.compute_order(ref)
     for g in range(6):
         assert [tuple(r) for r in p.tiles(g).tolist()] == po.tile_list(6, 2, 3, True, g, order)
