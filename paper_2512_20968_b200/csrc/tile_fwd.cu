@@ -16,6 +16,15 @@
 // The two sub-tiles ping-pong: while the tensor core runs PV/QK for one sub-tile the other
 // sub-tile's softmax runs on the CUDA cores.  P is consumed by the PV MMA straight from
 // TMEM (A operand), V is the MN-major B operand, so neither is re-staged through smem.
+//
+// Softmax details, each from a measurement (profiles/): the whole 128-column score row of a thread
+// is held in registers (one TMEM read per block); the reference max only follows the running max
+// when it moved by more than 2^8, so the accumulator rescale is rare; the arithmetic is packed
+// fp32x2; 2 of 8 exponentials run on the FMA pipe (degree-3 polynomial) because the MUFU's 16
+// ex2/clk/SM would otherwise take exactly as long as the MMAs; P is handed over in two 64-key
+// halves so the PV MMA starts while the second half is still being exponentiated; single-thread
+// roles are entered through elect.sync so TMA / MMA issue runs on the uniform datapath.
+// kSplit (plan precision = 1): P as hi + lo bf16, two PV MMAs.
 #include <cuda_bf16.h>
 
 #include "plan.hpp"
