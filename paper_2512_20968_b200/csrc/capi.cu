@@ -205,9 +205,12 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "tile_bwd: the backward kernel is built for head_dim 128 only");
     if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds");
     if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
-    CUtensorMap tmQ, tmK, tmV, tmdO;
+    CUtensorMap tmQ, tmK, tmV, tmdO, tmdQ;
+    const Strides sdq = strides_of(p, p->geom.heads_q);
     if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv) ||
-        !make_map(p, &tmdO, dO, p->geom.heads_q))
+        !make_map(p, &tmdO, dO, p->geom.heads_q) ||
+        !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)p->geom.n * p->geom.L, p->geom.batch, sdq.h * 4, sdq.row * 4,
+                          sdq.b * 4, 32))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     BwdParams bp;
     bp.gm = p->geom;
@@ -224,7 +227,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     bp.q_stride_b = sq.b; bp.q_stride_row = sq.row; bp.q_stride_h = sq.h;
     bp.k_stride_b = sk.b; bp.k_stride_row = sk.row; bp.k_stride_h = sk.h;
     ProfScope prof(MESH_ATTN_K_TILE_BWD, (cudaStream_t)stream);
-    const int e = launch_tile_bwd(bp, tmQ, tmK, tmV, tmdO, p->num_sms, (cudaStream_t)stream);
+    const int e = launch_tile_bwd(bp, tmQ, tmK, tmV, tmdO, tmdQ, p->num_sms, (cudaStream_t)stream);
     if (e) return cuda_fail("tile_bwd launch", e);
     g_launches.fetch_add(1);
     return MESH_ATTN_OK;

@@ -60,7 +60,7 @@ struct DeltaParams {
 int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int num_sms,
                     cudaStream_t stream);
 int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV,
-                    const CUtensorMap& tmdO, int num_sms, cudaStream_t stream);
+                    const CUtensorMap& tmdO, const CUtensorMap& tmdQ, int num_sms, cudaStream_t stream);
 int launch_merge(const MergeParams& p, cudaStream_t stream);
 int launch_delta(const DeltaParams& p, cudaStream_t stream);
 
