@@ -357,8 +357,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
                         umma_commit(s_full);
                     }
-                    // dK += dS^T Q first (it releases the Q/dO stage: the next load gets the longest possible lead), then
-                    // dQ^T = K^T dS^T, emptied by the drain group
+                    // dQ^T = K^T dS^T first: the drain group empties it while dK += dS^T Q runs, so dP^T(i+1), which reuses its
+                    // TMEM columns, is not held up (the Q ring has its own two stages, so releasing Q a little later costs nothing)
                     PT_MARK(2);
                     mbar_wait(ds_full, ds_ph);
                     ds_ph ^= 1;
@@ -368,16 +368,16 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
                         for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
-                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(&qd_empty[st_cur]);
+                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
+                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
+                    umma_commit(dq_full);
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
                         for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
-                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(dq_full);
+                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
+                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
+                    umma_commit(&qd_empty[st_cur]);
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
