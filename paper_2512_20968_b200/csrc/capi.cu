@@ -210,7 +210,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv) ||
         !make_map(p, &tmdO, dO, p->geom.heads_q) ||
         !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)p->geom.n * p->geom.L, p->geom.batch, sdq.h * 4, sdq.row * 4,
-                          sdq.b * 4, 32))
+                          sdq.b * 4, 16))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     BwdParams bp;
     bp.gm = p->geom;

@@ -63,8 +63,9 @@ template <int D, bool kSplit> struct BwdCfg {
     static constexpr int kDsBytes = kBlock * kBlock * 2;        // dS^T [128 kv x 128 q] bf16
     static constexpr int kNumDs = kSplit ? 2 : 1;               // hi (+ lo)
     static constexpr int kStages = kSplit ? 1 : 2;              // Q ring; split mode trades the second Q stage for the dS lo tile
-    static constexpr int kStgRows = 32;                         // dQ staging: two ping-pong buffers of [32 queries][D] fp32
-    static constexpr int kStgBytes = 2 * kStgRows * D * 4;
+    static constexpr int kStgRows = 16;                         // dQ staging: a ring of kStgBufs buffers of [16 queries][D] fp32
+    static constexpr int kStgBufs = 4;
+    static constexpr int kStgBytes = kStgBufs * kStgRows * D * 4;
     static constexpr int kOffK = 0;
     static constexpr int kOffV = kTileBytes;
     static constexpr int kOffQ = 2 * kTileBytes;                // kStages Q tiles
@@ -561,8 +562,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     else if (warp >= 12) {
         // =============================== dQ drain group ===============================
         // thread = head-dim index d (TMEM lane): dQ^T row d, all 128 queries of the step -> registers (the TMEM columns are
-        // released at once) -> shared-memory staging (two ping-pong buffers of [32 queries][128 d] fp32) -> one
-        // cp.reduce.async.bulk.tensor (add.f32) per quarter block, the next quarter written while the previous one is read.  The TMA engine does the L2 atomics at the same rate as
+        // released at once) -> shared-memory staging (a ring of four [16 queries][128 d] fp32 buffers) -> one
+        // cp.reduce.async.bulk.tensor (add.f32) per 16-query slice, up to three in flight while the next slice is written.  The TMA engine does the L2 atomics at the same rate as
         // red.global (6.1 vs 6.4 TB/s measured) but no instruction of it goes through the SM's load/store queue, where
         // 512 reds per step used to delay every tcgen05.ld / ld.shared / st.shared of the compute warps by hundreds of clocks.
         reg_alloc<kDrainRegs>();
@@ -588,9 +589,9 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
                 PT_MARK(1);
 #pragma unroll
-                for (int k = 0; k < kBlock / Cfg::kStgRows; ++k) {   // quarter k through staging buffer k & 1
-                    float* stg = sStg + (k & 1) * (Cfg::kStgRows * D);
-                    if (issuer) asm volatile("cp.async.bulk.wait_group.read 1;" ::: "memory");   // the reduce of quarter k-2 has read this buffer
+                for (int k = 0; k < kBlock / Cfg::kStgRows; ++k) {   // 16-query slice k through staging buffer k % kStgBufs
+                    float* stg = sStg + (k % Cfg::kStgBufs) * (Cfg::kStgRows * D);
+                    if (issuer) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(Cfg::kStgBufs - 1) : "memory");   // slice k - kStgBufs has been read
                     named_bar_sync(1, kBlock);
 #pragma unroll
                     for (int j = 0; j < Cfg::kStgRows; ++j) stg[j * D + d] = __uint_as_float(r[k * Cfg::kStgRows + j]);
