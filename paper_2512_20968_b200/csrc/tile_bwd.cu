@@ -13,18 +13,22 @@
 //   dQ^T = K^T dS^T         (TMEM columns 128..255, reusing dP^T once consumed)
 //                                                        A = K tile read M-major, B = dS^T read N-major
 //
-// dQ is produced TRANSPOSED (TMEM lane = head-dim index d, column = query) so that the drain's
-// `red.global.add.f32` has the 32 lanes of a warp on 32 consecutive floats of one dQ row: full
-// 128-byte lines per request.  (With lane = query row the same reduction is 32 scattered 16-byte
-// atomics per instruction and L2 tops out at 2.9 TB/s instead of 6.4 TB/s; profiles/r01_v1_README.md.)
+// dQ is produced TRANSPOSED (TMEM lane = head-dim index d, column = query): a drain thread then writes 32
+// consecutive floats of a dQ row per warp instruction into a row-major shared-memory staging tile, and the TMA
+// engine adds the tile into global dQ (cp.reduce.async.bulk.tensor, add.f32): full lines per request at the L2
+// atomic rate (6.1 TB/s measured; plain red.global with lane = query row: 2.9 TB/s), and none of it in the SM's
+// load/store queue (512 red.global per step delayed every tcgen05.ld / ld.shared of the compute warps by hundreds
+// of clocks; profiles/r01_v5_README.md).
 //
-//   warp 0      TMA producer: K,V per item; Q, dO, -lse*log2e, delta per step through a ring
+//   warp 0      TMA producer: K,V per item; Q (+ exponent offsets, delta) per step through a 2-stage ring; dO through
+//               a single buffer (dO(i+1) is only needed a full step after dV(i) released it)
 //   warp 1      MMA issuer (one thread)
 //   warp 2      TMEM allocator
 //   warps 4-7   compute group 0: key row = TMEM lane, query columns  0..63  of the block
 //   warps 8-11  compute group 1: key row = TMEM lane, query columns 64..127
 //               each: S^T -> P^T (regs + TMEM), dP^T -> dS^T (smem); epilogue: group 0 drains dK, group 1 drains dV
-//   warps 12-15 dQ drain group: dQ^T row d = TMEM lane -> registers -> atomics, overlapping the next step's MMAs
+//   warps 12-15 dQ drain group: dQ^T row d = TMEM lane -> registers (TMEM released) -> staging ring -> TMA reduce,
+//               overlapping the next step's MMAs
 //
 // The softmax scale is folded into P^T (its log2 is part of the exponent offset the preprocess kernel wrote), so
 // dS^T, dQ^T and dK come out already scaled and only dV is divided by it, once per item in the epilogue.
