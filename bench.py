@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C5", help="C1..C5 (BASELINE.json configs[0..4]); default: the 1M-token causal config")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target duration of the oracle sample")
+    ap.add_argument("--usp-lanes", type=int, default=1, help="Mesh-USP lanes U (PAPER.md L372-389): the partial workspace shrinks by U")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -323,7 +324,7 @@ def run_ours(args):
     w = W.CONFIGS[args.workload]
     peaks, peak_src = load_peaks()
     inp = W.make_inputs(w, "cuda", ("q", "k", "v", "do") if w.backward else ("q", "k", "v"))
-    plan = plan_for(w)
+    plan = plan_for(w, usp_lanes=args.usp_lanes)
     buf = Buffers(plan, w, backward=w.backward)
 
     def step():
@@ -426,6 +427,8 @@ def run_ours(args):
         "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roofline, "cpu_baseline": cpu, "kernels": kernels,
         "summary": summary,
     }
+    if args.usp_lanes > 1:
+        line["config"]["usp_lanes"] = args.usp_lanes
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()

@@ -34,6 +34,8 @@
  *   lse        fp32  [B, Hq, N]   natural log of the sum of exp of the SCALED scores
  *   partial_O  fp32  [g_count][slots][B][L][Hq][D]   slots = a (partial_mode 0) or a*b (1)
  *   partial_lse fp32 [g_count][slots][B][Hq][L]
+ *   (usp_lanes = U > 1: a simulated GPU holds Hq/U heads, so Hq in the two partial layouts is Hq/U; all other
+ *    tensors keep their full shape and the lanes address head slices of them.)
  * Token position of (p, s): seq_layout 0: p*L+s;  seq_layout 1 (striped): s*n+p.
  * Causal: key visible iff pos(key) <= pos(query).  A row with no visible key
  * gets O = 0, lse = -inf.  GQA: query head h reads KV head h / (Hq/Hkv).
@@ -74,7 +76,12 @@ typedef struct {
                                  1: one partial per pair (u,v): literal O_ij, lse_ij           */
     int32_t precision;        /* P (forward and backward) and dS as tensor-core operands: 0 one bf16,
                                  1 split hi+lo bf16 pairs (two MMAs each; needed for outlier scores)    */
-    int32_t reserved[5];      /* must be 0                                                             */
+    int32_t usp_lanes;        /* Mesh-USP: U >= 1 lanes (0 -> 1).  The Ulysses all-to-all leaves lane l with
+                                 query heads [l*Hq/U, (l+1)*Hq/U) (KV heads likewise) of ALL tokens, and each lane runs
+                                 Mesh-Attention on its own a x b mesh.  There are n*U simulated GPUs: g in [0, n*U) is
+                                 mesh GPU g % n of lane g / n; Q group q in [0, b*U) is group q % b of lane q / b.
+                                 The partial workspace of a simulated GPU shrinks by U.  heads_kv % U == 0.   */
+    int32_t reserved[4];      /* must be 0                                                             */
 } mesh_attn_plan_desc;
 
 /* what = ... for mesh_attn_plan_query */
@@ -84,7 +91,7 @@ enum {
     MESH_ATTN_Q_SLOTS_PER_GPU = 2,     /* a or a*b                                                        */
     MESH_ATTN_Q_FLOPS_FWD = 3,         /* algorithmic: 4*D*Hq*B*visible pairs                             */
     MESH_ATTN_Q_FLOPS_BWD = 4,         /* algorithmic: 10*D*Hq*B*visible pairs                            */
-    MESH_ATTN_Q_WAVES = 5,             /* number of Q groups = b                                          */
+    MESH_ATTN_Q_WAVES = 5,             /* number of Q groups = b * usp_lanes                              */
     MESH_ATTN_Q_MERGE_BYTES = 6,       /* algorithmic bytes moved by ONE merge call (one Q group)         */
     MESH_ATTN_Q_FWD_ITEMS_PER_GPU = 7, /* tile-forward work items per simulated GPU                       */
     MESH_ATTN_Q_BWD_ITEMS_PER_GPU = 8, /* tile-backward work items per simulated GPU                      */
@@ -96,7 +103,11 @@ enum {
     MESH_ATTN_Q_MESH_COMM_BYTES_FWD = 13,  /* per-GPU forward volume of this a x b tiling, closed form
                                               2(a+b-2) N d / n elements x 2 bytes (bf16), d = Hq*head_dim */
     MESH_ATTN_Q_MESH_COMM_BYTES_BWD = 14,  /* backward: twice the forward volume (Q,O,dO in, dQ out; K,V in, dK,dV out; Table 5) */
-    MESH_ATTN_Q_RING_COMM_BYTES_FWD = 15   /* Ring-Attention on the same n GPUs: (2 - 2/n) N d elements x 2 bytes */
+    MESH_ATTN_Q_RING_COMM_BYTES_FWD = 15,  /* Ring-Attention on the same n GPUs: (2 - 2/n) N d elements x 2 bytes */
+    MESH_ATTN_Q_USP_LANES = 16,            /* U                                                                          */
+    MESH_ATTN_Q_USP_A2A_BYTES_FWD = 17     /* per-GPU forward volume of the Ulysses all-to-alls around the lanes (Q, K, V in,
+                                              O out): (U-1)/U of the GPU's N/(n*U) tokens x (2 Hq + 2 Hkv) head_dim x 2 bytes;
+                                              with n = 1 and Hq = Hkv this is Table 1's Ulysses entry 4(U-1)/U^2 N d */
 };
 
 /* kinds in mesh_attn_plan_steps rows (step, kind, i, j) */
@@ -118,7 +129,8 @@ enum {
 int mesh_attn_plan_create(const mesh_attn_plan_desc* desc, mesh_attn_plan** out);
 void mesh_attn_plan_destroy(mesh_attn_plan* plan);
 
-/* am: host int32 [n*n] row-major, am[i*n+j] = g computing (Q_i, KV_j). */
+/* am: host int32 [n*n] row-major, am[i*n+j] = g computing (Q_i, KV_j).  The planner calls below
+ * (am, footprint, tiles, steps, tam_units, timeline) describe ONE lane's a x b mesh: g in [0, n). */
 int mesh_attn_plan_am(const mesh_attn_plan* plan, int32_t* am);
 
 /* Footprints of simulated GPU g: I^Q (a entries), I^KV (b entries) in
@@ -194,8 +206,9 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_co
                        const void* Q, const void* K, const void* V, const void* dO,
                        const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream);
 
-/* All waves: for each Q group r: tile_fwd(g_first = r*a, a) then merge(r). partial_O /
- * partial_lse must hold `a` simulated GPUs (query PARTIAL_*_BYTES * a). */
+/* All waves: for each lane and each Q group r of it: tile_fwd(g_first = lane*n + r*a, a) then
+ * merge(lane*b + r). partial_O / partial_lse must hold `a` simulated GPUs (query PARTIAL_*_BYTES * a).
+ * tile_fwd / tile_bwd ranges [g_first, g_first+g_count) must stay inside one lane (EINVAL). */
 int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
                       float* O, float* lse, float* partial_O, float* partial_lse, void* stream);
 

@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
             const float x = w_smem[(r * Hq + h) * m + k];
             w_smem[(r * Hq + h) * m + k] = (x == -INFINITY) ? 0.f : __expf(x - lse);
         }
-        p.lse[((size_t)bt * Hq + h) * ((size_t)gm.n * gm.L) + (size_t)u * gm.L + s0 + r] = lse;
+        p.lse[(size_t)bt * p.lse_stride_b + (size_t)h * ((size_t)gm.n * gm.L) + (size_t)u * gm.L + s0 + r] = lse;
     }
     __syncthreads();
 

@@ -28,7 +28,7 @@ int cuda_fail(const char* what, int err)
     return MESH_ATTN_ECUDA;
 }
 
-struct Strides { long long b, row, h; };   // element strides of a [B,N,H,D] / [B,H,N,D] tensor
+struct Strides { long long b, row, h; };   // element strides of a [B,N,H,D] / [B,H,N,D] tensor with H heads in all
 Strides strides_of(const mesh_attn_plan* p, int H)
 {
     const long long N = (long long)p->geom.n * p->geom.L, D = p->geom.head_dim;
@@ -36,11 +36,30 @@ Strides strides_of(const mesh_attn_plan* p, int H)
     return {N * H * D, D, N * D};
 }
 
-bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H)
+// Mesh-USP lane of a range of simulated GPUs / of a Q group: head slice [hq0, hq0 + geom.heads_q)
+// of the query-shaped tensors and [hk0, hk0 + geom.heads_kv) of the key-shaped ones; geom holds the LANE's head counts.
+struct Lane { int lane; long long hq0, hk0; };
+int lanes_of(const mesh_attn_plan* p) { return p->desc.usp_lanes > 1 ? p->desc.usp_lanes : 1; }
+Lane lane_at(const mesh_attn_plan* p, int lane) { return {lane, (long long)lane * p->geom.heads_q, (long long)lane * p->geom.heads_kv}; }
+bool lane_of_range(const mesh_attn_plan* p, int g_first, int g_count, Lane* out)
 {
-    const Strides s = strides_of(p, H);
+    const int n = p->geom.n;
+    if (g_first < 0 || g_count <= 0 || (long long)g_first + g_count > (long long)n * lanes_of(p)) return false;
+    if ((g_first + g_count - 1) / n != g_first / n) return false;
+    *out = lane_at(p, g_first / n);
+    return true;
+}
+template <class T> T* head_slice(T* base, long long h0, const Strides& s, int elem_bytes)
+{
+    return (T*)((char*)base + h0 * s.h * elem_bytes);
+}
+
+// bf16 tensor map of the lane's head slice: H_lane heads starting at h0 of a tensor with H_all heads
+bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0)
+{
+    const Strides s = strides_of(p, H_all);
     const uint64_t N = (uint64_t)p->geom.n * p->geom.L;
-    return make_tmap_bf16_4d(m, base, p->geom.head_dim, H, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, kBlock);
+    return make_tmap_bf16_4d(m, head_slice(base, h0, s, 2), p->geom.head_dim, H_lane, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, kBlock);
 }
 
 // ---- per-kernel device timing (mesh_attn_profile_*): event pairs around each launch ----
@@ -130,10 +149,12 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
 {
     if (int rc = check_device(p, "tile_fwd")) return rc;
     if (!Q || !K || !V || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, "tile_fwd: null pointer");
-    if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_fwd: simulated GPU range out of bounds");
+    Lane ln;
+    if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_fwd: simulated GPU range out of bounds (or crossing a USP lane)");
     if ((long long)g_count * (long long)p->fwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_fwd: too many work items in one call");
     CUtensorMap tmQ, tmK, tmV;
-    if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv))
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
+        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0))
         return fail(MESH_ATTN_ECUDA, "tile_fwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     FwdParams fp;
     fp.gm = p->geom;
@@ -141,7 +162,7 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     fp.segs = p->d_fwd_segs;
     fp.seglists = p->d_fwd_seglists;
     fp.items_per_gpu = (int)p->fwd_items.size();
-    fp.g_first = g_first;
+    fp.g_first = g_first % p->geom.n;
     fp.g_count = g_count;
     fp.split = p->desc.precision;
     fp.partial_O = partial_O;
@@ -158,10 +179,13 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
 {
     if (int rc = check_device(p, "merge")) return rc;
     if (!partial_O || !partial_lse || !O || !lse) return fail(MESH_ATTN_EINVAL, "merge: null pointer");
-    if (q_group < 0 || q_group >= p->geom.b) return fail(MESH_ATTN_EINVAL, "merge: q_group out of range (there are b Q groups, PAPER.md L178)");
+    if (q_group < 0 || q_group >= p->geom.b * lanes_of(p))
+        return fail(MESH_ATTN_EINVAL, "merge: q_group out of range (there are b Q groups per lane, PAPER.md L178)");
+    const Lane ln = lane_at(p, q_group / p->geom.b);
+    const long long N = (long long)p->geom.n * p->geom.L;
     MergeParams mp;
     mp.gm = p->geom;
-    mp.q_group = q_group;
+    mp.q_group = q_group % p->geom.b;
     mp.per = p->desc.partial_mode == 1 ? p->geom.b : 1;
     mp.m = p->geom.a * mp.per;
     int rows = 8;
@@ -170,9 +194,10 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
     mp.rows_per_block = rows;
     mp.partial_O = partial_O;
     mp.partial_lse = partial_lse;
-    mp.O = O;
-    mp.lse = lse;
-    const Strides s = strides_of(p, p->geom.heads_q);
+    const Strides s = strides_of(p, p->desc.heads_q);
+    mp.O = head_slice(O, ln.hq0, s, 4);
+    mp.lse = lse + ln.hq0 * N;
+    mp.lse_stride_b = (long long)p->desc.heads_q * N;
     mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_MERGE, (cudaStream_t)stream);
     const int e = launch_merge(mp, (cudaStream_t)stream);
@@ -187,8 +212,10 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
     if (!O || !dO || !lse || !bwd_ws) return fail(MESH_ATTN_EINVAL, "bwd_preprocess: null pointer");
     DeltaParams dp;
     dp.gm = p->geom;
+    dp.gm.heads_q = p->desc.heads_q;      // all lanes in one launch
+    dp.gm.heads_kv = p->desc.heads_kv;
     dp.O = O; dp.dO = dO; dp.lse = lse; dp.ws = bwd_ws;
-    const Strides s = strides_of(p, p->geom.heads_q);
+    const Strides s = strides_of(p, p->desc.heads_q);
     dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
     const int e = launch_delta(dp, (cudaStream_t)stream);
@@ -203,12 +230,17 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     if (int rc = check_device(p, "tile_bwd")) return rc;
     if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
     if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "tile_bwd: the backward kernel is built for head_dim 128 only");
-    if (g_first < 0 || g_count <= 0 || g_first + g_count > p->geom.n) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds");
+    Lane ln;
+    if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds (or crossing a USP lane)");
     if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
     CUtensorMap tmQ, tmK, tmV, tmdO, tmdQ;
-    const Strides sdq = strides_of(p, p->geom.heads_q);
-    if (!make_map(p, &tmQ, Q, p->geom.heads_q) || !make_map(p, &tmK, K, p->geom.heads_kv) || !make_map(p, &tmV, V, p->geom.heads_kv) ||
-        !make_map(p, &tmdO, dO, p->geom.heads_q) ||
+    const Strides sdq = strides_of(p, p->desc.heads_q), sdk = strides_of(p, p->desc.heads_kv);
+    const long long N = (long long)p->geom.n * p->geom.L;
+    dQ = head_slice(dQ, ln.hq0, sdq, 4);
+    dK = head_slice(dK, ln.hk0, sdk, 4);
+    dV = head_slice(dV, ln.hk0, sdk, 4);
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
+        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) || !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0) ||
         !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)p->geom.n * p->geom.L, p->geom.batch, sdq.h * 4, sdq.row * 4,
                           sdq.b * 4, 16))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
@@ -218,12 +250,14 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     bp.segs = p->d_bwd_segs;
     bp.seglists = p->d_bwd_seglists;
     bp.items_per_gpu = (int)p->bwd_items.size();
-    bp.g_first = g_first;
+    bp.g_first = g_first % p->geom.n;
     bp.g_count = g_count;
     bp.split = p->desc.precision;
-    bp.ws = bwd_ws;
+    bp.ws = bwd_ws + ln.hq0 * N;
+    bp.ws_plane = (long long)p->geom.batch * p->desc.heads_q * N;
+    bp.vec_stride_b = (long long)p->desc.heads_q * N;
     bp.dQ = dQ; bp.dK = dK; bp.dV = dV;
-    const Strides sq = strides_of(p, p->geom.heads_q), sk = strides_of(p, p->geom.heads_kv);
+    const Strides sq = sdq, sk = sdk;
     bp.q_stride_b = sq.b; bp.q_stride_row = sq.row; bp.q_stride_h = sq.h;
     bp.k_stride_b = sk.b; bp.k_stride_row = sk.row; bp.k_stride_h = sk.h;
     ProfScope prof(MESH_ATTN_K_TILE_BWD, (cudaStream_t)stream);
@@ -237,10 +271,11 @@ int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, con
                       float* partial_lse, void* stream)
 {
     if (int rc = check_device(p, "forward")) return rc;
-    for (int r = 0; r < p->geom.b; ++r) {   // one wave per Q group
-        if (int rc = mesh_attn_tile_fwd(p, r * p->geom.a, p->geom.a, Q, K, V, partial_O, partial_lse, stream)) return rc;
-        if (int rc = mesh_attn_merge(p, r, partial_O, partial_lse, O, lse, stream)) return rc;
-    }
+    for (int lane = 0; lane < lanes_of(p); ++lane)
+        for (int r = 0; r < p->geom.b; ++r) {   // one wave per Q group of each USP lane (L372-389)
+            if (int rc = mesh_attn_tile_fwd(p, lane * p->geom.n + r * p->geom.a, p->geom.a, Q, K, V, partial_O, partial_lse, stream)) return rc;
+            if (int rc = mesh_attn_merge(p, lane * p->geom.b + r, partial_O, partial_lse, O, lse, stream)) return rc;
+        }
     return MESH_ATTN_OK;
 }
 
@@ -253,14 +288,15 @@ int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, co
     const Geom& gm = p->geom;
     const size_t N = (size_t)gm.n * gm.L;
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaMemsetAsync(dQ, 0, (size_t)gm.batch * N * gm.heads_q * gm.head_dim * 4, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(dK, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(dV, 0, (size_t)gm.batch * N * gm.heads_kv * gm.head_dim * 4, st);
+    cudaError_t e = cudaMemsetAsync(dQ, 0, (size_t)gm.batch * N * p->desc.heads_q * gm.head_dim * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dK, 0, (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(dV, 0, (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim * 4, st);
     if (e != cudaSuccess) return cuda_fail("backward memset", (int)e);
     if (int rc = mesh_attn_bwd_preprocess(p, O, dO, lse, bwd_ws, stream)) return rc;
     // keep each launch's work-item count below 2^31: one call per Q group
-    for (int r = 0; r < gm.b; ++r)
-        if (int rc = mesh_attn_tile_bwd(p, r * gm.a, gm.a, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream)) return rc;
+    for (int lane = 0; lane < lanes_of(p); ++lane)
+        for (int r = 0; r < gm.b; ++r)
+            if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream)) return rc;
     return MESH_ATTN_OK;
 }
 
@@ -272,8 +308,8 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
         return fail(MESH_ATTN_EINVAL, "step_host: null pointer");
     const Geom& gm = p->geom;
     const size_t N = (size_t)gm.n * gm.L;
-    const size_t nq = (size_t)gm.batch * N * gm.heads_q * gm.head_dim, nk = (size_t)gm.batch * N * gm.heads_kv * gm.head_dim;
-    const size_t nl = (size_t)gm.batch * N * gm.heads_q;
+    const size_t nq = (size_t)gm.batch * N * p->desc.heads_q * gm.head_dim, nk = (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim;
+    const size_t nl = (size_t)gm.batch * N * p->desc.heads_q;
     cudaStream_t st = (cudaStream_t)stream;
     cudaError_t e = cudaMemcpyAsync(io->d_Q, io->Q_host, nq * 2, cudaMemcpyHostToDevice, st);
     if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, st);

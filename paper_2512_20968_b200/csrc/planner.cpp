@@ -239,6 +239,9 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     if (L % kBlock) return fail(MESH_ATTN_EINVAL, "plan_create: partition length L = seq_total/n must be a multiple of 128");
     if (d->heads_q % d->heads_kv) return fail(MESH_ATTN_EINVAL, "plan_create: heads_q must be a multiple of heads_kv (PAPER.md L427)");
     if (d->heads_q > 32767) return fail(MESH_ATTN_EINVAL, "plan_create: too many heads");
+    const int U = d->usp_lanes <= 0 ? 1 : d->usp_lanes;
+    if (d->heads_kv % U) return fail(MESH_ATTN_EINVAL, "plan_create: heads_kv must be a multiple of usp_lanes (PAPER.md L372-389: each lane holds 1/U of the heads)");
+    if ((int64_t)d->n * U > 32767) return fail(MESH_ATTN_EINVAL, "plan_create: n * usp_lanes too large");
     if (d->head_dim != 64 && d->head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "plan_create: head_dim must be 64 or 128");
     for (int v : {d->causal, d->kvr, d->order, d->seq_layout, d->tensor_layout, d->partial_mode, d->precision})
         if (v != 0 && v != 1) return fail(MESH_ATTN_EINVAL, "plan_create: flag fields must be 0 or 1");
@@ -255,7 +258,7 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     p->desc = *d;
     Geom& gm = p->geom;
     gm.n = d->n; gm.a = d->a; gm.b = d->b; gm.L = L;
-    gm.batch = d->batch; gm.heads_q = d->heads_q; gm.heads_kv = d->heads_kv; gm.head_dim = d->head_dim;
+    gm.batch = d->batch; gm.heads_q = d->heads_q / U; gm.heads_kv = d->heads_kv / U; gm.head_dim = d->head_dim;   // one lane's heads
     gm.group = d->heads_q / d->heads_kv;
     gm.causal = d->causal; gm.kvr = d->kvr; gm.striped = d->seq_layout;
     gm.slots_per_gpu = d->partial_mode == 1 ? d->a * d->b : d->a;
@@ -270,12 +273,12 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
         p->t_rs_kv = 2.0f * d->t_rs_q;
     } else {
         const double bw = 4.0e11, lat = 2.0e-5, rate = 8.0e14;
-        const double unit_q = (double)L * d->heads_q * d->head_dim * 2.0, unit_kv = (double)L * d->heads_kv * d->head_dim * 2.0;
+        const double unit_q = (double)L * gm.heads_q * d->head_dim * 2.0, unit_kv = (double)L * gm.heads_kv * d->head_dim * 2.0;
         p->t_ag_q = (float)((d->a - 1) * unit_q / k_q / bw + lat);
         p->t_ag_kv = (float)((d->b - 1) * 2.0 * unit_kv / k_kv / bw + lat);
         p->t_rs_q = (float)((d->a - 1) * unit_q / k_q / bw + lat);
         p->t_rs_kv = (float)((d->b - 1) * 2.0 * unit_kv / k_kv / bw + lat);
-        p->t_c = (float)(4.0 * d->head_dim * d->heads_q * ((double)d->a * L / k_q) * ((double)d->b * L / k_kv) * (d->causal ? 0.5 : 1.0) / rate);
+        p->t_c = (float)(4.0 * d->head_dim * gm.heads_q * ((double)d->a * L / k_q) * ((double)d->b * L / k_kv) * (d->causal ? 0.5 : 1.0) / rate);
     }
 
     // assignment matrix
@@ -427,14 +430,15 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
     const Geom& gm = p->geom;
     const int64_t N = (int64_t)gm.n * gm.L;
     const long double pairs = gm.causal ? (long double)N * (N + 1) / 2 : (long double)N * N;
-    const int64_t unit = (int64_t)gm.batch * gm.L * gm.heads_q;     // (row, head) pairs of one partition
+    const int64_t unit = (int64_t)gm.batch * gm.L * gm.heads_q;     // (row, head) pairs of one partition of one lane
+    const int64_t U = p->desc.usp_lanes > 1 ? p->desc.usp_lanes : 1, Hq = p->desc.heads_q, Hkv = p->desc.heads_kv;
     switch (what) {
         case MESH_ATTN_Q_PARTIAL_O_BYTES: *value = (int64_t)gm.slots_per_gpu * unit * gm.head_dim * 4; break;
         case MESH_ATTN_Q_PARTIAL_LSE_BYTES: *value = (int64_t)gm.slots_per_gpu * unit * 4; break;
         case MESH_ATTN_Q_SLOTS_PER_GPU: *value = gm.slots_per_gpu; break;
-        case MESH_ATTN_Q_FLOPS_FWD: *value = (int64_t)(4.0L * gm.head_dim * gm.heads_q * gm.batch * pairs); break;
-        case MESH_ATTN_Q_FLOPS_BWD: *value = (int64_t)(10.0L * gm.head_dim * gm.heads_q * gm.batch * pairs); break;
-        case MESH_ATTN_Q_WAVES: *value = gm.b; break;
+        case MESH_ATTN_Q_FLOPS_FWD: *value = (int64_t)(4.0L * gm.head_dim * Hq * gm.batch * pairs); break;
+        case MESH_ATTN_Q_FLOPS_BWD: *value = (int64_t)(10.0L * gm.head_dim * Hq * gm.batch * pairs); break;
+        case MESH_ATTN_Q_WAVES: *value = gm.b * U; break;
         case MESH_ATTN_Q_MERGE_BYTES: {
             // per output (row, head): m partial rows + m lse read, one row + one lse written (fp32)
             const int64_t m = p->desc.partial_mode == 1 ? (int64_t)gm.a * gm.b : gm.a;
@@ -446,7 +450,7 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
         case MESH_ATTN_Q_BLOCKS_FWD: {
             int64_t blocks = 0;
             for (int g = 0; g < gm.n; ++g) blocks += fwd_blocks_of_gpu(p, g);
-            *value = blocks * gm.heads_q * gm.batch;
+            *value = blocks * Hq * gm.batch;
             break;
         }
         case MESH_ATTN_Q_COMM_UNITS: {
@@ -478,7 +482,14 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             *value = (int64_t)((2.0L - 2.0L / gm.n) * Nd);
             break;
         }
-        case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * gm.heads_q * (int64_t)gm.n * gm.L * 4; break;
+        case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * Hq * (int64_t)gm.n * gm.L * 4; break;
+        case MESH_ATTN_Q_USP_LANES: *value = U; break;
+        case MESH_ATTN_Q_USP_A2A_BYTES_FWD: {
+            // the GPU holds N/(n U) tokens of all heads before the all-to-all and keeps 1/U of them
+            const long double tokens = (long double)gm.batch * gm.n * gm.L / ((long double)gm.n * U);
+            *value = (int64_t)(tokens * (U - 1) / U * (2.0L * Hq + 2.0L * Hkv) * gm.head_dim * 2.0L);
+            break;
+        }
         default: return fail(MESH_ATTN_EINVAL, "plan_query: unknown query");
     }
     return MESH_ATTN_OK;

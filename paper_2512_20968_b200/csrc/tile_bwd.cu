@@ -256,7 +256,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         // =============================== TMA producer ===============================
         if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0, do_ph = 0;
-            const float* nlse = p.ws + (size_t)gm.batch * gm.heads_q * N;      // ws[1] = log2(scale) - lse*log2e
+            const float* nlse = p.ws + p.ws_plane;                            // ws[1] = log2(scale) - lse*log2e
             for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
@@ -279,7 +279,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     const int row = u * gm.L + s0;
                     for (int bx = 0; bx < Cfg::kBoxes; ++bx)
                         tma_load_4d(sQ(stage) + bx * (kBlock * 128), &tmQ, &qd_full[stage], bx * 64, h, row, c.it.batch, kEvictLast);
-                    const size_t vec = ((size_t)c.it.batch * gm.heads_q + h) * N + row;
+                    const size_t vec = (size_t)c.it.batch * p.vec_stride_b + (size_t)h * N + row;
                     bulk_load(sLse(stage), nlse + vec, 512, &qd_full[stage]);
                     bulk_load(sDelta(stage), p.ws + vec, 512, &qd_full[stage]);
                     if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }

@@ -27,7 +27,9 @@ struct BwdParams {
     int items_per_gpu;
     int g_first, g_count;
     int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
-    const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess)
+    const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess); head 0 = first head of the lane
+    long long ws_plane;        // elements between ws[0] and ws[1] (B * all heads * N)
+    long long vec_stride_b;    // batch stride of the [B][Hq][N] vectors (all heads * N)
     float *dQ, *dK, *dV;       // fp32 accumulators
     // element strides of dQ (query-shaped) and dK/dV (key-shaped) tensors
     long long q_stride_b, q_stride_row, q_stride_h;
@@ -44,6 +46,7 @@ struct MergeParams {
     const float* partial_lse;
     float* O;
     float* lse;
+    long long lse_stride_b;    // batch stride of lse [B][Hq][N] (all heads * N)
     long long o_stride_b, o_stride_row, o_stride_h;   // element strides of O
 };
 

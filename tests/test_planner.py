@@ -193,3 +193,32 @@ def test_planner_analytics_against_paper_numbers():
             assert p.tam_units(8, alpha, node) == po.tam_internode_units(8, 8, 8, alpha, node)
     with pytest.raises(B.MeshAttnError):
         p.tam_units(8, 3)
+
+
+def test_usp_lanes_geometry_and_all_to_all_volume():
+    """S8(f).3, Mesh-USP: U lanes, each Mesh-Attention over 1/U of the heads.  The partial
+    workspace of a simulated GPU shrinks by U, the algorithmic work does not change, there are b*U waves; the
+    Ulysses all-to-all volume reduces, for one mesh GPU (n = 1) and MHA, to Table 1's 4(U-1)/U^2 N d."""
+    kw = dict(a=2, b=2, batch=1, seq_total=4 * 256, heads_q=16, heads_kv=8, head_dim=128, causal=1, seq_layout=1)
+    base = Plan(**kw)
+    for U in (2, 4, 8):
+        p = Plan(usp_lanes=U, **kw)
+        assert p.query(B.Q_USP_LANES) == U and base.query(B.Q_USP_LANES) == 1
+        for what in (B.Q_PARTIAL_O_BYTES, B.Q_PARTIAL_LSE_BYTES, B.Q_MERGE_BYTES, B.Q_FWD_ITEMS_PER_GPU, B.Q_BWD_ITEMS_PER_GPU):
+            assert p.query(what) * U == base.query(what), what
+        for what in (B.Q_FLOPS_FWD, B.Q_FLOPS_BWD, B.Q_BLOCKS_FWD, B.Q_BWD_WS_BYTES, B.Q_SLOTS_PER_GPU, B.Q_COMM_UNITS):
+            assert p.query(what) == base.query(what), what
+        assert p.query(B.Q_WAVES) == U * base.query(B.Q_WAVES)
+        assert np.array_equal(p.am(), base.am())                       # every lane uses the same a x b mesh
+    with pytest.raises(MeshAttnError) as e:
+        Plan(usp_lanes=3, **kw)                                         # 8 KV heads do not split into 3 lanes
+    assert e.value.status == B.EINVAL
+    assert base.query(B.Q_USP_A2A_BYTES_FWD) == 0
+    # pure Ulysses = one mesh GPU per lane: 4 (U-1)/U^2 N d elements (Table 1, P:L285), 2 bytes each
+    N, H, D = 8 * 1024, 16, 128
+    for U in (2, 8, 16):
+        p = Plan(usp_lanes=U, a=1, b=1, batch=1, seq_total=N, heads_q=H, heads_kv=H, head_dim=D)
+        assert p.query(B.Q_USP_A2A_BYTES_FWD) == 4 * (U - 1) * N * H * D * 2 // (U * U)
+    # GQA: K and V move Hkv heads only; n mesh GPUs per lane hold N/(n U) tokens each
+    p = Plan(usp_lanes=4, **kw)
+    assert p.query(B.Q_USP_A2A_BYTES_FWD) == (4 * 256 // (4 * 4)) * 3 * (2 * 16 + 2 * 8) * 128 * 2 // 4
