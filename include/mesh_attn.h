@@ -105,6 +105,10 @@ enum {
     MESH_ATTN_Q_MESH_COMM_BYTES_BWD = 14,  /* backward: twice the forward volume (Q,O,dO in, dQ out; K,V in, dK,dV out; Table 5) */
     MESH_ATTN_Q_RING_COMM_BYTES_FWD = 15,  /* Ring-Attention on the same n GPUs: (2 - 2/n) N d elements x 2 bytes */
     MESH_ATTN_Q_USP_LANES = 16,            /* U                                                                          */
+    MESH_ATTN_Q_BWD_PAIRED = 18,           /* 1 if tile_bwd runs as 2-CTA clusters sharing the Q / dO tile loads: backward work items
+                                              2k and 2k+1 visit the same Q blocks on every simulated GPU (holds for non-causal and
+                                              striped-causal plans with an even item count; MESH_ATTN_NO_PAIR=1 in the environment
+                                              at plan_create forces 0) */
     MESH_ATTN_Q_USP_A2A_BYTES_FWD = 17     /* per-GPU forward volume of the Ulysses all-to-alls around the lanes (Q, K, V in,
                                               O out): (U-1)/U of the GPU's N/(n*U) tokens x (2 Hq + 2 Hkv) head_dim x 2 bytes;
                                               with n = 1 and Hq = Hkv this is Table 1's Ulysses entry 4(U-1)/U^2 N d */
@@ -219,8 +223,14 @@ int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K,
 
 /* End-to-end step with HOST buffers (pinned or pageable): copies Q,K,V(,dO) host->device
  * into the caller's device staging buffers, runs forward (and backward if dO_host != NULL),
- * copies O, lse (and dQ,dK,dV) device->host; all on `stream`, which is synchronised before
- * returning.  d_* are caller-owned DEVICE buffers of the shapes above. */
+ * copies O, lse (and dQ,dK,dV) device->host, and synchronises `stream` before returning.
+ * The kernels run on `stream`; the copies run on two plan-owned streams (one per direction) ordered
+ * against it by events, so that transfers overlap the kernels that do not need them: K, V and the
+ * Q rows of the first Q group go up first, the other Q groups and dO follow behind the forward
+ * waves; O and lse come down during the backward, the dQ rows of Q group r as soon as the
+ * simulated GPUs of group r are done (batch 1, tensor_layout 0; whole tensors otherwise), dK and
+ * dV at the end.  One step_host per plan at a time.  d_* are caller-owned DEVICE buffers of the
+ * shapes above. */
 typedef struct {
     const void *Q_host, *K_host, *V_host, *dO_host;      /* bf16 host inputs (dO_host may be NULL) */
     float *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* fp32 host outputs (any may be NULL = not copied back) */

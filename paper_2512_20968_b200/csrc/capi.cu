@@ -55,11 +55,11 @@ template <class T> T* head_slice(T* base, long long h0, const Strides& s, int el
 }
 
 // bf16 tensor map of the lane's head slice: H_lane heads starting at h0 of a tensor with H_all heads
-bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0)
+bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0, int box_rows = kBlock)
 {
     const Strides s = strides_of(p, H_all);
     const uint64_t N = (uint64_t)p->geom.n * p->geom.L;
-    return make_tmap_bf16_4d(m, head_slice(base, h0, s, 2), p->geom.head_dim, H_lane, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, kBlock);
+    return make_tmap_bf16_4d(m, head_slice(base, h0, s, 2), p->geom.head_dim, H_lane, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, box_rows);
 }
 
 // ---- per-kernel device timing (mesh_attn_profile_*): event pairs around each launch ----
@@ -132,6 +132,17 @@ int upload_plan(mesh_attn_plan* p)
     p->d_fwd_seglists = (const SegList*)put(p->fwd_seglists.data(), p->fwd_seglists.size() * sizeof(SegList), b4);
     p->d_bwd_seglists = (const SegList*)put(p->bwd_seglists.data(), p->bwd_seglists.size() * sizeof(SegList), b5);
     if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
+    // step_host's copy engines: one stream per direction, events for the chunk hand-offs
+    cudaStream_t s0 = nullptr, s1 = nullptr;
+    e = cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking);
+    if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s1, cudaStreamNonBlocking);
+    p->s_h2d = s0; p->s_d2h = s1;
+    for (int i = 0; e == cudaSuccess && i < 2 * p->geom.b + 6; ++i) {
+        cudaEvent_t ev = nullptr;
+        e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
+        if (e == cudaSuccess) p->copy_events.push_back(ev);
+    }
+    if (e != cudaSuccess) { free_plan_device(p); return cuda_fail("plan_create: copy streams / events", (int)e); }
     return MESH_ATTN_OK;
 }
 
@@ -139,6 +150,11 @@ void free_plan_device(mesh_attn_plan* p)
 {
     if (p->d_blob) cudaFree(p->d_blob);
     p->d_blob = nullptr;
+    for (void* ev : p->copy_events) cudaEventDestroy((cudaEvent_t)ev);
+    p->copy_events.clear();
+    if (p->s_h2d) cudaStreamDestroy((cudaStream_t)p->s_h2d);
+    if (p->s_d2h) cudaStreamDestroy((cudaStream_t)p->s_d2h);
+    p->s_h2d = p->s_d2h = nullptr;
 }
 }  // namespace mesh_attn
 
@@ -239,8 +255,11 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     dQ = head_slice(dQ, ln.hq0, sdq, 4);
     dK = head_slice(dK, ln.hk0, sdk, 4);
     dV = head_slice(dV, ln.hk0, sdk, 4);
-    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
-        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) || !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0) ||
+    // paired items (2-CTA clusters): each CTA loads 64-row halves of the Q / dO tiles and multicasts them
+    const bool pair = p->bwd_pairable && ((long long)g_count * (long long)p->bwd_items.size()) >= 2 && !p->no_pair;
+    const int qbox = pair ? kBlock / 2 : kBlock;
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
+        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) || !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox) ||
         !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)p->geom.n * p->geom.L, p->geom.batch, sdq.h * 4, sdq.row * 4,
                           sdq.b * 4, 16))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
@@ -253,6 +272,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     bp.g_first = g_first % p->geom.n;
     bp.g_count = g_count;
     bp.split = p->desc.precision;
+    bp.pair = pair ? 1 : 0;
     bp.ws = bwd_ws + ln.hq0 * N;
     bp.ws_plane = (long long)p->geom.batch * p->desc.heads_q * N;
     bp.vec_stride_b = (long long)p->desc.heads_q * N;
@@ -306,33 +326,84 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
     if (!io || !io->Q_host || !io->K_host || !io->V_host || !io->d_Q || !io->d_K || !io->d_V || !io->d_O || !io->d_lse || !io->d_partial_O ||
         !io->d_partial_lse)
         return fail(MESH_ATTN_EINVAL, "step_host: null pointer");
+    const bool bwd = io->dO_host != nullptr;
+    if (bwd && (!io->d_dO || !io->d_bwd_ws || !io->d_dQ || !io->d_dK || !io->d_dV)) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
+    if (bwd && p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "step_host: the backward kernel is built for head_dim 128 only");
     const Geom& gm = p->geom;
+    const int U = lanes_of(p), nb = gm.b;
     const size_t N = (size_t)gm.n * gm.L;
     const size_t nq = (size_t)gm.batch * N * p->desc.heads_q * gm.head_dim, nk = (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim;
     const size_t nl = (size_t)gm.batch * N * p->desc.heads_q;
-    cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaMemcpyAsync(io->d_Q, io->Q_host, nq * 2, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, st);
-    if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, st);
-    const bool bwd = io->dO_host != nullptr;
-    if (bwd) {
-        if (!io->d_dO || !io->d_bwd_ws || !io->d_dQ || !io->d_dK || !io->d_dV) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
-        if (e == cudaSuccess) e = cudaMemcpyAsync(io->d_dO, io->dO_host, nq * 2, cudaMemcpyHostToDevice, st);
+    cudaStream_t st = (cudaStream_t)stream, up = (cudaStream_t)p->s_h2d, down = (cudaStream_t)p->s_d2h;
+    auto ev = [&](int i) { return (cudaEvent_t)p->copy_events[i]; };
+    // events: 0 start, 1 K,V on the device, 2 dO on the device, 3 forward done, 4 backward done, 5 copies back done,
+    //         6+r Q rows of Q group r on the device, 6+b+r dQ rows of Q group r final
+    // Rows of Q group r are one contiguous byte range when batch == 1 in the [B,N,H,D] layout: then Q goes up and dQ comes
+    // down group by group, behind / ahead of the waves that need them; otherwise whole tensors move.
+    const bool by_group = gm.batch == 1 && p->desc.tensor_layout == 0 && nb > 1;
+    const size_t q_chunk = nq / nb;                   // elements of one Q group's rows
+    cudaError_t e = cudaEventRecord(ev(0), st);
+    auto ok = [&]() { return e == cudaSuccess; };
+    if (ok()) e = cudaStreamWaitEvent(up, ev(0), 0);
+    if (ok()) e = cudaStreamWaitEvent(down, ev(0), 0);
+    // ---- host -> device, in the order the kernels need the data
+    if (ok()) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, up);
+    if (ok()) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, up);
+    if (ok()) e = cudaEventRecord(ev(1), up);
+    for (int r = 0; r < nb && ok(); ++r) {
+        if (by_group) e = cudaMemcpyAsync((char*)io->d_Q + r * q_chunk * 2, (const char*)io->Q_host + r * q_chunk * 2, q_chunk * 2, cudaMemcpyHostToDevice, up);
+        else if (r == 0) e = cudaMemcpyAsync(io->d_Q, io->Q_host, nq * 2, cudaMemcpyHostToDevice, up);
+        if (ok()) e = cudaEventRecord(ev(6 + r), up);
     }
-    if (e != cudaSuccess) return cuda_fail("step_host H2D", (int)e);
-    if (int rc = mesh_attn_forward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_lse, io->d_partial_O, io->d_partial_lse, stream)) return rc;
-    if (bwd)
-        if (int rc = mesh_attn_backward(p, io->d_Q, io->d_K, io->d_V, io->d_O, io->d_dO, io->d_lse, io->d_bwd_ws, io->d_dQ, io->d_dK, io->d_dV, stream))
-            return rc;
-    if (io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * 4, cudaMemcpyDeviceToHost, st);
-    if (e == cudaSuccess && io->lse_host) e = cudaMemcpyAsync(io->lse_host, io->d_lse, nl * 4, cudaMemcpyDeviceToHost, st);
     if (bwd) {
-        if (e == cudaSuccess && io->dQ_host) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * 4, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * 4, cudaMemcpyDeviceToHost, st);
-        if (e == cudaSuccess && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * 4, cudaMemcpyDeviceToHost, st);
+        if (ok()) e = cudaMemcpyAsync(io->d_dO, io->dO_host, nq * 2, cudaMemcpyHostToDevice, up);      // lands during the forward
+        if (ok()) e = cudaEventRecord(ev(2), up);
     }
-    if (e == cudaSuccess) e = cudaStreamSynchronize(st);
-    if (e != cudaSuccess) return cuda_fail("step_host D2H", (int)e);
+    if (!ok()) return cuda_fail("step_host H2D", (int)e);
+    // ---- forward: wave r of every lane needs K, V and the Q rows of group r
+    e = cudaStreamWaitEvent(st, ev(1), 0);
+    for (int lane = 0; lane < U; ++lane)
+        for (int r = 0; r < nb; ++r) {
+            if (lane == 0 && ok()) e = cudaStreamWaitEvent(st, ev(6 + r), 0);
+            if (!ok()) return cuda_fail("step_host forward", (int)e);
+            if (int rc = mesh_attn_tile_fwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_partial_O, io->d_partial_lse, stream)) return rc;
+            if (int rc = mesh_attn_merge(p, lane * nb + r, io->d_partial_O, io->d_partial_lse, io->d_O, io->d_lse, stream)) return rc;
+        }
+    e = cudaEventRecord(ev(3), st);
+    if (ok()) e = cudaStreamWaitEvent(down, ev(3), 0);
+    if (ok() && io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * 4, cudaMemcpyDeviceToHost, down);   // during the backward
+    if (ok() && io->lse_host) e = cudaMemcpyAsync(io->lse_host, io->d_lse, nl * 4, cudaMemcpyDeviceToHost, down);
+    if (bwd) {
+        // ---- backward: the simulated GPUs of Q group r hold exactly the Q partitions of group r, so dQ of those rows is
+        // final once the last lane's call for r has run (Alg.3 l.6)
+        if (ok()) e = cudaStreamWaitEvent(st, ev(2), 0);
+        if (ok()) e = cudaMemsetAsync(io->d_dQ, 0, nq * 4, st);
+        if (ok()) e = cudaMemsetAsync(io->d_dK, 0, nk * 4, st);
+        if (ok()) e = cudaMemsetAsync(io->d_dV, 0, nk * 4, st);
+        if (!ok()) return cuda_fail("step_host backward setup", (int)e);
+        if (int rc = mesh_attn_bwd_preprocess(p, io->d_O, io->d_dO, io->d_lse, io->d_bwd_ws, stream)) return rc;
+        for (int lane = 0; lane < U; ++lane)
+            for (int r = 0; r < nb; ++r) {
+                if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_dO, io->d_bwd_ws, io->d_dQ, io->d_dK,
+                                                io->d_dV, stream))
+                    return rc;
+                if (lane == U - 1 && by_group && io->dQ_host) {
+                    e = cudaEventRecord(ev(6 + nb + r), st);
+                    if (ok()) e = cudaStreamWaitEvent(down, ev(6 + nb + r), 0);
+                    if (ok()) e = cudaMemcpyAsync(io->dQ_host + r * q_chunk, io->d_dQ + r * q_chunk, q_chunk * 4, cudaMemcpyDeviceToHost, down);
+                    if (!ok()) return cuda_fail("step_host dQ D2H", (int)e);
+                }
+            }
+        e = cudaEventRecord(ev(4), st);
+        if (ok()) e = cudaStreamWaitEvent(down, ev(4), 0);
+        if (ok() && io->dQ_host && !by_group) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * 4, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * 4, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * 4, cudaMemcpyDeviceToHost, down);
+    }
+    if (ok()) e = cudaEventRecord(ev(5), down);
+    if (ok()) e = cudaStreamWaitEvent(st, ev(5), 0);
+    if (ok()) e = cudaStreamSynchronize(st);
+    if (!ok()) return cuda_fail("step_host D2H", (int)e);
     return MESH_ATTN_OK;
 }
 

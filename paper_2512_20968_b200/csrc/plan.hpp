@@ -102,6 +102,9 @@ struct mesh_attn_plan {
     std::vector<mesh_attn::BwdItem> bwd_items;
     std::vector<mesh_attn::Seg> fwd_segs, bwd_segs;
     std::vector<mesh_attn::SegList> fwd_seglists, bwd_seglists;
+    // backward items 2k and 2k+1 visit the same Q blocks on every simulated GPU (tile_bwd then runs 2-CTA clusters that
+    // share the Q / dO tile loads); no_pair = environment override MESH_ATTN_NO_PAIR=1 (A/B measurements)
+    bool bwd_pairable = false, no_pair = false;
 
     // device copies (null when no CUDA device was present at creation)
     int device = -1;
@@ -113,6 +116,10 @@ struct mesh_attn_plan {
     const mesh_attn::Seg* d_bwd_segs = nullptr;
     const mesh_attn::SegList* d_fwd_seglists = nullptr;
     const mesh_attn::SegList* d_bwd_seglists = nullptr;
+    // copy streams and events of mesh_attn_step_host (cudaStream_t / cudaEvent_t), created with the device copies
+    void* s_h2d = nullptr;
+    void* s_d2h = nullptr;
+    std::vector<void*> copy_events;               // 2*b + 6
 };
 
 namespace mesh_attn {

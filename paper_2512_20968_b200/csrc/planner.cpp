@@ -12,6 +12,7 @@
 // No CUDA calls here except through mesh_attn::upload_plan (capi.cu).
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <set>
@@ -205,6 +206,37 @@ void build_worklists(mesh_attn_plan* p)
         }
 }
 
+// First Q block of segment sg that item (kv_local, t0) of simulated GPU g visits (the rule of tile_bwd.cu's QWalk).
+int bwd_first_row(const Geom& gm, int g, const Seg& sg, int kv_local, int t0)
+{
+    if (!gm.causal) return sg.begin;
+    const int u = (g / gm.a) * gm.a + sg.part_local, v = kv_partition(gm, g, kv_local);
+    const int x = t0 - causal_off(gm, u, v) - (kBlock - 1);
+    return x > sg.begin ? std::min(sg.end, ((x + kBlock - 1) / kBlock) * kBlock) : sg.begin;
+}
+
+// Do backward items 2k and 2k+1 walk the same (Q partition, head, block) sequence on every simulated GPU?
+bool bwd_items_pairable(const mesh_attn_plan* p)
+{
+    const Geom& gm = p->geom;
+    const size_t cnt = p->bwd_items.size();
+    if (cnt < 2 || cnt % 2) return false;
+    // the walk depends on g only through the causal offsets of the contiguous layout
+    const int g_span = (gm.causal && !gm.striped) ? gm.n : 1;
+    for (int g = 0; g < g_span; ++g)
+        for (size_t k = 0; k < cnt; k += 2) {
+            const BwdItem &x = p->bwd_items[k], &y = p->bwd_items[k + 1];
+            if (x.batch != y.batch || x.head_kv != y.head_kv || x.seglist != y.seglist) return false;
+            if (!gm.causal) continue;
+            const SegList sl = p->bwd_seglists[x.seglist];
+            for (int i = 0; i < sl.count; ++i) {
+                const Seg& sg = p->bwd_segs[sl.offset + i];
+                if (bwd_first_row(gm, g, sg, x.kv_local, x.t0) != bwd_first_row(gm, g, sg, y.kv_local, y.t0)) return false;
+            }
+        }
+    return true;
+}
+
 // number of 128x128 score blocks the forward computes for one simulated GPU g and one head
 int64_t fwd_blocks_of_gpu(const mesh_attn_plan* p, int g)
 {
@@ -299,6 +331,8 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
         trivial_schedule(k_q, k_kv, true, p->steps_bwd, p->order_bwd);
     }
     build_worklists(p);
+    p->bwd_pairable = bwd_items_pairable(p);
+    if (const char* e = std::getenv("MESH_ATTN_NO_PAIR")) p->no_pair = e[0] == '1';
 
     const int rc = upload_plan(p);
     if (rc != MESH_ATTN_OK) { delete p; return rc; }
@@ -484,6 +518,7 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
         }
         case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * Hq * (int64_t)gm.n * gm.L * 4; break;
         case MESH_ATTN_Q_USP_LANES: *value = U; break;
+        case MESH_ATTN_Q_BWD_PAIRED: *value = (p->bwd_pairable && !p->no_pair) ? 1 : 0; break;
         case MESH_ATTN_Q_USP_A2A_BYTES_FWD: {
             // the GPU holds N/(n U) tokens of all heads before the all-to-all and keeps 1/U of them
             const long double tokens = (long double)gm.batch * gm.n * gm.L / ((long double)gm.n * U);

@@ -188,7 +188,12 @@ template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, floa
     }
 }
 
-template <int D, bool kSplit>
+// kPair: the kernel runs as thread-block clusters of two CTAs that take work items 2k and 2k+1, which the planner has
+// checked to walk the SAME sequence of Q blocks (BwdParams::pair).  Each CTA then loads only half of every Q / dO tile
+// (64 rows) and the TMA multicasts it into both CTAs' shared memory, which halves the L2 -> SM tile traffic; a tile slot
+// is released to both loaders (multicast tcgen05.commit) because either one writes into both CTAs.  tmQ / tmdO are then
+// tensor maps with 64-row boxes.
+template <int D, bool kSplit, bool kPair>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmdO,
@@ -232,7 +237,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV); prefetch_tmap(&tmdO); prefetch_tmap(&tmdQ);
         mbar_init(kv_full, 1);
         mbar_init(kv_empty, 1);
-        for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&qd_full[s], 1); mbar_init(&qd_empty[s], 1); }
+        for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&qd_full[s], 1); mbar_init(&qd_empty[s], kPair ? 2 : 1); }
         mbar_init(s_full, 1);
         mbar_init(p_full, kCompute);
         mbar_init(dp_full, 1);
@@ -242,14 +247,16 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(dkv_full, 1);
         mbar_init(dkv_empty, kCompute);
         mbar_init(do_full, 1);
-        mbar_init(do_empty, 1);
+        mbar_init(do_empty, kPair ? 2 : 1);
         fence_mbar_init();
     }
     if (warp == 2) tmem_alloc<512>(tmem_slot);
     tc_fence_before();
     __syncthreads();
+    if constexpr (kPair) cluster_sync();                // the peer's barriers are initialised before anything is sent to them
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
+    const uint32_t pair_rank = kPair ? cluster_ctarank() : 0;
 
     if (warp < 4) reg_dealloc<kCtrlRegs>();
     if (warp == 0) {
@@ -277,8 +284,13 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mbar_wait(&qd_empty[stage], ring_phase ^ 1);
                     mbar_expect_tx(&qd_full[stage], Cfg::kTileBytes + 1024);
                     const int row = u * gm.L + s0;
-                    for (int bx = 0; bx < Cfg::kBoxes; ++bx)
-                        tma_load_4d(sQ(stage) + bx * (kBlock * 128), &tmQ, &qd_full[stage], bx * 64, h, row, c.it.batch, kEvictLast);
+                    for (int bx = 0; bx < Cfg::kBoxes; ++bx) {
+                        if constexpr (kPair)
+                            tma_load_4d_mc(sQ(stage) + bx * (kBlock * 128) + pair_rank * (64 * 128), &tmQ, &qd_full[stage], bx * 64, h,
+                                           row + pair_rank * 64, c.it.batch, 3, kEvictLast);
+                        else
+                            tma_load_4d(sQ(stage) + bx * (kBlock * 128), &tmQ, &qd_full[stage], bx * 64, h, row, c.it.batch, kEvictLast);
+                    }
                     const size_t vec = (size_t)c.it.batch * p.vec_stride_b + (size_t)h * N + row;
                     bulk_load(sLse(stage), nlse + vec, 512, &qd_full[stage]);
                     bulk_load(sDelta(stage), p.ws + vec, 512, &qd_full[stage]);
@@ -286,8 +298,13 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     mbar_wait(do_empty, do_ph ^ 1);      // dV of the previous step has consumed the dO tile
                     do_ph ^= 1;
                     mbar_expect_tx(do_full, Cfg::kTileBytes);
-                    for (int bx = 0; bx < Cfg::kBoxes; ++bx)
-                        tma_load_4d(sdO + bx * (kBlock * 128), &tmdO, do_full, bx * 64, h, row, c.it.batch, kEvictLast);
+                    for (int bx = 0; bx < Cfg::kBoxes; ++bx) {
+                        if constexpr (kPair)
+                            tma_load_4d_mc(sdO + bx * (kBlock * 128) + pair_rank * (64 * 128), &tmdO, do_full, bx * 64, h, row + pair_rank * 64,
+                                           c.it.batch, 3, kEvictLast);
+                        else
+                            tma_load_4d(sdO + bx * (kBlock * 128), &tmdO, do_full, bx * 64, h, row, c.it.batch, kEvictLast);
+                    }
                 }
             }
         }
@@ -355,7 +372,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         for (int kk = 0; kk < kBlock / 16; ++kk)
                             umma_ts(tmem + Cfg::kColDV, tmem + Cfg::kColS + (kk >> 2) * 64 + x * 32 + (kk & 3) * 8,
                                     umma_desc(adO + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(do_empty);               // the dO tile may be refilled for the next step
+                    if constexpr (kPair) umma_commit_mc(do_empty, 3);      // the dO tile may be refilled for the next step
+                    else umma_commit(do_empty);
                     uint32_t st_next = 0;
                     if (Cfg::kStages > 1 && more) {      // S^T(i+1) as early as possible: P^T(i+1) is computed under this step's MMAs
                         st_next = next_stage();
@@ -382,7 +400,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         for (int kk = 0; kk < kBlock / 16; ++kk)
                             umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
                                     umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(&qd_empty[st_cur]);
+                    if constexpr (kPair) umma_commit_mc(&qd_empty[st_cur], 3);
+                    else umma_commit(&qd_empty[st_cur]);
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
@@ -615,19 +634,43 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     tc_fence_before();
     __syncthreads();
+    if constexpr (kPair) cluster_sync();                // no CTA leaves while its peer may still write into it or arrive on its barriers
     if (warp == 2) tmem_dealloc<512>(tmem);
 }
 
-template <int D, bool kSplit>
+template <int D, bool kSplit, bool kPair>
 int launch_one(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmdO,
                const CUtensorMap& tmdQ, int grid, cudaStream_t stream)
 {
     using Cfg = BwdCfg<D, kSplit>;
     static_assert(Cfg::kSmemBytes <= 227 * 1024, "tile_bwd shared memory over the 227 KB CTA limit");
-    cudaError_t e = cudaFuncSetAttribute(tile_bwd_kernel<D, kSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
+    auto kernel = tile_bwd_kernel<D, kSplit, kPair>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
     if (e != cudaSuccess) return (int)e;
-    tile_bwd_kernel<D, kSplit><<<grid, kBwdThreads, Cfg::kSmemBytes, stream>>>(tmQ, tmK, tmV, tmdO, tmdQ, p);
-    return (int)cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.blockDim = dim3(kBwdThreads);
+    cfg.dynamicSmemBytes = Cfg::kSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    if (kPair) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        static int max_clusters = -1;                   // co-resident 2-CTA clusters of this kernel (GPCs with an odd SM count leave one SM out)
+        if (max_clusters < 0) {
+            cfg.gridDim = dim3(2);
+            int n = 0;
+            e = cudaOccupancyMaxActiveClusters(&n, kernel, &cfg);
+            if (e != cudaSuccess) return (int)e;
+            max_clusters = n;
+        }
+        if (max_clusters <= 0) return (int)cudaErrorLaunchOutOfResources;
+        grid = (grid / 2 < max_clusters ? grid / 2 : max_clusters) * 2;
+    }
+    cfg.gridDim = dim3(grid);
+    e = cudaLaunchKernelEx(&cfg, kernel, tmQ, tmK, tmV, tmdO, tmdQ, p);
+    return e != cudaSuccess ? (int)e : (int)cudaGetLastError();
 }
 
 }  // namespace
@@ -639,7 +682,11 @@ int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
-    return p.split ? launch_one<128, true>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream) : launch_one<128, false>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
+    if (p.pair)
+        return p.split ? launch_one<128, true, true>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
+                       : launch_one<128, false, true>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
+    return p.split ? launch_one<128, true, false>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
+                   : launch_one<128, false, false>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
 }
 
 }  // namespace mesh_attn

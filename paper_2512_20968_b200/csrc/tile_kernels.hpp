@@ -27,6 +27,7 @@ struct BwdParams {
     int items_per_gpu;
     int g_first, g_count;
     int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
+    int pair;                  // 1: items 2k, 2k+1 walk the same Q blocks -> 2-CTA clusters with multicast Q/dO tiles (tmQ, tmdO: 64-row boxes)
     const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess); head 0 = first head of the lane
     long long ws_plane;        // elements between ws[0] and ws[1] (B * all heads * N)
     long long vec_stride_b;    // batch stride of the [B][Hq][N] vectors (all heads * N)

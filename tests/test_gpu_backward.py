@@ -80,6 +80,32 @@ def test_scaled_configs_full_keys(oracle, name, L, hq):
     check_invariants(w, inp, buf)
 
 
+@pytest.mark.parametrize("name", ["C2", "C5"])
+def test_paired_and_unpaired_kernel_variants(oracle, monkeypatch, name):
+    """tile_bwd as 2-CTA clusters with multicast Q / dO tiles (MESH_ATTN_Q_BWD_PAIRED) and as single CTAs
+    (MESH_ATTN_NO_PAIR=1 at plan creation): both against the oracle, and against each other."""
+    from paper_2512_20968_b200.binding import Q_BWD_PAIRED
+
+    w = W.scaled_down(W.CONFIGS[name], 256, heads_q=2)
+    if w.n > 16:
+        w = replace(w, a=4, b=4, seq_total=16 * 256)         # C5's mask, layout and order on a 4 x 4 mesh
+    inp = W.make_inputs(w, "cuda")
+    rng = np.random.default_rng(5)
+    rows = np.unique(np.concatenate([rng.integers(0, w.seq_total, 32), [0, w.seq_total - 1, w.L - 1, w.L]]))
+    qrows, qheads = all_pairs(rows, range(w.heads_q))
+    krows, kheads = all_pairs(rows[:16], range(w.heads_kv))
+    bufs = []
+    for no_pair in ("0", "1"):
+        monkeypatch.setenv("MESH_ATTN_NO_PAIR", no_pair)
+        plan, buf = run_fwd_bwd(w, inp)
+        assert plan.query(Q_BWD_PAIRED) == (1 if no_pair == "0" else 0)
+        check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
+        check_invariants(w, inp, buf)
+        bufs.append(buf)
+    for x, y in ((bufs[0].dQ, bufs[1].dQ), (bufs[0].dK, bufs[1].dK), (bufs[0].dV, bufs[1].dV)):
+        assert (x - y).abs().max().item() <= 1e-3            # atomics: the summation order is run-dependent
+
+
 @pytest.mark.parametrize("layout,kvr", [("contiguous", True), ("striped", False), ("striped", True)])
 def test_causal_small_full(oracle, layout, kvr):
     """every row / key of a small causal problem (3x2 mesh, GQA 2:1): exercises diagonal blocks, fully masked

@@ -222,3 +222,17 @@ def test_usp_lanes_geometry_and_all_to_all_volume():
     # GQA: K and V move Hkv heads only; n mesh GPUs per lane hold N/(n U) tokens each
     p = Plan(usp_lanes=4, **kw)
     assert p.query(B.Q_USP_A2A_BYTES_FWD) == (4 * 256 // (4 * 4)) * 3 * (2 * 16 + 2 * 8) * 128 * 2 // 4
+
+
+def test_backward_item_pairing_rule():
+    """tile_bwd shares Q / dO tile loads between two CTAs only when items 2k, 2k+1 visit the same Q blocks: always for
+    non-causal plans, for striped-causal plans (same key block of two KV partitions: the causal offset 0 / -1 does not
+    move the first visible Q block), never when the item count is odd or the contiguous causal layout shifts the walks."""
+    kw = dict(batch=1, heads_q=2, heads_kv=1, head_dim=128)
+    assert Plan(a=2, b=2, seq_total=4 * 256, **kw).query(B.Q_BWD_PAIRED) == 1
+    assert Plan(a=2, b=2, seq_total=4 * 256, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 1
+    assert Plan(a=4, b=4, seq_total=16 * 256, causal=1, seq_layout=1, order=1, kvr=1, **kw).query(B.Q_BWD_PAIRED) == 1
+    assert Plan(a=2, b=2, seq_total=4 * 256, causal=1, seq_layout=0, **kw).query(B.Q_BWD_PAIRED) == 0
+    assert Plan(a=1, b=1, seq_total=128, **kw).query(B.Q_BWD_PAIRED) == 0          # a single item
+    assert Plan(a=3, b=3, seq_total=9 * 128, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 0   # 3 partitions per key block
+    assert Plan(a=3, b=3, seq_total=9 * 256, **kw).query(B.Q_BWD_PAIRED) == 1
