@@ -30,8 +30,8 @@ METRIC = "attention_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one ncu capture of this command
-# (profiles/r01_v5_traffic_c5_tile_bwd.csv; profiles/r01_v6_ncu_c2_bwd.txt, r01_v5_ncu_c2_fwd.txt): workload -> kernel -> bytes
-NCU_TRAFFIC = {"C5": {"tile_bwd": 2183521001472 + 1133708182272}, "C2": {"tile_bwd": 3047004000 + 1805074000, "tile_fwd": 908874752 + 569961216}}
+# (profiles/r01_v6_traffic_c5_tile_bwd.csv; profiles/r01_v6_ncu_c2_bwd.txt, r01_v5_ncu_c2_fwd.txt): workload -> kernel -> bytes
+NCU_TRAFFIC = {"C5": {"tile_bwd": 2134681542144 + 1102663412992}, "C2": {"tile_bwd": 3047004000 + 1805074000, "tile_fwd": 908874752 + 569961216}}
 
 
 def parse_args():
