@@ -204,8 +204,9 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const float* O, const v
  * and ACCUMULATE (atomic fp32 adds: the sums of Alg.3 l.6-7 and the GQA group sum)
  *   dV_v += P^T dO_u,  dK_v += scale dS^T Q_u,  dQ_u += scale dS K_v.
  * bwd_ws is what mesh_attn_bwd_preprocess wrote.  The caller zeroes dQ, dK, dV before the
- * first call.  head_dim must be 128 (EUNSUPPORTED otherwise: the kernel's transposed dQ
- * accumulator needs head_dim = 128 rows). */
+ * first call.  head_dim 64 runs the head_dim-128 kernel on zero-padded tiles (the TMA fills the
+ * out-of-bounds upper 64 columns with zeros; the transposed dQ accumulator needs 128 rows), i.e.
+ * at half the tensor-core efficiency. */
 int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_count,
                        const void* Q, const void* K, const void* V, const void* dO,
                        const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream);

@@ -245,7 +245,6 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
 {
     if (int rc = check_device(p, "tile_bwd")) return rc;
     if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
-    if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "tile_bwd: the backward kernel is built for head_dim 128 only");
     Lane ln;
     if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds (or crossing a USP lane)");
     if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
@@ -303,7 +302,6 @@ int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, co
                        const float* lse, float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
 {
     if (int rc = check_device(p, "backward")) return rc;
-    if (p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "backward: the backward kernel is built for head_dim 128 only");
     if (!dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward: null pointer");
     const Geom& gm = p->geom;
     const size_t N = (size_t)gm.n * gm.L;
@@ -328,7 +326,6 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
         return fail(MESH_ATTN_EINVAL, "step_host: null pointer");
     const bool bwd = io->dO_host != nullptr;
     if (bwd && (!io->d_dO || !io->d_bwd_ws || !io->d_dQ || !io->d_dK || !io->d_dV)) return fail(MESH_ATTN_EINVAL, "step_host: null backward buffer");
-    if (bwd && p->geom.head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "step_host: the backward kernel is built for head_dim 128 only");
     const Geom& gm = p->geom;
     const int U = lanes_of(p), nb = gm.b;
     const size_t N = (size_t)gm.n * gm.L;

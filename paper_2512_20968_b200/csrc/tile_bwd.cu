@@ -174,10 +174,10 @@ __device__ __forceinline__ void tma_reduce_add_4d(const CUtensorMap* m, const vo
 }
 // TMEM accumulator [128 lanes x D columns] -> x scale -> atomic add into a global row of D floats
 // (item epilogue only: once per 128-key block)
-template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, float* grow, float scale)
+template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, float* grow, float scale, int dv)
 {
 #pragma unroll 1
-    for (int ch = 0; ch < D / 32; ++ch) {
+    for (int ch = 0; ch < dv / 32; ++ch) {                  // dv = the tensors' head_dim (64: the upper accumulator columns are zero)
         uint32_t r[32];
         tmem_ld_x32(taddr + ch * 32, r);
         tmem_ld_wait();
@@ -576,7 +576,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_after();
             float* grow = (wg == 0 ? p.dK : p.dV) + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
                           (size_t)c.it.head_kv * p.k_stride_h;
-            drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? 1.0f : 1.0f / gm.scale);
+            drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? 1.0f : 1.0f / gm.scale, gm.head_dim);
             tc_fence_before();
             mbar_arrive(dkv_empty);
         }
@@ -593,6 +593,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const int d = ((warp & 3) << 5) | lane;
         const uint32_t tDQ = tmem + ((uint32_t)((warp & 3) * 32) << 16) + Cfg::kColDP;
         const bool issuer = threadIdx.x == 12 * 32;
+        const int dv = gm.head_dim;                      // 64: dQ^T rows 64..127 are zero and stay in the CTA
         uint32_t dq_ph = 0;
         PT_DECL;
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
@@ -613,11 +614,12 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 PT_MARK(1);
 #pragma unroll
                 for (int k = 0; k < kBlock / Cfg::kStgRows; ++k) {   // 16-query slice k through staging buffer k % kStgBufs
-                    float* stg = sStg + (k % Cfg::kStgBufs) * (Cfg::kStgRows * D);
+                    float* stg = sStg + (k % Cfg::kStgBufs) * (Cfg::kStgRows * D);      // rows of dv floats (the reduce's box)
                     if (issuer) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(Cfg::kStgBufs - 1) : "memory");   // slice k - kStgBufs has been read
                     named_bar_sync(1, kBlock);
 #pragma unroll
-                    for (int j = 0; j < Cfg::kStgRows; ++j) stg[j * D + d] = __uint_as_float(r[k * Cfg::kStgRows + j]);
+                    for (int j = 0; j < Cfg::kStgRows; ++j)
+                        if (d < dv) stg[j * dv + d] = __uint_as_float(r[k * Cfg::kStgRows + j]);
                     fence_proxy_async_smem();
                     named_bar_sync(1, kBlock);
                     if (issuer) {
@@ -678,7 +680,8 @@ int launch_one(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tm
 int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmdO,
                     const CUtensorMap& tmdQ, int num_sms, cudaStream_t stream)
 {
-    if (p.gm.head_dim != 128) return (int)cudaErrorNotSupported;     // capi.cu reports EUNSUPPORTED before getting here
+    // head_dim 64 runs the head_dim-128 kernel: the TMA zero-fills the out-of-bounds upper 64 columns of every tile
+    if (p.gm.head_dim != 128 && p.gm.head_dim != 64) return (int)cudaErrorNotSupported;
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
