@@ -109,6 +109,11 @@ enum {
                                               2k and 2k+1 visit the same Q blocks on every simulated GPU (holds for non-causal and
                                               striped-causal plans with an even item count; MESH_ATTN_NO_PAIR=1 in the environment
                                               at plan_create forces 0) */
+    MESH_ATTN_Q_GOO_PARTIAL_O_BYTES = 19,  /* mesh_attn_forward_goo: bytes of partial_O for ONE simulated GPU (a*k_kv slots); x a */
+    MESH_ATTN_Q_GOO_PARTIAL_LSE_BYTES = 20,
+    MESH_ATTN_Q_GOO_COMM_BYTES = 21,       /* bytes the forward step list's collectives move for the a GPUs of one Q group:
+                                              k_q (AG-Q + RS-Q) of (a-1) Q chunks + k_kv AG-KV of (b-1) K and V chunks, each x a
+                                              (= a x MESH_ATTN_Q_MESH_COMM_BYTES_FWD, the per-GPU volume of P:L290-292) */
     MESH_ATTN_Q_USP_A2A_BYTES_FWD = 17     /* per-GPU forward volume of the Ulysses all-to-alls around the lanes (Q, K, V in,
                                               O out): (U-1)/U of the GPU's N/(n*U) tokens x (2 Hq + 2 Hkv) head_dim x 2 bytes;
                                               with n = 1 and Hq = Hkv this is Table 1's Ulysses entry 4(U-1)/U^2 N d */
@@ -216,6 +221,20 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_co
  * tile_fwd / tile_bwd ranges [g_first, g_first+g_count) must stay inside one lane (EINVAL). */
 int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
                       float* O, float* lse, float* partial_O, float* partial_lse, void* stream);
+
+/* GOO executor for the `a` simulated GPUs of Q group q_group: runs the plan's forward STEP
+ * LIST (mesh_attn_plan_steps) step by step.  A step's compute tasks C-i-j (Q chunk i of every Q partition of the group
+ * against KV chunk j of every KV partition of each GPU's footprint) are chunk-granular tile_fwd launches on `stream`
+ * writing partial slot (g - g_first, u_local*k_kv + j); the step's communication task (AG-KV-j, AG-Q-i, RS-Q-i) is stood
+ * in for by device-to-device copies of the bytes it would move for these `a` GPUs (repeated comm_repeat times to model
+ * a slower link; 0 = no copies) into comm_ws, on a plan-owned stream when overlap != 0 (else on `stream`, i.e.
+ * serialised with the compute); both streams join at the end of every step.  Last, the a*k_kv partials of every
+ * row are merged into O and lse.  One GPU holds all of Q, K, V, so the copies carry no data dependence: they reproduce
+ * the schedule's timing, the result is the attention of mesh_attn_forward.  partial_O / partial_lse: `a` x
+ * MESH_ATTN_Q_GOO_PARTIAL_*_BYTES.  Time it with events on `stream`. */
+int mesh_attn_forward_goo(const mesh_attn_plan* plan, int32_t q_group, const void* Q, const void* K, const void* V,
+                          float* O, float* lse, float* partial_O, float* partial_lse,
+                          void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap, void* stream);
 
 /* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
 int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,

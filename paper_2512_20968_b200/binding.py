@@ -24,7 +24,7 @@ lib = C.CDLL(str(_LIB_PATH))
 OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 (Q_PARTIAL_O_BYTES, Q_PARTIAL_LSE_BYTES, Q_SLOTS_PER_GPU, Q_FLOPS_FWD, Q_FLOPS_BWD, Q_WAVES, Q_MERGE_BYTES,
  Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE, Q_BWD_WS_BYTES,
- Q_MESH_COMM_BYTES_FWD, Q_MESH_COMM_BYTES_BWD, Q_RING_COMM_BYTES_FWD, Q_USP_LANES, Q_USP_A2A_BYTES_FWD, Q_BWD_PAIRED) = range(19)
+ Q_MESH_COMM_BYTES_FWD, Q_MESH_COMM_BYTES_BWD, Q_RING_COMM_BYTES_FWD, Q_USP_LANES, Q_USP_A2A_BYTES_FWD, Q_BWD_PAIRED, Q_GOO_PARTIAL_O_BYTES, Q_GOO_PARTIAL_LSE_BYTES, Q_GOO_COMM_BYTES) = range(22)
 TASK_AG_KV, TASK_AG_Q, TASK_RS_Q, TASK_C, TASK_RS_KV = range(5)
 
 
@@ -64,6 +64,7 @@ lib.mesh_attn_merge.argtypes = [_P, C.c_int32, _P, _P, _P, _P, _P]
 lib.mesh_attn_bwd_preprocess.argtypes = [_P] * 6
 lib.mesh_attn_tile_bwd.argtypes = [_P, C.c_int32, C.c_int32] + [_P] * 9
 lib.mesh_attn_forward.argtypes = [_P] * 9
+lib.mesh_attn_forward_goo.argtypes = [_P, C.c_int32] + [_P] * 8 + [C.c_int64, C.c_int32, C.c_int32, _P]
 lib.mesh_attn_backward.argtypes = [_P] * 12
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
 lib.mesh_attn_launch_count.restype = C.c_int64
@@ -76,7 +77,7 @@ lib.mesh_attn_last_error.restype = C.c_char_p
 EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
-    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
+    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
 ]
 K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
@@ -198,6 +199,11 @@ class Plan:
 
     def forward(self, Q, K, V, O, lse, partial_O, partial_lse, stream=None):
         _check(lib.mesh_attn_forward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _ptr(partial_O), _ptr(partial_lse), _stream(stream)))
+
+    def forward_goo(self, q_group, Q, K, V, O, lse, partial_O, partial_lse, comm_ws=None, comm_repeat=0, overlap=True, stream=None):
+        nbytes = 0 if comm_ws is None else comm_ws.numel() * comm_ws.element_size()
+        _check(lib.mesh_attn_forward_goo(self._h, q_group, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _ptr(partial_O), _ptr(partial_lse),
+                                         _ptr(comm_ws), nbytes, comm_repeat, int(bool(overlap)), _stream(stream)))
 
     def backward(self, Q, K, V, O, dO, lse, bwd_ws, dQ, dK, dV, stream=None):
         _check(lib.mesh_attn_backward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(lse), _ptr(bwd_ws),

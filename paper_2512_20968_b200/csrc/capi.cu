@@ -1,6 +1,7 @@
 // capi.cu -- C-ABI entry points of libmesh_attn.so (include/mesh_attn.h): argument checking,
 // TMA tensor-map construction, kernel launches.  No allocation and no host synchronisation in
 // the hot calls; every launch goes to the caller's stream.
+#include <algorithm>
 #include <atomic>
 #include <cstdio>
 #include <cstring>
@@ -114,9 +115,10 @@ int upload_plan(mesh_attn_plan* p)
     auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
     const size_t b0 = al(p->fwd_items.size() * sizeof(FwdItem)), b1 = al(p->bwd_items.size() * sizeof(BwdItem)),
                  b2 = al(p->fwd_segs.size() * sizeof(Seg)), b3 = al(p->bwd_segs.size() * sizeof(Seg)),
-                 b4 = al(p->fwd_seglists.size() * sizeof(SegList)), b5 = al(p->bwd_seglists.size() * sizeof(SegList));
+                 b4 = al(p->fwd_seglists.size() * sizeof(SegList)), b5 = al(p->bwd_seglists.size() * sizeof(SegList)),
+                 b6 = al(p->goo_items.size() * sizeof(FwdItem));
     char* d = nullptr;
-    cudaError_t e = cudaMalloc(&d, b0 + b1 + b2 + b3 + b4 + b5 + 256);
+    cudaError_t e = cudaMalloc(&d, b0 + b1 + b2 + b3 + b4 + b5 + b6 + 256);
     if (e != cudaSuccess) return cuda_fail("cudaMalloc(work lists)", (int)e);
     p->d_blob = d;
     auto put = [&](const void* src, size_t bytes, size_t cap) {
@@ -131,13 +133,14 @@ int upload_plan(mesh_attn_plan* p)
     p->d_bwd_segs = (const Seg*)put(p->bwd_segs.data(), p->bwd_segs.size() * sizeof(Seg), b3);
     p->d_fwd_seglists = (const SegList*)put(p->fwd_seglists.data(), p->fwd_seglists.size() * sizeof(SegList), b4);
     p->d_bwd_seglists = (const SegList*)put(p->bwd_seglists.data(), p->bwd_seglists.size() * sizeof(SegList), b5);
+    p->d_goo_items = (const FwdItem*)put(p->goo_items.data(), p->goo_items.size() * sizeof(FwdItem), b6);
     if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
     // step_host's copy engines: one stream per direction, events for the chunk hand-offs
     cudaStream_t s0 = nullptr, s1 = nullptr;
     e = cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s1, cudaStreamNonBlocking);
     p->s_h2d = s0; p->s_d2h = s1;
-    for (int i = 0; e == cudaSuccess && i < 2 * p->geom.b + 6; ++i) {
+    for (int i = 0; e == cudaSuccess && i < 2 * p->geom.b + 8; ++i) {
         cudaEvent_t ev = nullptr;
         e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
         if (e == cudaSuccess) p->copy_events.push_back(ev);
@@ -160,24 +163,27 @@ void free_plan_device(mesh_attn_plan* p)
 
 extern "C" {
 
-int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
-                       float* partial_O, float* partial_lse, void* stream)
+// tile_fwd over an item list (the plan's fused list, or one compute task of the GOO executor)
+static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int items_per_gpu, int slots_per_gpu, int32_t g_first, int32_t g_count,
+                           const void* Q, const void* K, const void* V, float* partial_O, float* partial_lse, void* stream, const char* who)
 {
-    if (int rc = check_device(p, "tile_fwd")) return rc;
-    if (!Q || !K || !V || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, "tile_fwd: null pointer");
+    if (int rc = check_device(p, who)) return rc;
+    if (!Q || !K || !V || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null pointer");
     Lane ln;
-    if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_fwd: simulated GPU range out of bounds (or crossing a USP lane)");
-    if ((long long)g_count * (long long)p->fwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_fwd: too many work items in one call");
+    if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, std::string(who) + ": simulated GPU range out of bounds (or crossing a USP lane)");
+    if ((long long)g_count * (long long)items_per_gpu >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, std::string(who) + ": too many work items in one call");
+    if (items_per_gpu == 0) return MESH_ATTN_OK;
     CUtensorMap tmQ, tmK, tmV;
     if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
         !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0))
-        return fail(MESH_ATTN_ECUDA, "tile_fwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
+        return fail(MESH_ATTN_ECUDA, std::string(who) + ": cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     FwdParams fp;
     fp.gm = p->geom;
-    fp.items = p->d_fwd_items;
+    fp.gm.slots_per_gpu = slots_per_gpu;
+    fp.items = items;
     fp.segs = p->d_fwd_segs;
     fp.seglists = p->d_fwd_seglists;
-    fp.items_per_gpu = (int)p->fwd_items.size();
+    fp.items_per_gpu = items_per_gpu;
     fp.g_first = g_first % p->geom.n;
     fp.g_count = g_count;
     fp.split = p->desc.precision;
@@ -185,13 +191,13 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     fp.partial_lse = partial_lse;
     ProfScope prof(MESH_ATTN_K_TILE_FWD, (cudaStream_t)stream);
     const int e = launch_tile_fwd(fp, tmQ, tmK, tmV, p->num_sms, (cudaStream_t)stream);
-    if (e) return cuda_fail("tile_fwd launch", e);
+    if (e) return cuda_fail(who, e);
     g_launches.fetch_add(1);
     return MESH_ATTN_OK;
 }
 
-int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, float* O, float* lse,
-                    void* stream)
+static int launch_merge_slots(const mesh_attn_plan* p, int32_t q_group, int per, int slots_per_gpu, const float* partial_O, const float* partial_lse,
+                              float* O, float* lse, void* stream)
 {
     if (int rc = check_device(p, "merge")) return rc;
     if (!partial_O || !partial_lse || !O || !lse) return fail(MESH_ATTN_EINVAL, "merge: null pointer");
@@ -201,8 +207,9 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
     const long long N = (long long)p->geom.n * p->geom.L;
     MergeParams mp;
     mp.gm = p->geom;
+    mp.gm.slots_per_gpu = slots_per_gpu;
     mp.q_group = q_group % p->geom.b;
-    mp.per = p->desc.partial_mode == 1 ? p->geom.b : 1;
+    mp.per = per;
     mp.m = p->geom.a * mp.per;
     int rows = 8;
     while (rows > 1 && ((size_t)rows * p->geom.heads_q * mp.m * 4 > 64 * 1024 || p->geom.L % rows)) rows >>= 1;
@@ -220,6 +227,21 @@ int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* parti
     if (e) return cuda_fail("merge launch", e);
     g_launches.fetch_add(1);
     return MESH_ATTN_OK;
+}
+
+int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
+                       float* partial_O, float* partial_lse, void* stream)
+{
+    if (int rc = check_device(p, "tile_fwd")) return rc;
+    return launch_fwd_list(p, p->d_fwd_items, (int)p->fwd_items.size(), p->geom.slots_per_gpu, g_first, g_count, Q, K, V, partial_O, partial_lse, stream,
+                           "tile_fwd");
+}
+
+int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, float* O, float* lse,
+                    void* stream)
+{
+    if (int rc = check_device(p, "merge")) return rc;
+    return launch_merge_slots(p, q_group, p->desc.partial_mode == 1 ? p->geom.b : 1, p->geom.slots_per_gpu, partial_O, partial_lse, O, lse, stream);
 }
 
 int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void* dO, const float* lse, float* bwd_ws, void* stream)
@@ -296,6 +318,84 @@ int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, con
             if (int rc = mesh_attn_merge(p, lane * p->geom.b + r, partial_O, partial_lse, O, lse, stream)) return rc;
         }
     return MESH_ATTN_OK;
+}
+
+// bytes the collective task (kind) delivers to / takes from the `a` simulated GPUs of one Q group
+static long long goo_task_bytes(const mesh_attn_plan* p, int kind)
+{
+    const Geom& gm = p->geom;
+    const long long unit_q = (long long)gm.batch * (gm.L / p->k_q) * gm.heads_q * gm.head_dim * 2;      // one Q chunk (bf16; O counted alike, L35)
+    const long long unit_kv = (long long)gm.batch * (gm.L / p->k_kv) * gm.heads_kv * gm.head_dim * 2;   // one K (or V) chunk
+    switch (kind) {
+        case MESH_ATTN_TASK_AG_Q: case MESH_ATTN_TASK_RS_Q: return (long long)gm.a * (gm.a - 1) * unit_q;
+        case MESH_ATTN_TASK_AG_KV: return (long long)gm.a * (gm.b - 1) * 2 * unit_kv;
+        default: return 0;
+    }
+}
+
+int mesh_attn_forward_goo(const mesh_attn_plan* p, int32_t q_group, const void* Q, const void* K, const void* V, float* O, float* lse,
+                          float* partial_O, float* partial_lse, void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap,
+                          void* stream)
+{
+    if (int rc = check_device(p, "forward_goo")) return rc;
+    if (!Q || !K || !V || !O || !lse || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, "forward_goo: null pointer");
+    if (comm_repeat < 0 || (comm_repeat > 0 && (!comm_ws || comm_ws_bytes < 4096))) return fail(MESH_ATTN_EINVAL, "forward_goo: comm_ws too small");
+    const Geom& gm = p->geom;
+    if (q_group < 0 || q_group >= gm.b * lanes_of(p)) return fail(MESH_ATTN_EINVAL, "forward_goo: q_group out of range");
+    const int lane = q_group / gm.b, r = q_group % gm.b, g_first = lane * gm.n + r * gm.a, slots = gm.a * p->k_kv;
+    cudaStream_t st = (cudaStream_t)stream, cs = overlap ? (cudaStream_t)p->s_h2d : st;
+    cudaEvent_t ev_fork = (cudaEvent_t)p->copy_events[2 * gm.b + 6], ev_join = (cudaEvent_t)p->copy_events[2 * gm.b + 7];
+    const long long q_bytes = (long long)gm.batch * gm.n * gm.L * p->desc.heads_q * gm.head_dim * 2;
+    const long long kv_bytes = (long long)gm.batch * gm.n * gm.L * p->desc.heads_kv * gm.head_dim * 2;
+    const long long part_bytes = (long long)gm.a * slots * gm.batch * gm.L * gm.heads_q * gm.head_dim * 4;
+    // stand-in for a collective: device-to-device copies of its byte count out of the tensor it would move
+    auto copy_bytes = [&](const void* src, long long src_bytes, long long bytes) -> cudaError_t {
+        const long long chunk = std::min<long long>(std::min<long long>(src_bytes, comm_ws_bytes), bytes);
+        for (int rep = 0; rep < comm_repeat; ++rep)
+            for (long long done = 0; done < bytes; done += chunk) {
+                const cudaError_t e = cudaMemcpyAsync(comm_ws, src, (size_t)std::min(chunk, bytes - done), cudaMemcpyDeviceToDevice, cs);
+                if (e != cudaSuccess) return e;
+            }
+        return cudaSuccess;
+    };
+    const std::vector<int32_t>& rows = p->steps_fwd;
+    const size_t nrows = rows.size() / 4;
+    for (size_t at = 0; at < nrows;) {
+        const int step = rows[4 * at];
+        cudaError_t e = cudaSuccess;
+        if (overlap) {
+            e = cudaEventRecord(ev_fork, st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_fork, 0);
+        }
+        // the step's communication task first (its own stream when overlapping), then its compute tasks
+        for (size_t k = at; k < nrows && rows[4 * k] == step && e == cudaSuccess; ++k) {
+            const int kind = rows[4 * k + 1];
+            if (comm_repeat == 0 || kind == MESH_ATTN_TASK_C) continue;
+            const long long bytes = goo_task_bytes(p, kind);
+            if (kind == MESH_ATTN_TASK_AG_Q) e = copy_bytes(Q, q_bytes, bytes);
+            else if (kind == MESH_ATTN_TASK_RS_Q) e = copy_bytes(partial_O, part_bytes, bytes);
+            else if (kind == MESH_ATTN_TASK_AG_KV) {
+                e = copy_bytes(K, kv_bytes, bytes / 2);
+                if (e == cudaSuccess) e = copy_bytes(V, kv_bytes, bytes / 2);
+            }
+        }
+        if (e != cudaSuccess) return cuda_fail("forward_goo: communication stand-in", (int)e);
+        size_t k = at;
+        for (; k < nrows && rows[4 * k] == step; ++k) {
+            if (rows[4 * k + 1] != MESH_ATTN_TASK_C) continue;
+            const SegList task = p->goo_task[(size_t)rows[4 * k + 2] * p->k_kv + rows[4 * k + 3]];
+            if (int rc = launch_fwd_list(p, p->d_goo_items + task.offset, task.count, slots, g_first, gm.a, Q, K, V, partial_O, partial_lse, stream,
+                                         "forward_goo"))
+                return rc;
+        }
+        if (overlap) {                                       // a step ends when its communication and its computation are done
+            e = cudaEventRecord(ev_join, cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_join, 0);
+            if (e != cudaSuccess) return cuda_fail("forward_goo: step barrier", (int)e);
+        }
+        at = k;
+    }
+    return launch_merge_slots(p, q_group, p->k_kv, slots, partial_O, partial_lse, O, lse, stream);
 }
 
 int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const float* O, const void* dO,

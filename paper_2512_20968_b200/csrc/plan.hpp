@@ -102,6 +102,11 @@ struct mesh_attn_plan {
     std::vector<mesh_attn::BwdItem> bwd_items;
     std::vector<mesh_attn::Seg> fwd_segs, bwd_segs;
     std::vector<mesh_attn::SegList> fwd_seglists, bwd_seglists;
+    // chunk-granular forward lists for the GOO executor (mesh_attn_forward_goo): the items of compute task C-i-j
+    // (Q chunk i of every Q partition x KV chunk j of every KV partition) are
+    // goo_items[goo_task[i*k_kv+j].offset .. +count), partial slot = u_local*k_kv + j
+    std::vector<mesh_attn::FwdItem> goo_items;
+    std::vector<mesh_attn::SegList> goo_task;
     // backward items 2k and 2k+1 visit the same Q blocks on every simulated GPU (tile_bwd then runs 2-CTA clusters that
     // share the Q / dO tile loads); no_pair = environment override MESH_ATTN_NO_PAIR=1 (A/B measurements)
     bool bwd_pairable = false, no_pair = false;
@@ -111,6 +116,7 @@ struct mesh_attn_plan {
     int num_sms = 0;
     void* d_blob = nullptr;
     const mesh_attn::FwdItem* d_fwd_items = nullptr;
+    const mesh_attn::FwdItem* d_goo_items = nullptr;
     const mesh_attn::BwdItem* d_bwd_items = nullptr;
     const mesh_attn::Seg* d_fwd_segs = nullptr;
     const mesh_attn::Seg* d_bwd_segs = nullptr;

@@ -182,6 +182,39 @@ void build_worklists(mesh_attn_plan* p)
             }
         }
 
+    // ---------- forward, one list per compute task C-i-j (GOO executor) ----------
+    p->goo_task.assign((size_t)p->k_q * p->k_kv, SegList{0, 0});
+    for (auto& task : p->order_fwd) {
+        const int i = task.first, j = task.second;
+        SegList sl{(int32_t)p->fwd_segs.size(), 0};
+        for (int jj = 0; jj < gm.b; ++jj) { p->fwd_segs.push_back(Seg{jj, j * Lkv, (j + 1) * Lkv}); ++sl.count; }
+        const int list_id = (int)p->fwd_seglists.size();
+        p->fwd_seglists.push_back(sl);
+        SegList range{(int32_t)p->goo_items.size(), 0};
+        for (int bt = 0; bt < gm.batch; ++bt)
+            for (int hk = 0; hk < gm.heads_kv; ++hk) {
+                std::vector<FwdItem> grp;
+                for (int h = hk * gm.group; h < (hk + 1) * gm.group; ++h)
+                    for (int ul = 0; ul < gm.a; ++ul)
+                        for (int q0 = i * Lq; q0 < (i + 1) * Lq; q0 += 2 * kBlock) {
+                            FwdItem it{};
+                            it.batch = (int16_t)bt;
+                            it.u_local = (int16_t)ul;
+                            it.head = (int16_t)h;
+                            it.seglist = (int16_t)list_id;
+                            it.q0 = q0;
+                            it.nrows = (int16_t)std::min(2 * kBlock, (i + 1) * Lq - q0);
+                            it.slot = (int16_t)(ul * p->k_kv + j);
+                            grp.push_back(it);
+                        }
+                if (gm.causal)
+                    std::stable_sort(grp.begin(), grp.end(), [](const FwdItem& x, const FwdItem& y) { return x.q0 > y.q0; });
+                p->goo_items.insert(p->goo_items.end(), grp.begin(), grp.end());
+            }
+        range.count = (int32_t)p->goo_items.size() - range.offset;
+        p->goo_task[(size_t)i * p->k_kv + j] = range;
+    }
+
     // ---------- backward: item = (batch, kv_local, kv head, 128-key block) ----------
     const std::vector<int> kv_chunks_b = first_appearance<int>(p->order_bwd, false);
     for (int bt = 0; bt < gm.batch; ++bt)
@@ -518,6 +551,15 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
         }
         case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * Hq * (int64_t)gm.n * gm.L * 4; break;
         case MESH_ATTN_Q_USP_LANES: *value = U; break;
+        case MESH_ATTN_Q_GOO_PARTIAL_O_BYTES: *value = (int64_t)gm.a * p->k_kv * unit * gm.head_dim * 4; break;
+        case MESH_ATTN_Q_GOO_PARTIAL_LSE_BYTES: *value = (int64_t)gm.a * p->k_kv * unit * 4; break;
+        case MESH_ATTN_Q_GOO_COMM_BYTES: {
+            // what the forward step list moves for ONE Q group (its a simulated GPUs): k_q AG-Q + k_q RS-Q + k_kv AG-KV tasks
+            const int64_t unit_q = (int64_t)gm.batch * (gm.L / p->k_q) * gm.heads_q * gm.head_dim * 2;
+            const int64_t unit_kv = (int64_t)gm.batch * (gm.L / p->k_kv) * gm.heads_kv * gm.head_dim * 2;
+            *value = (int64_t)gm.a * (2ll * p->k_q * (gm.a - 1) * unit_q + 2ll * p->k_kv * (gm.b - 1) * unit_kv);
+            break;
+        }
         case MESH_ATTN_Q_BWD_PAIRED: *value = (p->bwd_pairable && !p->no_pair) ? 1 : 0; break;
         case MESH_ATTN_Q_USP_A2A_BYTES_FWD: {
             // the GPU holds N/(n U) tokens of all heads before the all-to-all and keeps 1/U of them

@@ -236,3 +236,13 @@ def test_backward_item_pairing_rule():
     assert Plan(a=1, b=1, seq_total=128, **kw).query(B.Q_BWD_PAIRED) == 0          # a single item
     assert Plan(a=3, b=3, seq_total=9 * 128, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 0   # 3 partitions per key block
     assert Plan(a=3, b=3, seq_total=9 * 256, **kw).query(B.Q_BWD_PAIRED) == 1
+
+
+def test_goo_executor_volumes():
+    """The bytes the executor's communication stand-ins move for one Q group are a x the per-GPU closed form
+    2(a+b-2) N d / n, whatever the chunking; its partial workspace holds k_kv slots per Q partition."""
+    for k_q, k_kv in ((1, 1), (2, 2), (4, 2)):
+        p = Plan(a=4, b=2, batch=1, seq_total=8 * 1024, heads_q=8, heads_kv=8, head_dim=128, order=1, k_q=k_q, k_kv=k_kv)
+        assert p.query(B.Q_GOO_COMM_BYTES) == 4 * p.query(B.Q_MESH_COMM_BYTES_FWD)
+        assert p.query(B.Q_GOO_PARTIAL_O_BYTES) == k_kv * p.query(B.Q_PARTIAL_O_BYTES)
+        assert p.query(B.Q_GOO_PARTIAL_LSE_BYTES) == k_kv * p.query(B.Q_PARTIAL_LSE_BYTES)
