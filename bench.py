@@ -43,6 +43,9 @@ def parse_args():
     ap.add_argument("--workload", default="C5", help="C1..C5 (BASELINE.json configs[0..4]); default: the 1M-token causal config")
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="target duration of the oracle sample")
     ap.add_argument("--usp-lanes", type=int, default=1, help="Mesh-USP lanes U (PAPER.md L372-389): the partial workspace shrinks by U")
+    ap.add_argument("--goo-executor", type=int, default=-1, metavar="R",
+                    help="separate mode (not the driver's bench line): time the GOO executor (mesh_attn_forward_goo) on --workload with every "
+                         "communication stand-in copied R times, overlapped vs serialised, against the fused forward")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -434,9 +437,66 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+def run_goo_executor(args):
+    """the forward step list executed task by task.  Prints one JSON line of its own."""
+    import torch
+
+    import __graft_entry__ as entry
+    import contextlib
+    with contextlib.redirect_stdout(sys.stderr):
+        entry.build()
+    from paper_2512_20968_b200 import Buffers, plan_for
+    from paper_2512_20968_b200 import binding as B
+    from paper_2512_20968_b200 import workloads as W
+
+    torch.cuda.set_device(0)
+    w = W.CONFIGS[args.workload]
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    plan = plan_for(w)
+    buf = Buffers(plan, w, backward=False)
+    f32 = dict(dtype=torch.float32, device="cuda")
+    part_O = torch.empty(plan.query(B.Q_GOO_PARTIAL_O_BYTES) * w.a // 4, **f32)
+    part_lse = torch.empty(plan.query(B.Q_GOO_PARTIAL_LSE_BYTES) * w.a // 4, **f32)
+    comm_ws = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def timed(fn):
+        best = []
+        for it in range(args.warmup + args.steps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            if it >= args.warmup:
+                best.append(e0.elapsed_time(e1))
+        return statistics.median(best)
+
+    R = args.goo_executor
+    goo = lambda rep, ov: [plan.forward_goo(r, inp["q"], inp["k"], inp["v"], buf.O, buf.lse, part_O, part_lse, comm_ws=comm_ws,
+                                            comm_repeat=rep, overlap=ov) for r in range(w.b)]
+    t_fused = timed(lambda: plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse))
+    t_compute = timed(lambda: goo(0, True))
+    t_overlap = timed(lambda: goo(R, True))
+    t_serial = timed(lambda: goo(R, False))
+    makespan, serial, exposed = plan.timeline()
+    steps = plan.steps()
+    line = {
+        "mode": "goo_executor", "config": workload_config(w), "comm_repeat": R,
+        "comm_bytes_per_q_group": plan.query(B.Q_GOO_COMM_BYTES), "steps": int(steps[:, 0].max()) + 1 if len(steps) else 0,
+        "compute_tasks_per_q_group": w.k_q * w.k_kv,
+        "ms": {"fused_forward": t_fused, "executor_no_comm": t_compute, "executor_overlapped": t_overlap, "executor_serialised": t_serial},
+        "exposed_comm_ms": {"overlapped": t_overlap - t_compute, "serialised": t_serial - t_compute},
+        "model_cost_units": {"makespan": makespan, "serial": serial, "exposed_comm": exposed},
+    }
+    print(json.dumps(line), flush=True)
+
+
 def main():
     args = parse_args()
-    if args.impl == "reference":
+    if args.goo_executor >= 0:
+        run_goo_executor(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)
