@@ -219,6 +219,7 @@ def workload_config(w, note=""):
         "heads_kv": w.heads_kv, "head_dim": w.head_dim, "seq_layout": w.seq_layout, "kvr": w.kvr, "order": w.order,
         "k_q": w.k_q, "k_kv": w.k_kv, "passes": "fwd+merge+bwd" if w.backward else "fwd+merge",
         "inputs": "bf16 iid N(0,1)" + (" with 4 of 128 Q/K channels x8" if w.outlier else ""),
+        "precision": "split hi+lo P/dS operands (the mode parity-tested on outlier scores)" if w.outlier else "single bf16 operands",
         "l2": "inputs larger than L2 (no flush needed)" if w.seq_total * w.heads_q * w.head_dim * 2 > (126 << 20) else "L2-resident (report only)",
     }
     if note:

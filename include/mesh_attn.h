@@ -236,6 +236,34 @@ int mesh_attn_forward_goo(const mesh_attn_plan* plan, int32_t q_group, const voi
                           float* O, float* lse, float* partial_O, float* partial_lse,
                           void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap, void* stream);
 
+/* ---- per-rank calls (Alg.2, Alg.3) ----------------------
+ * The compute steps of ONE GPU g of a real n-GPU job, on tensors that hold only what that GPU has after its
+ * all-gathers (device pointers, caller-owned; usp_lanes == 1, partial_mode == 0, else EUNSUPPORTED).  The
+ * collectives themselves are the caller's (paper_2512_20968_b200/distributed.py issues them with torch.distributed);
+ * the arithmetic is that of mesh_attn_tile_fwd / merge / bwd_preprocess / tile_bwd for simulated GPU g — same
+ * kernels and work lists, only the row addressing differs: partition slot k of a query-shaped local tensor is the
+ * k-th entry of I_g^Q (partition (g/a)*a + k, i.e. the k-th member of g's Q group), slot t of a key-shaped one the t-th
+ * entry of I_g^KV (mesh_attn_plan_footprint order); row = slot*L + s.
+ *   Q_loc, dO_loc bf16, dQ_loc fp32  [B, a*L, Hq, D]  (tensor_layout 1: [B, Hq, a*L, D])
+ *   K_loc, V_loc  bf16, dK_loc, dV_loc fp32  [B, b*L, Hkv, D]
+ *   partial_O fp32 [a][B][L][Hq][D], partial_lse fp32 [a][B][Hq][L]: slot k is the partial for Q partition
+ *     (g/a)*a + k, to be delivered to that rank (RS-O, Alg.2 l.6)
+ *   rank_merge: partial_*_recv are the `a` partials of the rank's OWN Q partition, slot k from the k-th member of
+ *     its Q group; O_own fp32 [B, L, Hq, D], lse_own fp32 [B][Hq][L]
+ *   rank_bwd_preprocess: ws_own fp32 [2][B][Hq][L] (delta, exponent offset) of the own partition
+ *   rank_bwd: ws_loc fp32 [2][B][Hq][a*L]: the ws_own of the Q group's members, member k at rows k*L.. (gathering
+ *     delta and the offset instead of O saves the all-gather of O that Alg.3 l.1 lists);
+ *     dQ_loc, dK_loc, dV_loc are ACCUMULATED into (caller zeroes) and hold this GPU's contribution for every
+ *     partition of its footprint: the reduce-scatters of Alg.3 l.6-7 sum them over the Q group / KV group. */
+int mesh_attn_rank_fwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc,
+                       float* partial_O, float* partial_lse, void* stream);
+int mesh_attn_rank_merge(const mesh_attn_plan* plan, const float* partial_O_recv, const float* partial_lse_recv,
+                         float* O_own, float* lse_own, void* stream);
+int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* plan, const float* O_own, const void* dO_own, const float* lse_own,
+                                  float* ws_own, void* stream);
+int mesh_attn_rank_bwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc,
+                       const void* dO_loc, const float* ws_loc, float* dQ_loc, float* dK_loc, float* dV_loc, void* stream);
+
 /* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
 int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
                        const float* O, const void* dO, const float* lse, float* bwd_ws,

@@ -66,6 +66,10 @@ lib.mesh_attn_tile_bwd.argtypes = [_P, C.c_int32, C.c_int32] + [_P] * 9
 lib.mesh_attn_forward.argtypes = [_P] * 9
 lib.mesh_attn_forward_goo.argtypes = [_P, C.c_int32] + [_P] * 8 + [C.c_int64, C.c_int32, C.c_int32, _P]
 lib.mesh_attn_backward.argtypes = [_P] * 12
+lib.mesh_attn_rank_fwd.argtypes = [_P, C.c_int32] + [_P] * 6
+lib.mesh_attn_rank_merge.argtypes = [_P] * 6
+lib.mesh_attn_rank_bwd_preprocess.argtypes = [_P] * 6
+lib.mesh_attn_rank_bwd.argtypes = [_P, C.c_int32] + [_P] * 9
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
 lib.mesh_attn_launch_count.restype = C.c_int64
 lib.mesh_attn_profile_enable.argtypes = [C.c_int32, C.c_int32]
@@ -79,6 +83,7 @@ EXPORTED = [
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
+    "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
 ]
 K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
 
@@ -208,6 +213,20 @@ class Plan:
     def backward(self, Q, K, V, O, dO, lse, bwd_ws, dQ, dK, dV, stream=None):
         _check(lib.mesh_attn_backward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(lse), _ptr(bwd_ws),
                                       _ptr(dQ), _ptr(dK), _ptr(dV), _stream(stream)))
+
+    # ---- per-rank calls (one GPU of a real n-GPU job; tensors hold the rank's gathered partitions only) ----
+    def rank_fwd(self, g, Q_loc, K_loc, V_loc, partial_O, partial_lse, stream=None):
+        _check(lib.mesh_attn_rank_fwd(self._h, g, _ptr(Q_loc), _ptr(K_loc), _ptr(V_loc), _ptr(partial_O), _ptr(partial_lse), _stream(stream)))
+
+    def rank_merge(self, partial_O_recv, partial_lse_recv, O_own, lse_own, stream=None):
+        _check(lib.mesh_attn_rank_merge(self._h, _ptr(partial_O_recv), _ptr(partial_lse_recv), _ptr(O_own), _ptr(lse_own), _stream(stream)))
+
+    def rank_bwd_preprocess(self, O_own, dO_own, lse_own, ws_own, stream=None):
+        _check(lib.mesh_attn_rank_bwd_preprocess(self._h, _ptr(O_own), _ptr(dO_own), _ptr(lse_own), _ptr(ws_own), _stream(stream)))
+
+    def rank_bwd(self, g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc, stream=None):
+        _check(lib.mesh_attn_rank_bwd(self._h, g, _ptr(Q_loc), _ptr(K_loc), _ptr(V_loc), _ptr(dO_loc), _ptr(ws_loc),
+                                      _ptr(dQ_loc), _ptr(dK_loc), _ptr(dV_loc), _stream(stream)))
 
     def step_host(self, stream=None, **buffers):
         io = HostIO()

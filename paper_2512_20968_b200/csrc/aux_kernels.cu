@@ -59,7 +59,7 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
             const float x = w_smem[(r * Hq + h) * m + k];
             w_smem[(r * Hq + h) * m + k] = (x == -INFINITY) ? 0.f : __expf(x - lse);
         }
-        p.lse[(size_t)bt * p.lse_stride_b + (size_t)h * ((size_t)gm.n * gm.L) + (size_t)u * gm.L + s0 + r] = lse;
+        p.lse[(size_t)bt * p.lse_stride_b + (size_t)h * (size_t)gm.rows_q + (size_t)u * gm.L + s0 + r] = lse;
     }
     __syncthreads();
 
@@ -101,7 +101,7 @@ template <int D>
 __global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
 {
     const Geom& gm = p.gm;
-    const long long N = (long long)gm.n * gm.L;
+    const long long N = gm.rows_q;
     const long long wid = (long long)blockIdx.x * 8 + (threadIdx.x >> 5);
     const int lane = threadIdx.x & 31;
     if (wid >= (long long)gm.batch * N * gm.heads_q) return;
@@ -157,7 +157,7 @@ int launch_merge(const MergeParams& p, cudaStream_t stream)
 int launch_delta(const DeltaParams& p, cudaStream_t stream)
 {
     const Geom& gm = p.gm;
-    const long long warps = (long long)gm.batch * gm.n * gm.L * gm.heads_q;
+    const long long warps = (long long)gm.batch * gm.rows_q * gm.heads_q;
     const unsigned grid = (unsigned)((warps + 7) / 8);
     if (gm.head_dim == 128) delta_kernel<128><<<grid, 256, 0, stream>>>(p);
     else delta_kernel<64><<<grid, 256, 0, stream>>>(p);

@@ -30,9 +30,9 @@ int cuda_fail(const char* what, int err)
 }
 
 struct Strides { long long b, row, h; };   // element strides of a [B,N,H,D] / [B,H,N,D] tensor with H heads in all
-Strides strides_of(const mesh_attn_plan* p, int H)
+Strides strides_of(const mesh_attn_plan* p, int H, long long rows = 0)
 {
-    const long long N = (long long)p->geom.n * p->geom.L, D = p->geom.head_dim;
+    const long long N = rows ? rows : (long long)p->geom.n * p->geom.L, D = p->geom.head_dim;
     if (p->desc.tensor_layout == 0) return {N * H * D, (long long)H * D, D};
     return {N * H * D, D, N * D};
 }
@@ -56,10 +56,11 @@ template <class T> T* head_slice(T* base, long long h0, const Strides& s, int el
 }
 
 // bf16 tensor map of the lane's head slice: H_lane heads starting at h0 of a tensor with H_all heads
-bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0, int box_rows = kBlock)
+bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0, int box_rows = kBlock,
+              long long rows = 0)
 {
-    const Strides s = strides_of(p, H_all);
-    const uint64_t N = (uint64_t)p->geom.n * p->geom.L;
+    const Strides s = strides_of(p, H_all, rows);
+    const uint64_t N = rows ? (uint64_t)rows : (uint64_t)p->geom.n * p->geom.L;
     return make_tmap_bf16_4d(m, head_slice(base, h0, s, 2), p->geom.head_dim, H_lane, N, p->geom.batch, s.h * 2, s.row * 2, s.b * 2, box_rows);
 }
 
@@ -165,8 +166,10 @@ extern "C" {
 
 // tile_fwd over an item list (the plan's fused list, or one compute task of the GOO executor)
 static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int items_per_gpu, int slots_per_gpu, int32_t g_first, int32_t g_count,
-                           const void* Q, const void* K, const void* V, float* partial_O, float* partial_lse, void* stream, const char* who)
+                           const void* Q, const void* K, const void* V, float* partial_O, float* partial_lse, void* stream, const char* who,
+                           bool local = false)
 {
+    const long long rq = local ? (long long)p->geom.a * p->geom.L : 0, rk = local ? (long long)p->geom.b * p->geom.L : 0;
     if (int rc = check_device(p, who)) return rc;
     if (!Q || !K || !V || !partial_O || !partial_lse) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null pointer");
     Lane ln;
@@ -174,12 +177,14 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
     if ((long long)g_count * (long long)items_per_gpu >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, std::string(who) + ": too many work items in one call");
     if (items_per_gpu == 0) return MESH_ATTN_OK;
     CUtensorMap tmQ, tmK, tmV;
-    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
-        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0))
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, kBlock, rq) ||
+        !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, rk) ||
+        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, rk))
         return fail(MESH_ATTN_ECUDA, std::string(who) + ": cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     FwdParams fp;
     fp.gm = p->geom;
     fp.gm.slots_per_gpu = slots_per_gpu;
+    if (local) { fp.gm.local = 1; fp.gm.rows_q = (int32_t)rq; fp.gm.rows_kv = (int32_t)rk; }
     fp.items = items;
     fp.segs = p->d_fwd_segs;
     fp.seglists = p->d_fwd_seglists;
@@ -262,8 +267,8 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
     return MESH_ATTN_OK;
 }
 
-int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
-                       const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
+static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
+                      const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream, bool local)
 {
     if (int rc = check_device(p, "tile_bwd")) return rc;
     if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
@@ -271,21 +276,24 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds (or crossing a USP lane)");
     if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
     CUtensorMap tmQ, tmK, tmV, tmdO, tmdQ;
-    const Strides sdq = strides_of(p, p->desc.heads_q), sdk = strides_of(p, p->desc.heads_kv);
-    const long long N = (long long)p->geom.n * p->geom.L;
+    const long long N = local ? (long long)p->geom.a * p->geom.L : (long long)p->geom.n * p->geom.L;     // query-shaped rows
+    const long long Nk = local ? (long long)p->geom.b * p->geom.L : (long long)p->geom.n * p->geom.L;   // key-shaped rows
+    const Strides sdq = strides_of(p, p->desc.heads_q, N), sdk = strides_of(p, p->desc.heads_kv, Nk);
     dQ = head_slice(dQ, ln.hq0, sdq, 4);
     dK = head_slice(dK, ln.hk0, sdk, 4);
     dV = head_slice(dV, ln.hk0, sdk, 4);
     // paired items (2-CTA clusters): each CTA loads 64-row halves of the Q / dO tiles and multicasts them
     const bool pair = p->bwd_pairable && ((long long)g_count * (long long)p->bwd_items.size()) >= 2 && !p->no_pair;
     const int qbox = pair ? kBlock / 2 : kBlock;
-    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox) || !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) ||
-        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0) || !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox) ||
-        !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)p->geom.n * p->geom.L, p->geom.batch, sdq.h * 4, sdq.row * 4,
-                          sdq.b * 4, 16))
+    if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox, N) ||
+        !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, Nk) ||
+        !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, Nk) ||
+        !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox, N) ||
+        !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)N, p->geom.batch, sdq.h * 4, sdq.row * 4, sdq.b * 4, 16))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     BwdParams bp;
     bp.gm = p->geom;
+    if (local) { bp.gm.local = 1; bp.gm.rows_q = (int32_t)N; bp.gm.rows_kv = (int32_t)Nk; }
     bp.items = p->d_bwd_items;
     bp.segs = p->d_bwd_segs;
     bp.seglists = p->d_bwd_seglists;
@@ -306,6 +314,86 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
     if (e) return cuda_fail("tile_bwd launch", e);
     g_launches.fetch_add(1);
     return MESH_ATTN_OK;
+}
+
+int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
+                       const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
+{
+    return launch_bwd(p, g_first, g_count, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream, false);
+}
+
+// ---- per-rank calls: the tensors hold only the partitions ONE GPU has after its all-gathers ----
+static int check_rank(const mesh_attn_plan* p, int32_t g, const char* who)
+{
+    if (int rc = check_device(p, who)) return rc;
+    if (lanes_of(p) != 1 || p->desc.partial_mode != 0)
+        return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": per-rank calls need usp_lanes == 1 and partial_mode == 0");
+    if (g < 0 || g >= p->geom.n) return fail(MESH_ATTN_EINVAL, std::string(who) + ": rank g out of range");
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_rank_fwd(const mesh_attn_plan* p, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc, float* partial_O,
+                       float* partial_lse, void* stream)
+{
+    if (int rc = check_rank(p, g, "rank_fwd")) return rc;
+    return launch_fwd_list(p, p->d_fwd_items, (int)p->fwd_items.size(), p->geom.slots_per_gpu, g, 1, Q_loc, K_loc, V_loc, partial_O, partial_lse, stream,
+                           "rank_fwd", true);
+}
+
+int mesh_attn_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, const float* partial_lse_recv, float* O_own, float* lse_own,
+                         void* stream)
+{
+    if (int rc = check_rank(p, 0, "rank_merge")) return rc;
+    if (!partial_O_recv || !partial_lse_recv || !O_own || !lse_own) return fail(MESH_ATTN_EINVAL, "rank_merge: null pointer");
+    const Geom& g0 = p->geom;
+    MergeParams mp;
+    mp.gm = g0;
+    mp.gm.a = 1;                      // one Q partition (the rank's own) ...
+    mp.gm.rows_q = g0.L;              // ... in tensors of L rows
+    mp.gm.slots_per_gpu = g0.a;
+    mp.q_group = 0;
+    mp.per = g0.a;                    // slot(k) = k: the partial received from the k-th member of the Q group
+    mp.m = g0.a;
+    int rows = 8;
+    while (rows > 1 && ((size_t)rows * g0.heads_q * mp.m * 4 > 64 * 1024 || g0.L % rows)) rows >>= 1;
+    if ((size_t)rows * g0.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, "rank_merge: heads_q * partial count too large");
+    mp.rows_per_block = rows;
+    mp.partial_O = partial_O_recv;
+    mp.partial_lse = partial_lse_recv;
+    const Strides s = strides_of(p, g0.heads_q, g0.L);
+    mp.O = O_own;
+    mp.lse = lse_own;
+    mp.lse_stride_b = (long long)g0.heads_q * g0.L;
+    mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
+    ProfScope prof(MESH_ATTN_K_MERGE, (cudaStream_t)stream);
+    const int e = launch_merge(mp, (cudaStream_t)stream);
+    if (e) return cuda_fail("rank_merge launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* p, const float* O_own, const void* dO_own, const float* lse_own, float* ws_own, void* stream)
+{
+    if (int rc = check_rank(p, 0, "rank_bwd_preprocess")) return rc;
+    if (!O_own || !dO_own || !lse_own || !ws_own) return fail(MESH_ATTN_EINVAL, "rank_bwd_preprocess: null pointer");
+    DeltaParams dp;
+    dp.gm = p->geom;
+    dp.gm.rows_q = p->geom.L;
+    dp.O = O_own; dp.dO = dO_own; dp.lse = lse_own; dp.ws = ws_own;
+    const Strides s = strides_of(p, p->geom.heads_q, p->geom.L);
+    dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
+    ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
+    const int e = launch_delta(dp, (cudaStream_t)stream);
+    if (e) return cuda_fail("rank_bwd_preprocess launch", e);
+    g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
+int mesh_attn_rank_bwd(const mesh_attn_plan* p, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc, const void* dO_loc,
+                       const float* ws_loc, float* dQ_loc, float* dK_loc, float* dV_loc, void* stream)
+{
+    if (int rc = check_rank(p, g, "rank_bwd")) return rc;
+    return launch_bwd(p, g, 1, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc, stream, true);
 }
 
 int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, float* O, float* lse, float* partial_O,

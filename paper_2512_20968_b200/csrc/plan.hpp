@@ -63,6 +63,11 @@ struct Geom {
     int32_t batch, heads_q, heads_kv, head_dim, group;  // group = heads_q / heads_kv
     int32_t causal, kvr, striped;
     int32_t slots_per_gpu;
+    // rows of the query-shaped (Q, O, dO, dQ, lse, delta) and key-shaped (K, V, dK, dV) tensors a call receives:
+    // n*L for the simulated-GPU calls; a*L and b*L for the per-rank calls (mesh_attn_rank_*), whose tensors hold only
+    // the gathered partitions of ONE GPU, slot k = k-th entry of I_g^Q / I_g^KV
+    int32_t rows_q, rows_kv;
+    int32_t local;      // 1: per-rank tensors (row of partition = slot*L + s), 0: all n partitions (row = p*L + s)
     float scale;        // softmax scale
     float scale_log2;   // scale * log2(e)
 };
@@ -73,6 +78,10 @@ inline MA_HD int kv_partition(const Geom& gm, int g, int kv_local)
     const int c = g % gm.a;
     return gm.kvr ? c + kv_local * gm.a : c * gm.b + kv_local;
 }
+
+// Partition index that addresses the rows of Q partition u / KV partition v in the tensors of the call
+inline MA_HD int q_row_part(const Geom& gm, int u, int u_local) { return gm.local ? u_local : u; }
+inline MA_HD int kv_row_part(const Geom& gm, int v, int kv_local) { return gm.local ? kv_local : v; }
 
 // Causal offset of pair (Q_u, KV_v): key local row t is visible to query local row s iff
 // t <= s + off.  Contiguous: pos = p*L+s  ->  off = (u-v)*L.  Striped: pos = s*n+p  ->

@@ -327,6 +327,8 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     gm.group = d->heads_q / d->heads_kv;
     gm.causal = d->causal; gm.kvr = d->kvr; gm.striped = d->seq_layout;
     gm.slots_per_gpu = d->partial_mode == 1 ? d->a * d->b : d->a;
+    gm.rows_q = gm.rows_kv = d->seq_total;   // the simulated-GPU calls see all n partitions; mesh_attn_rank_* override
+    gm.local = 0;
     gm.scale = d->softmax_scale > 0.f ? d->softmax_scale : 1.0f / std::sqrt((float)d->head_dim);
     gm.scale_log2 = (float)((double)gm.scale * 1.4426950408889634);
     p->k_q = k_q; p->k_kv = k_kv;

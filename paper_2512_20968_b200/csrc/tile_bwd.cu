@@ -91,21 +91,22 @@ struct QWalk {
     const Geom& gm;
     const Seg* segs;
     int nseg, g, v, t0, head_kv;
-    int si = -1, hh = 0, s_lo = 0, s_hi = 0, u = 0, off = 0;
+    int si = -1, hh = 0, s_lo = 0, s_hi = 0, u = 0, urow = 0, off = 0;
     __device__ __forceinline__ QWalk(const Geom& gm_, const Seg* segs_, int nseg_, int g_, int v_, int t0_, int head_kv_)
         : gm(gm_), segs(segs_), nseg(nseg_), g(g_), v(v_), t0(t0_), head_kv(head_kv_) {}
-    // next run: Q partition u, query head h, first local query row s0, number of blocks n >= 1, causal offset off
+    // next run: row-addressing index of Q partition u (plan.hpp q_row_part), query head h, first local query row s0, number of blocks n >= 1, causal offset off
     __device__ bool next_run(int& u_out, int& h_out, int& s0_out, int& n_out, int& off_out)
     {
         while (true) {
             if (si >= 0 && s_lo < s_hi && hh < gm.group) {
-                u_out = u; h_out = head_kv * gm.group + hh; s0_out = s_lo; n_out = (s_hi - s_lo) / kBlock; off_out = off;
+                u_out = urow; h_out = head_kv * gm.group + hh; s0_out = s_lo; n_out = (s_hi - s_lo) / kBlock; off_out = off;
                 ++hh;
                 return true;
             }
             if (++si >= nseg) return false;
             const Seg sg = segs[si];
             u = (g / gm.a) * gm.a + sg.part_local;
+            urow = q_row_part(gm, u, sg.part_local);
             hh = 0;
             s_lo = sg.begin;
             s_hi = sg.end;
@@ -140,7 +141,7 @@ struct QStep {
 
 struct BwdItemCtx {
     BwdItem it;
-    int g_local, g, v, nseg;
+    int g_local, g, v, vrow, nseg;
     const Seg* segs;
 };
 
@@ -151,6 +152,7 @@ __device__ __forceinline__ BwdItemCtx load_bwd_item(const BwdParams& p, int idx)
     c.it = p.items[idx - c.g_local * p.items_per_gpu];
     c.g = p.g_first + c.g_local;
     c.v = kv_partition(p.gm, c.g, c.it.kv_local);
+    c.vrow = kv_row_part(p.gm, c.v, c.it.kv_local);
     const SegList sl = p.seglists[c.it.seglist];
     c.segs = p.segs + sl.offset;
     c.nseg = sl.count;
@@ -229,7 +231,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const Geom& gm = p.gm;
     const int total_items = p.items_per_gpu * p.g_count;
-    const long long N = (long long)gm.n * gm.L;
+    const long long N = gm.rows_q;
     constexpr int kCompute = 2 * kBlock;                // threads of the two compute groups
 
     if (threadIdx.x == 0) {
@@ -277,8 +279,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         kv_phase ^= 1;
                         mbar_expect_tx(kv_full, 2 * Cfg::kTileBytes);
                         for (int bx = 0; bx < Cfg::kBoxes; ++bx) {
-                            tma_load_4d(sK + bx * (kBlock * 128), &tmK, kv_full, bx * 64, c.it.head_kv, c.v * gm.L + c.it.t0, c.it.batch, kEvictFirst);
-                            tma_load_4d(sV + bx * (kBlock * 128), &tmV, kv_full, bx * 64, c.it.head_kv, c.v * gm.L + c.it.t0, c.it.batch, kEvictFirst);
+                            tma_load_4d(sK + bx * (kBlock * 128), &tmK, kv_full, bx * 64, c.it.head_kv, c.vrow * gm.L + c.it.t0, c.it.batch, kEvictFirst);
+                            tma_load_4d(sV + bx * (kBlock * 128), &tmV, kv_full, bx * 64, c.it.head_kv, c.vrow * gm.L + c.it.t0, c.it.batch, kEvictFirst);
                         }
                     }
                     mbar_wait(&qd_empty[stage], ring_phase ^ 1);
@@ -574,7 +576,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             mbar_wait(dkv_full, dkv_ph);
             dkv_ph ^= 1;
             tc_fence_after();
-            float* grow = (wg == 0 ? p.dK : p.dV) + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.v * gm.L + c.it.t0 + row) * p.k_stride_row +
+            float* grow = (wg == 0 ? p.dK : p.dV) + (size_t)c.it.batch * p.k_stride_b + ((size_t)c.vrow * gm.L + c.it.t0 + row) * p.k_stride_row +
                           (size_t)c.it.head_kv * p.k_stride_h;
             drain_rows<D>(tmem + lane_base + (wg == 0 ? Cfg::kColDK : Cfg::kColDV), grow, wg == 0 ? 1.0f : 1.0f / gm.scale, gm.head_dim);
             tc_fence_before();

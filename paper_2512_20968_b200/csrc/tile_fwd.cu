@@ -63,12 +63,13 @@ template <int D> struct FwdCfg {
 
 // The 128-key KV blocks of a work item in plan order: segment by segment (KV partition v, local key rows
 // [begin, end) clipped to the rows visible to the item's last query row), block by block.  Every role runs the same
-// nest; f(v, t0, off): KV partition, first local key row, causal offset (key t visible to row s iff t <= s + off).
-struct KvRange { int v, off, t_lo, t_hi; };
+// nest; f(vrow, t0, off): row-addressing index of the KV partition, first local key row, causal offset (key t visible to row s iff t <= s + off).
+struct KvRange { int v, vrow, off, t_lo, t_hi; };   // vrow: partition index that addresses v's rows (plan.hpp kv_row_part)
 __device__ __forceinline__ KvRange kv_range(const Geom& gm, const Seg sg, int g, int u, int q_last)
 {
     KvRange r;
     r.v = kv_partition(gm, g, sg.part_local);
+    r.vrow = kv_row_part(gm, r.v, sg.part_local);
     r.t_lo = sg.begin;
     r.t_hi = sg.end;
     r.off = 0x20000000;
@@ -84,7 +85,7 @@ __device__ __forceinline__ void for_each_kv_block(const Geom& gm, const Seg* seg
 {
     for (int si = 0; si < nseg; ++si) {
         const KvRange r = kv_range(gm, segs[si], g, u, q_last);
-        for (int t0 = r.t_lo; t0 < r.t_hi; t0 += kBlock) f(r.v, t0, r.off);
+        for (int t0 = r.t_lo; t0 < r.t_hi; t0 += kBlock) f(r.vrow, t0, r.off);
     }
 }
 __device__ __forceinline__ int count_kv_blocks(const Geom& gm, const Seg* segs, int nseg, int g, int u, int q_last)
@@ -173,7 +174,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         for (int t = 0; t < c.nt; ++t)
                             for (int bx = 0; bx < Cfg::kBoxes; ++bx)
                                 tma_load_4d(sQ + t * Cfg::kTileBytes + bx * (kBlock * 128), &tmQ, q_full, bx * 64, c.it.head,
-                                            c.u * gm.L + c.it.q0 + t * kBlock, c.it.batch, kEvictFirst);
+                                            q_row_part(gm, c.u, c.it.u_local) * gm.L + c.it.q0 + t * kBlock, c.it.batch, kEvictFirst);
                     }
                     const int hk = c.it.head / gm.group;
                     for (int kv = 0; kv < 2; ++kv) {       // K block then V block through the ring

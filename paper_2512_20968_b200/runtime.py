@@ -13,6 +13,7 @@ def plan_for(w: Workload, **overrides) -> Plan:
         a=w.a, b=w.b, n=w.n, batch=w.batch, seq_total=w.seq_total, heads_q=w.heads_q, heads_kv=w.heads_kv, head_dim=w.head_dim,
         causal=int(w.causal), kvr=int(w.kvr), seq_layout=int(w.seq_layout == "striped"), order=int(w.order == "greedy"),
         k_q=w.k_q, k_kv=w.k_kv,
+        precision=1 if w.outlier else 0,   # outlier scores (BASELINE.json configs[2]) need hi+lo P / dS operands for the gradient bar
     )
     kw.update(overrides)
     return Plan(**kw)

@@ -1,7 +1,8 @@
 """N > 1 path on the CPU (gloo, world_size 2).  The hot path does not shard (BASELINE.json: no sharding, no
 collectives; replicas only), so the multi-rank logic is bench.py's bookkeeping: every rank
 builds the same plan, the job time is the max over ranks, the job value is the sum of the ranks' work over that time,
-and the oracle arm runs on rank 0 only."""
+and the oracle arm runs on rank 0 only.  The method's own sharding (paper_2512_20968_b200/distributed.py)
+is driven here with stand-in compute: the collectives, groups and slot order of Alg.2 / Alg.3 on 2 and 4 gloo ranks."""
 import json
 import os
 import socket
@@ -71,3 +72,66 @@ def test_reference_arm_runs_on_rank0_only():
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
     assert outs[1] == ""
+
+
+def _mesh_worker(rank: int, world: int, port: int, a: int, b: int, causal: bool, heads_q: int, heads_kv: int, out_dir: str):
+    sys.path.insert(0, str(ROOT))
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port), RANK=str(rank), WORLD_SIZE=str(world))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    torch.set_num_threads(2)
+    from paper_2512_20968_b200 import plan_for
+    from paper_2512_20968_b200 import workloads as W
+    from paper_2512_20968_b200.distributed import MeshAttnRank
+    from tests.rank_standin import StandInKernels
+
+    L, D = 128, 64
+    w = W.Workload("mesh", 7, causal, a, b, 1, L * a * b, heads_q, heads_kv, D, seq_layout="striped" if causal else "contiguous")
+    plan = plan_for(w)
+    inp = W.make_inputs(w, "cpu")                                # same seed on every rank
+    own = {k: v[:, rank * L:(rank + 1) * L].contiguous() for k, v in inp.items()}
+    me = MeshAttnRank(plan, kernels=StandInKernels(plan, w.seq_layout))
+    O, lse = me.forward(own["q"], own["k"], own["v"])
+    dQ, dK, dV = me.backward(own["do"])
+    torch.save({"O": O, "lse": lse, "dQ": dQ, "dK": dK, "dV": dV}, Path(out_dir, f"rank{rank}.pt"))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+def _check_mesh(tmp_path, a, b, causal, heads_q, heads_kv):
+    from paper_2512_20968_b200 import workloads as W
+
+    world, L, D = a * b, 128, 64
+    mp.spawn(_mesh_worker, args=(world, _free_port(), a, b, causal, heads_q, heads_kv, str(tmp_path)), nprocs=world, join=True)
+    res = [torch.load(tmp_path / f"rank{r}.pt") for r in range(world)]
+    got = {k: torch.cat([r[k] for r in res], dim=2 if k == "lse" else 1).double() for k in res[0]}
+    # full attention and its gradients from the definition (torch fp64 autograd), global token order via the position map
+    w = W.Workload("mesh", 7, causal, a, b, 1, L * world, heads_q, heads_kv, D, seq_layout="striped" if causal else "contiguous")
+    inp = {k: v.double() for k, v in W.make_inputs(w, "cpu").items()}
+    q, k, v = (inp[x].clone().requires_grad_(True) for x in ("q", "k", "v"))
+    p, s = torch.arange(w.seq_total) // L, torch.arange(w.seq_total) % L
+    pos = s * world + p if causal else p * L + s
+    grp = heads_q // heads_kv
+    S = torch.einsum("bshd,bthd->bhst", q, k.repeat_interleave(grp, dim=2)) * w.scale
+    if causal:
+        S = S.masked_fill(pos[None, :] > pos[:, None], float("-inf"))
+    O = torch.einsum("bhst,bthd->bshd", torch.softmax(S, -1), v.repeat_interleave(grp, dim=2))
+    O.backward(inp["do"])
+    ref = {"O": O.detach(), "lse": torch.logsumexp(S, -1).detach(), "dQ": q.grad, "dK": k.grad, "dV": v.grad}
+    for name in ref:
+        err = (got[name] - ref[name]).abs().max().item()
+        assert err < 2e-4, f"{name}: max abs error {err:.3e} (fp32 buffers between the steps)"
+
+
+def test_mesh_ranks_world2_q_group(tmp_path):
+    """a = 2, b = 1: one Q group of two ranks (AG-Q, RS-O, RS-dQ carry data; the KV groups are singletons)."""
+    _check_mesh(tmp_path, 2, 1, True, 2, 2)
+
+
+def test_mesh_ranks_world2_kv_group(tmp_path):
+    """a = 1, b = 2: one KV group of two ranks (AG-KV, RS-dKV); GQA 4 query heads on 2 KV heads."""
+    _check_mesh(tmp_path, 1, 2, False, 4, 2)
+
+
+def test_mesh_ranks_world4(tmp_path):
+    """2 x 2 mesh, causal, striped: both group kinds, KV partition rotation (KV group of rank g = {g mod a + t*a})."""
+    _check_mesh(tmp_path, 2, 2, True, 2, 1)
