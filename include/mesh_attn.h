@@ -259,6 +259,15 @@ int mesh_attn_rank_fwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc,
                        float* partial_O, float* partial_lse, void* stream);
 int mesh_attn_rank_merge(const mesh_attn_plan* plan, const float* partial_O_recv, const float* partial_lse_recv,
                          float* O_own, float* lse_own, void* stream);
+/* RS-O of Alg.2 l.6 FUSED into its reducer over peer memory: the same merge, but partial k is read straight from
+ * where the k-th member of the rank's Q group wrote it -- peer_partial_O[k] fp32 [B][L][Hq][D] and peer_partial_lse[k]
+ * fp32 [B][Hq][L] are DEVICE-ACCESSIBLE addresses in this process (the member's partial slot for this rank's partition:
+ * its own memory for k = own index, a peer GPU's memory mapped through CUDA IPC / NVLink peer access otherwise), given as
+ * two HOST arrays of `a` pointers (copied into the launch; a <= 16).  The loads of the merge are then the transfer: no
+ * all-to-all, no receive buffer, and the exchange overlaps the arithmetic load by load.  The caller orders the launch after
+ * the members' rank_fwd (an event or a barrier across the group).  Bit-identical to rank_merge on the same partials. */
+int mesh_attn_rank_merge_peers(const mesh_attn_plan* plan, const float* const* peer_partial_O, const float* const* peer_partial_lse,
+                               float* O_own, float* lse_own, void* stream);
 int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* plan, const float* O_own, const void* dO_own, const float* lse_own,
                                   float* ws_own, void* stream);
 int mesh_attn_rank_bwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc,

@@ -68,6 +68,7 @@ lib.mesh_attn_forward_goo.argtypes = [_P, C.c_int32] + [_P] * 8 + [C.c_int64, C.
 lib.mesh_attn_backward.argtypes = [_P] * 12
 lib.mesh_attn_rank_fwd.argtypes = [_P, C.c_int32] + [_P] * 6
 lib.mesh_attn_rank_merge.argtypes = [_P] * 6
+lib.mesh_attn_rank_merge_peers.argtypes = [_P, C.POINTER(_P), C.POINTER(_P), _P, _P, _P]
 lib.mesh_attn_rank_bwd_preprocess.argtypes = [_P] * 6
 lib.mesh_attn_rank_bwd.argtypes = [_P, C.c_int32] + [_P] * 9
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
@@ -83,7 +84,7 @@ EXPORTED = [
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
-    "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
+    "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
 ]
 K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
 
@@ -220,6 +221,13 @@ class Plan:
 
     def rank_merge(self, partial_O_recv, partial_lse_recv, O_own, lse_own, stream=None):
         _check(lib.mesh_attn_rank_merge(self._h, _ptr(partial_O_recv), _ptr(partial_lse_recv), _ptr(O_own), _ptr(lse_own), _stream(stream)))
+
+    def rank_merge_peers(self, peer_partial_O, peer_partial_lse, O_own, lse_own, stream=None):
+        """peer_partial_O / peer_partial_lse: sequences of `a` tensors or device addresses (member k's partial for this rank's partition)"""
+        m = len(peer_partial_O)
+        po = (_P * m)(*[_ptr(t) for t in peer_partial_O])
+        pl = (_P * m)(*[_ptr(t) for t in peer_partial_lse])
+        _check(lib.mesh_attn_rank_merge_peers(self._h, po, pl, _ptr(O_own), _ptr(lse_own), _stream(stream)))
 
     def rank_bwd_preprocess(self, O_own, dO_own, lse_own, ws_own, stream=None):
         _check(lib.mesh_attn_rank_bwd_preprocess(self._h, _ptr(O_own), _ptr(dO_own), _ptr(lse_own), _ptr(ws_own), _stream(stream)))

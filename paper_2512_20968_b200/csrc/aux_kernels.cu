@@ -29,7 +29,7 @@ constexpr int kMergeUnroll = 8;
 // Q partition.  Phase 1: one thread per (row, head) turns the m LSE values into weights
 // w_k = exp(lse_k - lse*) (smem) and writes lse*.  Phase 2: every thread streams float4 columns:
 // out = sum_k w_k * partial_k.
-template <int D>
+template <int D, bool kPeers>
 __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams p)
 {
     extern __shared__ float w_smem[];            // [rows][Hq][m]
@@ -45,7 +45,8 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
         float mx = -INFINITY;
         for (int k = 0; k < m; ++k) {
             const size_t slot = (size_t)(k / p.per) * gm.slots_per_gpu + (size_t)ul * p.per + (k % p.per);
-            const float x = p.partial_lse[slot * unit_lse + ((size_t)bt * Hq + h) * gm.L + s0 + r];
+            const float* src_lse = kPeers ? p.peer_lse[k] : p.partial_lse + slot * unit_lse;
+            const float x = src_lse[((size_t)bt * Hq + h) * gm.L + s0 + r];
             w_smem[(r * Hq + h) * m + k] = x;
             mx = fmaxf(mx, x);
         }
@@ -65,7 +66,8 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
 
     constexpr int V = D / 4;                                        // float4 per (row, head)
     const int total = rows * Hq * V;
-    const float4* src = reinterpret_cast<const float4*>(p.partial_O) + ((size_t)bt * gm.L + s0) * Hq * V;
+    const size_t src_at = ((size_t)bt * gm.L + s0) * Hq * V;    // float4 index of the block's first element inside one partial
+    const float4* src = reinterpret_cast<const float4*>(p.partial_O) + src_at;
     for (int i = threadIdx.x; i < total; i += kMergeThreads) {
         const int rh = i / V, d4 = i - rh * V;                     // rh = r*Hq + h : contiguous in the partial buffers
         const float* w = w_smem + rh * m;
@@ -77,7 +79,7 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
                 const int k = k0 + kk;
                 if (k < m) {
                     const size_t slot = (size_t)(k / p.per) * gm.slots_per_gpu + (size_t)ul * p.per + (k % p.per);
-                    x[kk] = ld_stream(src + slot * (unit_o / 4) + i);
+                    x[kk] = ld_stream(kPeers ? reinterpret_cast<const float4*>(p.peer_O[k]) + src_at + i : src + slot * (unit_o / 4) + i);
                 }
             }
 #pragma unroll
@@ -142,16 +144,14 @@ int launch_merge(const MergeParams& p, cudaStream_t stream)
     const size_t smem = (size_t)p.rows_per_block * gm.heads_q * p.m * sizeof(float);
     dim3 grid(gm.L / p.rows_per_block, gm.a, gm.batch);
     cudaError_t e;
-    if (gm.head_dim == 128) {
-        e = cudaFuncSetAttribute(merge_kernel<128>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto go = [&](auto kernel) {
+        e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return (int)e;
-        merge_kernel<128><<<grid, kMergeThreads, smem, stream>>>(p);
-    } else {
-        e = cudaFuncSetAttribute(merge_kernel<64>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return (int)e;
-        merge_kernel<64><<<grid, kMergeThreads, smem, stream>>>(p);
-    }
-    return (int)cudaGetLastError();
+        kernel<<<grid, kMergeThreads, smem, stream>>>(p);
+        return (int)cudaGetLastError();
+    };
+    if (gm.head_dim == 128) return p.peers ? go(merge_kernel<128, true>) : go(merge_kernel<128, false>);
+    return p.peers ? go(merge_kernel<64, true>) : go(merge_kernel<64, false>);
 }
 
 int launch_delta(const DeltaParams& p, cudaStream_t stream)

@@ -215,6 +215,7 @@ static int launch_merge_slots(const mesh_attn_plan* p, int32_t q_group, int per,
     mp.gm.slots_per_gpu = slots_per_gpu;
     mp.q_group = q_group % p->geom.b;
     mp.per = per;
+    mp.peers = 0;
     mp.m = p->geom.a * mp.per;
     int rows = 8;
     while (rows > 1 && ((size_t)rows * p->geom.heads_q * mp.m * 4 > 64 * 1024 || p->geom.L % rows)) rows >>= 1;
@@ -340,11 +341,11 @@ int mesh_attn_rank_fwd(const mesh_attn_plan* p, int32_t g, const void* Q_loc, co
                            "rank_fwd", true);
 }
 
-int mesh_attn_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, const float* partial_lse_recv, float* O_own, float* lse_own,
-                         void* stream)
+static int launch_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, const float* partial_lse_recv, const float* const* peer_O,
+                             const float* const* peer_lse, float* O_own, float* lse_own, void* stream, const char* who)
 {
-    if (int rc = check_rank(p, 0, "rank_merge")) return rc;
-    if (!partial_O_recv || !partial_lse_recv || !O_own || !lse_own) return fail(MESH_ATTN_EINVAL, "rank_merge: null pointer");
+    if (int rc = check_rank(p, 0, who)) return rc;
+    if (!O_own || !lse_own) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null pointer");
     const Geom& g0 = p->geom;
     MergeParams mp;
     mp.gm = g0;
@@ -354,9 +355,19 @@ int mesh_attn_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, c
     mp.q_group = 0;
     mp.per = g0.a;                    // slot(k) = k: the partial received from the k-th member of the Q group
     mp.m = g0.a;
+    mp.peers = peer_O ? 1 : 0;
+    if (peer_O) {
+        if (g0.a > kMaxPeers) return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": Q groups of more than 16 GPUs are not supported");
+        for (int k = 0; k < g0.a; ++k) {
+            if (!peer_O[k] || !peer_lse[k]) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null peer pointer");
+            if (((uintptr_t)peer_O[k] & 15) != 0) return fail(MESH_ATTN_EINVAL, std::string(who) + ": peer partials must be 16-byte aligned");
+            mp.peer_O[k] = peer_O[k];
+            mp.peer_lse[k] = peer_lse[k];
+        }
+    }
     int rows = 8;
     while (rows > 1 && ((size_t)rows * g0.heads_q * mp.m * 4 > 64 * 1024 || g0.L % rows)) rows >>= 1;
-    if ((size_t)rows * g0.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, "rank_merge: heads_q * partial count too large");
+    if ((size_t)rows * g0.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": heads_q * partial count too large");
     mp.rows_per_block = rows;
     mp.partial_O = partial_O_recv;
     mp.partial_lse = partial_lse_recv;
@@ -367,9 +378,23 @@ int mesh_attn_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, c
     mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_MERGE, (cudaStream_t)stream);
     const int e = launch_merge(mp, (cudaStream_t)stream);
-    if (e) return cuda_fail("rank_merge launch", e);
+    if (e) return cuda_fail(who, e);
     g_launches.fetch_add(1);
     return MESH_ATTN_OK;
+}
+
+int mesh_attn_rank_merge(const mesh_attn_plan* p, const float* partial_O_recv, const float* partial_lse_recv, float* O_own, float* lse_own,
+                         void* stream)
+{
+    if (!partial_O_recv || !partial_lse_recv) return fail(MESH_ATTN_EINVAL, "rank_merge: null pointer");
+    return launch_rank_merge(p, partial_O_recv, partial_lse_recv, nullptr, nullptr, O_own, lse_own, stream, "rank_merge");
+}
+
+int mesh_attn_rank_merge_peers(const mesh_attn_plan* p, const float* const* peer_partial_O, const float* const* peer_partial_lse, float* O_own,
+                               float* lse_own, void* stream)
+{
+    if (!peer_partial_O || !peer_partial_lse) return fail(MESH_ATTN_EINVAL, "rank_merge_peers: null pointer table");
+    return launch_rank_merge(p, nullptr, nullptr, peer_partial_O, peer_partial_lse, O_own, lse_own, stream, "rank_merge_peers");
 }
 
 int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* p, const float* O_own, const void* dO_own, const float* lse_own, float* ws_own, void* stream)

@@ -7,6 +7,8 @@
 
 namespace mesh_attn {
 
+constexpr int kMaxPeers = 16;   // largest Q group the peer-memory merge takes (a <= 16: BASELINE.json's largest mesh)
+
 struct FwdParams {
     Geom gm;
     const FwdItem* items;      // per-simulated-GPU template, items_per_gpu entries
@@ -45,6 +47,11 @@ struct MergeParams {
     int rows_per_block;
     const float* partial_O;
     const float* partial_lse;
+    // peers != 0 (mesh_attn_rank_merge_peers): partial k is read from peer_O[k] / peer_lse[k] ([B][L][Hq][D] / [B][Hq][L]
+    // each, possibly another GPU's memory mapped into this process) instead of slot k of partial_O / partial_lse
+    int peers;
+    const float* peer_O[kMaxPeers];
+    const float* peer_lse[kMaxPeers];
     float* O;
     float* lse;
     long long lse_stride_b;    // batch stride of lse [B][Hq][N] (all heads * N)

@@ -41,6 +41,10 @@ def play_ranks(plan, w, inp, backward=True):
         O_own = torch.full((B, L, Hq, D), float("nan"), **f32)
         lse_own = torch.full((B, Hq, L), float("nan"), **f32)
         plan.rank_merge(rO, rl, O_own, lse_own)
+        # the same merge reading each partial where its producer wrote it (separate allocations stand in for peer memory)
+        O_peer, lse_peer = torch.full_like(O_own, float("nan")), torch.full_like(lse_own, float("nan"))
+        plan.rank_merge_peers([partials[m][0][k_u] for m in members], [partials[m][1][k_u] for m in members], O_peer, lse_peer)
+        assert torch.equal(O_peer, O_own) and torch.equal(lse_peer, lse_own), "peer-memory merge differs from rank_merge"
         own.append((O_own, lse_own))
         part(O, u).copy_(O_own)
         lse[:, :, u * L:(u + 1) * L].copy_(lse_own)
