@@ -268,6 +268,12 @@ int mesh_attn_rank_merge(const mesh_attn_plan* plan, const float* partial_O_recv
  * the members' rank_fwd (an event or a barrier across the group).  Bit-identical to rank_merge on the same partials. */
 int mesh_attn_rank_merge_peers(const mesh_attn_plan* plan, const float* const* peer_partial_O, const float* const* peer_partial_lse,
                                float* O_own, float* lse_own, void* stream);
+/* The reduce-scatters of Alg.3 l.6-7 in the same peer-memory form: out[i] = sum_k peers[k][i], i < count
+ * (fp32; count a multiple of 4; every buffer 16-byte aligned; 1 <= m <= 16).  peers is a HOST array of m device-accessible
+ * addresses: for RS-dQ member k's dQ_loc at this rank's slot (m = a, count = L*Hq*D with batch 1, else one call per
+ * batch), for RS-dKV member t's dK_loc / dV_loc at this rank's slot (m = b).  Plain sums in member order (deterministic,
+ * unlike a ring reduce-scatter whose order depends on the rank). */
+int mesh_attn_rank_sum_peers(const mesh_attn_plan* plan, const float* const* peers, int32_t m, int64_t count, float* out, void* stream);
 int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* plan, const float* O_own, const void* dO_own, const float* lse_own,
                                   float* ws_own, void* stream);
 int mesh_attn_rank_bwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc,

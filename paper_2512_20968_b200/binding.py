@@ -70,6 +70,7 @@ lib.mesh_attn_rank_fwd.argtypes = [_P, C.c_int32] + [_P] * 6
 lib.mesh_attn_rank_merge.argtypes = [_P] * 6
 lib.mesh_attn_rank_merge_peers.argtypes = [_P, C.POINTER(_P), C.POINTER(_P), _P, _P, _P]
 lib.mesh_attn_rank_bwd_preprocess.argtypes = [_P] * 6
+lib.mesh_attn_rank_sum_peers.argtypes = [_P, C.POINTER(_P), C.c_int32, C.c_int64, _P, _P]
 lib.mesh_attn_rank_bwd.argtypes = [_P, C.c_int32] + [_P] * 9
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
 lib.mesh_attn_launch_count.restype = C.c_int64
@@ -84,7 +85,7 @@ EXPORTED = [
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
-    "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
+    "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_sum_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
 ]
 K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
 
@@ -228,6 +229,11 @@ class Plan:
         po = (_P * m)(*[_ptr(t) for t in peer_partial_O])
         pl = (_P * m)(*[_ptr(t) for t in peer_partial_lse])
         _check(lib.mesh_attn_rank_merge_peers(self._h, po, pl, _ptr(O_own), _ptr(lse_own), _stream(stream)))
+
+    def rank_sum_peers(self, peers, out, stream=None):
+        """out = sum of the fp32 buffers `peers` (tensors with out's element count, or device addresses)"""
+        tab = (_P * len(peers))(*[_ptr(t) for t in peers])
+        _check(lib.mesh_attn_rank_sum_peers(self._h, tab, len(peers), out.numel(), _ptr(out), _stream(stream)))
 
     def rank_bwd_preprocess(self, O_own, dO_own, lse_own, ws_own, stream=None):
         _check(lib.mesh_attn_rank_bwd_preprocess(self._h, _ptr(O_own), _ptr(dO_own), _ptr(lse_own), _ptr(ws_own), _stream(stream)))

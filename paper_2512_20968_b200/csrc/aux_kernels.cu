@@ -4,6 +4,8 @@
 //   delta_kernel   backward preprocess Delta = rowsum(dO o O), plus -lse*log2e
 // Both are streaming kernels: 16-byte vector loads, many independent loads in flight per
 // thread, streaming cache hints, no shared-memory reuse of the bulk data.
+#include <algorithm>
+
 #include <cuda_bf16.h>
 
 #include "tile_kernels.hpp"
@@ -136,7 +138,35 @@ __global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
     }
 }
 
+// out = sum of m buffers (fp32, float4 granularity), grid-stride, up to 8 independent 16-byte loads in flight per thread
+__global__ void __launch_bounds__(256) sum_peers_kernel(const SumParams p)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < p.count4; i += stride) {
+        float4 acc = make_float4(0.f, 0.f, 0.f, 0.f);
+        for (int k0 = 0; k0 < p.m; k0 += kMergeUnroll) {
+            float4 x[kMergeUnroll];
+#pragma unroll
+            for (int kk = 0; kk < kMergeUnroll; ++kk)
+                if (k0 + kk < p.m) x[kk] = ld_stream(reinterpret_cast<const float4*>(p.src[k0 + kk]) + i);
+#pragma unroll
+            for (int kk = 0; kk < kMergeUnroll; ++kk)
+                if (k0 + kk < p.m) { acc.x += x[kk].x; acc.y += x[kk].y; acc.z += x[kk].z; acc.w += x[kk].w; }
+        }
+        st_stream(reinterpret_cast<float4*>(p.out) + i, acc);
+    }
+}
+
 }  // namespace
+
+int launch_sum_peers(const SumParams& p, int num_sms, cudaStream_t stream)
+{
+    const long long blocks = (p.count4 + 255) / 256;
+    const unsigned grid = (unsigned)std::min<long long>(blocks, (long long)num_sms * 8);
+    if (grid == 0) return 0;
+    sum_peers_kernel<<<grid, 256, 0, stream>>>(p);
+    return (int)cudaGetLastError();
+}
 
 int launch_merge(const MergeParams& p, cudaStream_t stream)
 {

@@ -397,6 +397,26 @@ int mesh_attn_rank_merge_peers(const mesh_attn_plan* p, const float* const* peer
     return launch_rank_merge(p, nullptr, nullptr, peer_partial_O, peer_partial_lse, O_own, lse_own, stream, "rank_merge_peers");
 }
 
+int mesh_attn_rank_sum_peers(const mesh_attn_plan* p, const float* const* peers, int32_t m, int64_t count, float* out, void* stream)
+{
+    if (int rc = check_device(p, "rank_sum_peers")) return rc;
+    if (!peers || !out) return fail(MESH_ATTN_EINVAL, "rank_sum_peers: null pointer");
+    if (m < 1 || m > kMaxPeers) return fail(MESH_ATTN_EUNSUPPORTED, "rank_sum_peers: 1 <= m <= 16 buffers");
+    if (count < 0 || (count & 3) || ((uintptr_t)out & 15)) return fail(MESH_ATTN_EINVAL, "rank_sum_peers: count must be a multiple of 4 floats, buffers 16-byte aligned");
+    SumParams sp;
+    sp.m = m;
+    sp.count4 = count / 4;
+    sp.out = out;
+    for (int k = 0; k < m; ++k) {
+        if (!peers[k] || ((uintptr_t)peers[k] & 15)) return fail(MESH_ATTN_EINVAL, "rank_sum_peers: null or misaligned peer pointer");
+        sp.src[k] = peers[k];
+    }
+    const int e = launch_sum_peers(sp, p->num_sms, (cudaStream_t)stream);
+    if (e) return cuda_fail("rank_sum_peers launch", e);
+    if (count) g_launches.fetch_add(1);
+    return MESH_ATTN_OK;
+}
+
 int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* p, const float* O_own, const void* dO_own, const float* lse_own, float* ws_own, void* stream)
 {
     if (int rc = check_rank(p, 0, "rank_bwd_preprocess")) return rc;

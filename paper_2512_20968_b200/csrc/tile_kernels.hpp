@@ -58,6 +58,13 @@ struct MergeParams {
     long long o_stride_b, o_stride_row, o_stride_h;   // element strides of O
 };
 
+struct SumParams {               // out[i] = sum_k src[k][i]: the reduce-scatters of Alg.3 l.6-7 read from where the members wrote
+    int m;
+    long long count4;            // float4 elements
+    const float* src[kMaxPeers];
+    float* out;
+};
+
 struct DeltaParams {
     Geom gm;
     const float* O;
@@ -74,5 +81,6 @@ int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
                     const CUtensorMap& tmdO, const CUtensorMap& tmdQ, int num_sms, cudaStream_t stream);
 int launch_merge(const MergeParams& p, cudaStream_t stream);
 int launch_delta(const DeltaParams& p, cudaStream_t stream);
+int launch_sum_peers(const SumParams& p, int num_sms, cudaStream_t stream);
 
 }  // namespace mesh_attn

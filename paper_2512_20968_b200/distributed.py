@@ -14,10 +14,18 @@ C-ABI calls (``mesh_attn_rank_fwd / rank_merge / rank_bwd_preprocess / rank_bwd`
               rank_bwd: this GPU's contribution to dQ of its Q partitions and dK, dV of its KV partitions
               RS-dQ (sum over the Q group), RS-dKV (sum over the KV group)
 
-This is the NCCL-collective form, NOT a fused compute+collective kernel, and it has never run on more than one GPU
-(this build's boxes have one): the per-rank kernels are parity-tested on one B200 by playing the n ranks one after the
-other (tests/test_gpu_rank_calls.py), the group construction / slot order / routing by world-size 2 and 4 gloo
-processes with stand-in compute (tests/test_multirank_cpu.py).  Needs kvr = 1 (with KV partition rotation the ranks
+Two forms of the exchanges that FOLLOW a compute step (RS-O, RS-dQ, RS-dKV):
+  * ``peer_memory=False``: NCCL collectives (all-to-all + rank_merge; reduce_scatter) -- the baseline;
+  * ``peer_memory=True`` : the partial buffers live in symmetric memory (``torch.distributed._symmetric_memory``) and the
+    reducer reads every member's partial where it was written, over NVLink (``mesh_attn_rank_merge_peers``,
+    ``mesh_attn_rank_sum_peers``): the loads of the reducer ARE the transfer, there is no receive buffer and no
+    separate collective.  Each partial is read exactly once, so peer reads cost no extra link traffic.  The all-gathers
+    that PRECEDE a compute step stay NCCL copies into local HBM on purpose: every Q / K / V tile is re-read by dozens of
+    work items, and peer memory is not cached in the reader's L2.
+Neither form has run on more than one GPU (this build's boxes have one): the per-rank kernels, the peer-memory reducers
+included, are parity-tested on one B200 by playing the n ranks one after the other (tests/test_gpu_rank_calls.py), the
+group construction / slot order / routing by world-size 2 and 4 gloo processes with stand-in compute
+(tests/test_multirank_cpu.py); the symmetric-memory rendezvous of ``peer_memory=True`` is unexecuted code.  Needs kvr = 1 (with KV partition rotation the ranks
 that share a KV footprint are exactly the owners of its partitions, L157-161), usp_lanes = 1, tensor_layout 0.
 """
 from __future__ import annotations
@@ -85,8 +93,9 @@ class MeshAttnRank:
     """One rank of the job.  ``kernels`` is the object whose ``rank_*`` methods do the arithmetic: the Plan itself
     (default; there is no other product path), or a stand-in with the same four methods in the CPU tests."""
 
-    def __init__(self, plan, rank: int | None = None, world_size: int | None = None, kernels=None):
+    def __init__(self, plan, rank: int | None = None, world_size: int | None = None, kernels=None, peer_memory: bool = False):
         self.plan = plan
+        self.peer_memory = peer_memory
         self.g = dist.get_rank() if rank is None else rank
         world = dist.get_world_size() if world_size is None else world_size
         d = plan.desc
@@ -109,6 +118,26 @@ class MeshAttnRank:
             if list(ranks) == self.kv_ranks:
                 self.kv_group = grp
         self._saved = None
+        self._symm = None
+
+    def _symmetric(self, dev):
+        """symmetric-memory buffers of the peer-memory form, created and exchanged once (collective over each group)"""
+        if self._symm is None:
+            import torch.distributed._symmetric_memory as symm_mem
+
+            a, b, B, L, Hq, Hkv, D = self.a, self.b, self.B, self.L, self.Hq, self.Hkv, self.D
+            f32 = dict(dtype=torch.float32, device=dev)
+            bufs = {"pO": ((a, B, L, Hq, D), self.q_group), "plse": ((a, B, Hq, L), self.q_group), "dQ": ((B, a * L, Hq, D), self.q_group),
+                    "dK": ((B, b * L, Hkv, D), self.kv_group), "dV": ((B, b * L, Hkv, D), self.kv_group)}
+            self._symm = {}
+            for name, (shape, grp) in bufs.items():
+                t = symm_mem.empty(*shape, **f32)
+                self._symm[name] = (t, symm_mem.rendezvous(t, grp))
+        return self._symm
+
+    @staticmethod
+    def _slot_ptrs(handle, members: int, slot: int, slot_elems: int):
+        return [int(handle.buffer_ptrs[k]) + slot * slot_elems * 4 for k in range(members)]
 
     # Alg.2 (PAPER.md L167-174)
     def forward(self, Q_own: torch.Tensor, K_own: torch.Tensor, V_own: torch.Tensor):
@@ -118,14 +147,22 @@ class MeshAttnRank:
         Q_loc = _gather_slots(Q_own, self.q_ranks, self.q_group)          # l.1 AG-Q
         K_loc = _gather_slots(K_own, self.kv_ranks, self.kv_group)        # l.2 AG-KV
         V_loc = _gather_slots(V_own, self.kv_ranks, self.kv_group)
-        partial_O = torch.empty((a, B, L, Hq, D), dtype=torch.float32, device=dev)
-        partial_lse = torch.empty((a, B, Hq, L), dtype=torch.float32, device=dev)
-        self.kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)      # l.3-5
-        recv_O = _exchange_slots(partial_O, self.q_ranks, self.q_index, self.q_group)       # l.6 RS-O: slot k -> member k
-        recv_lse = _exchange_slots(partial_lse, self.q_ranks, self.q_index, self.q_group)
         O_own = torch.empty((B, L, Hq, D), dtype=torch.float32, device=dev)
         lse_own = torch.empty((B, Hq, L), dtype=torch.float32, device=dev)
-        self.kernels.rank_merge(recv_O, recv_lse, O_own, lse_own)                       # ... with the online-softmax reducer
+        if self.peer_memory:
+            (partial_O, hO), (partial_lse, hl) = self._symmetric(dev)["pO"], self._symmetric(dev)["plse"]
+            hO.barrier()                                                                # the members have merged the previous step's partials
+            self.kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)  # l.3-5
+            hO.barrier()                                                                # every member's partials are written
+            self.kernels.rank_merge_peers(self._slot_ptrs(hO, a, self.q_index, B * L * Hq * D),     # l.6 RS-O fused into the reducer
+                                          self._slot_ptrs(hl, a, self.q_index, B * Hq * L), O_own, lse_own)
+        else:
+            partial_O = torch.empty((a, B, L, Hq, D), dtype=torch.float32, device=dev)
+            partial_lse = torch.empty((a, B, Hq, L), dtype=torch.float32, device=dev)
+            self.kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)      # l.3-5
+            recv_O = _exchange_slots(partial_O, self.q_ranks, self.q_index, self.q_group)   # l.6 RS-O: slot k -> member k
+            recv_lse = _exchange_slots(partial_lse, self.q_ranks, self.q_index, self.q_group)
+            self.kernels.rank_merge(recv_O, recv_lse, O_own, lse_own)                       # ... with the online-softmax reducer
         self._saved = (Q_loc, K_loc, V_loc, O_own, lse_own)
         return O_own, lse_own
 
@@ -143,6 +180,23 @@ class MeshAttnRank:
         ws_all = torch.empty((a, 2, B, Hq, L), dtype=torch.float32, device=dev)
         dist.all_gather(list(ws_all.unbind(0)), ws_own, group=self.q_group)
         ws_loc = ws_all.permute(1, 2, 3, 0, 4).reshape(2, B, Hq, a * L).contiguous()    # member k at rows k*L..
+        if self.peer_memory:
+            if B != 1:
+                raise ValueError("peer_memory=True takes batch 1 (a rank's slot of a local gradient must be contiguous)")
+            sm = self._symmetric(dev)
+            (dQ_loc, hQ), (dK_loc, hK), (dV_loc, hV) = sm["dQ"], sm["dK"], sm["dV"]
+            hQ.barrier(); hK.barrier()                                                  # the previous step's sums have been read
+            for t in (dQ_loc, dK_loc, dV_loc):
+                t.zero_()
+            self.kernels.rank_bwd(self.g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc)   # l.3-5
+            hQ.barrier(); hK.barrier()
+            dQ_own = torch.empty((B, L, Hq, D), dtype=torch.float32, device=dev)
+            dK_own = torch.empty((B, L, Hkv, D), dtype=torch.float32, device=dev)
+            dV_own = torch.empty((B, L, Hkv, D), dtype=torch.float32, device=dev)
+            self.kernels.rank_sum_peers(self._slot_ptrs(hQ, a, self.q_index, L * Hq * D), dQ_own)        # l.6 RS-dQ as peer reads
+            self.kernels.rank_sum_peers(self._slot_ptrs(hK, b, self.kv_index, L * Hkv * D), dK_own)      # l.7 RS-dKV
+            self.kernels.rank_sum_peers(self._slot_ptrs(hV, b, self.kv_index, L * Hkv * D), dV_own)
+            return dQ_own, dK_own, dV_own
         dQ_loc = torch.zeros((B, a * L, Hq, D), dtype=torch.float32, device=dev)
         dK_loc = torch.zeros((B, b * L, Hkv, D), dtype=torch.float32, device=dev)
         dV_loc = torch.zeros((B, b * L, Hkv, D), dtype=torch.float32, device=dev)

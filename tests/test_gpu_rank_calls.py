@@ -59,6 +59,7 @@ def play_ranks(plan, w, inp, backward=True):
     dQ = torch.zeros((B, n * L, Hq, D), **f32)
     dK = torch.zeros((B, n * L, Hkv, D), **f32)
     dV = torch.zeros((B, n * L, Hkv, D), **f32)
+    grads_loc = []
     for g in range(n):
         iq, ikv = foot[g]
         Ql, Kl, Vl = loc[g]
@@ -68,11 +69,16 @@ def play_ranks(plan, w, inp, backward=True):
         dKl = torch.zeros((B, b * L, Hkv, D), **f32)
         dVl = torch.zeros((B, b * L, Hkv, D), **f32)
         plan.rank_bwd(g, Ql, Kl, Vl, dOl, ws_loc, dQl, dKl, dVl)
-        for k, u in enumerate(iq):
-            part(dQ, int(u)).add_(part(dQl, k))
-        for t, v in enumerate(ikv):
-            part(dK, int(v)).add_(part(dKl, t))
-            part(dV, int(v)).add_(part(dVl, t))
+        grads_loc.append((dQl, dKl, dVl))
+    # RS-dQ / RS-dKV: rank u sums its slot of every member's local gradients, read where the members wrote them
+    assert B == 1
+    for u in range(n):
+        q_members, kv_members = [int(x) for x in foot[u][0]], [int(x) for x in foot[u][1]]
+        k_u, t_u = q_members.index(u), kv_members.index(u)
+        for which, members, slot, dst in ((0, q_members, k_u, dQ), (1, kv_members, t_u, dK), (2, kv_members, t_u, dV)):
+            own_sum = torch.empty_like(part(dst, u)[0])
+            plan.rank_sum_peers([part(grads_loc[m][which], slot)[0] for m in members], own_sum)
+            part(dst, u).copy_(own_sum)
     torch.cuda.synchronize()
     return O, lse, (dQ, dK, dV)
 
