@@ -135,3 +135,32 @@ def test_mesh_ranks_world2_kv_group(tmp_path):
 def test_mesh_ranks_world4(tmp_path):
     """2 x 2 mesh, causal, striped: both group kinds, KV partition rotation (KV group of rank g = {g mod a + t*a})."""
     _check_mesh(tmp_path, 2, 2, True, 2, 1)
+
+
+def test_mesh_groups_follow_the_assignment_matrix():
+    """Q group of rank g = the ranks of its tile row, KV group = the ranks sharing its rotated KV footprint (PAPER.md L116,
+    L157-161): both contain g, partition the ranks, and every (i, j) cell of the AM is owned by the one rank that sits in
+    i's Q group and j's KV group.  Without KV rotation, or with a world size other than n, the mapping is refused."""
+    import numpy as np
+    import pytest
+
+    from paper_2512_20968_b200 import plan_for
+    from paper_2512_20968_b200 import workloads as W
+    from paper_2512_20968_b200.distributed import mesh_groups
+
+    for a, b in ((2, 2), (3, 3), (2, 4), (4, 2)):
+        w = W.Workload("m", 7, True, a, b, 1, 128 * a * b, 2, 2, 64, seq_layout="striped")
+        plan = plan_for(w)
+        qg, kg = mesh_groups(plan, a * b)
+        am = plan.am()
+        assert sorted(set(map(tuple, qg))) == [tuple(range(r * a, (r + 1) * a)) for r in range(b)]
+        assert sorted(set(map(tuple, kg))) == [tuple(c + t * a for t in range(b)) for c in range(a)]
+        for i in range(a * b):
+            for j in range(a * b):
+                owners = [g for g in range(a * b) if i in qg[g] and j in kg[g]]
+                assert owners == [int(am[i, j])]
+        with pytest.raises(ValueError):
+            mesh_groups(plan, a * b + 1)
+    w = W.Workload("m", 7, False, 2, 2, 1, 512, 2, 2, 64, kvr=False)
+    with pytest.raises(ValueError):
+        mesh_groups(plan_for(w), 4)
