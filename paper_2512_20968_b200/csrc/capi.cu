@@ -217,7 +217,10 @@ static int launch_merge_slots(const mesh_attn_plan* p, int32_t q_group, int per,
     mp.per = per;
     mp.peers = 0;
     mp.m = p->geom.a * mp.per;
-    int rows = 8;
+    // rows per block: 2 measured best on every BASELINE.json geometry (isolated launches, 1 / 2 / 4 / 8 rows: C2 4.7 / 5.1 / 5.1 /
+    // 4.6, C4 6.25 / 6.48 / 6.25 / 6.13, C5 6.22 / 6.65 / 6.61 / 6.44 TB/s; profiles/r01_v7_README.md): small blocks keep the
+    // weight phase short and many blocks streaming
+    int rows = 2;
     while (rows > 1 && ((size_t)rows * p->geom.heads_q * mp.m * 4 > 64 * 1024 || p->geom.L % rows)) rows >>= 1;
     if ((size_t)rows * p->geom.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, "merge: heads_q * partial count too large");
     mp.rows_per_block = rows;
@@ -365,7 +368,7 @@ static int launch_rank_merge(const mesh_attn_plan* p, const float* partial_O_rec
             mp.peer_lse[k] = peer_lse[k];
         }
     }
-    int rows = 8;
+    int rows = 2;                     // as in launch_merge_slots
     while (rows > 1 && ((size_t)rows * g0.heads_q * mp.m * 4 > 64 * 1024 || g0.L % rows)) rows >>= 1;
     if ((size_t)rows * g0.heads_q * mp.m * 4 > 200 * 1024) return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": heads_q * partial count too large");
     mp.rows_per_block = rows;
