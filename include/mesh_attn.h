@@ -279,6 +279,18 @@ int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* plan, const float* O_own
 int mesh_attn_rank_bwd(const mesh_attn_plan* plan, int32_t g, const void* Q_loc, const void* K_loc, const void* V_loc,
                        const void* dO_loc, const float* ws_loc, float* dQ_loc, float* dK_loc, float* dV_loc, void* stream);
 
+/* The backward step list (mesh_attn_plan_steps pass 1; reading R12: the paper omits the backward schedule, P:L238,
+ * so the order is parity-unpinned) executed task by task for the `a` simulated GPUs of Q group q_group, like
+ * mesh_attn_forward_goo: compute task C-i-j = a chunk-granular tile_bwd launch (the 128-key blocks of KV chunk j of every KV
+ * partition of each footprint, against Q chunk i of every Q partition), the step's collective (AG of Q, O, dO chunk i = 3 Q
+ * units; AG-KV-j; RS-dQ-i; RS-dKV-j) stood in for by device-to-device copies of its bytes on a plan-owned stream when
+ * overlap != 0, a barrier per step.  ACCUMULATES into dQ, dK, dV exactly what mesh_attn_tile_bwd(q_group*a, a) adds (any
+ * order of the compute tasks gives the same sums up to fp32 rounding); the caller zeroes them and runs
+ * mesh_attn_bwd_preprocess first. */
+int mesh_attn_backward_goo(const mesh_attn_plan* plan, int32_t q_group, const void* Q, const void* K, const void* V, const void* dO,
+                           const float* bwd_ws, float* dQ, float* dK, float* dV,
+                           void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap, void* stream);
+
 /* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
 int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
                        const float* O, const void* dO, const float* lse, float* bwd_ws,

@@ -66,6 +66,7 @@ lib.mesh_attn_tile_bwd.argtypes = [_P, C.c_int32, C.c_int32] + [_P] * 9
 lib.mesh_attn_forward.argtypes = [_P] * 9
 lib.mesh_attn_forward_goo.argtypes = [_P, C.c_int32] + [_P] * 8 + [C.c_int64, C.c_int32, C.c_int32, _P]
 lib.mesh_attn_backward.argtypes = [_P] * 12
+lib.mesh_attn_backward_goo.argtypes = [_P, C.c_int32] + [_P] * 9 + [C.c_int64, C.c_int32, C.c_int32, _P]
 lib.mesh_attn_rank_fwd.argtypes = [_P, C.c_int32] + [_P] * 6
 lib.mesh_attn_rank_merge.argtypes = [_P] * 6
 lib.mesh_attn_rank_merge_peers.argtypes = [_P, C.POINTER(_P), C.POINTER(_P), _P, _P, _P]
@@ -83,7 +84,7 @@ lib.mesh_attn_last_error.restype = C.c_char_p
 EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
-    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
+    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
     "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_sum_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
 ]
@@ -211,6 +212,11 @@ class Plan:
         nbytes = 0 if comm_ws is None else comm_ws.numel() * comm_ws.element_size()
         _check(lib.mesh_attn_forward_goo(self._h, q_group, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _ptr(partial_O), _ptr(partial_lse),
                                          _ptr(comm_ws), nbytes, comm_repeat, int(bool(overlap)), _stream(stream)))
+
+    def backward_goo(self, q_group, Q, K, V, dO, bwd_ws, dQ, dK, dV, comm_ws=None, comm_repeat=0, overlap=True, stream=None):
+        nbytes = 0 if comm_ws is None else comm_ws.numel() * comm_ws.element_size()
+        _check(lib.mesh_attn_backward_goo(self._h, q_group, _ptr(Q), _ptr(K), _ptr(V), _ptr(dO), _ptr(bwd_ws), _ptr(dQ), _ptr(dK), _ptr(dV),
+                                          _ptr(comm_ws), nbytes, comm_repeat, int(bool(overlap)), _stream(stream)))
 
     def backward(self, Q, K, V, O, dO, lse, bwd_ws, dQ, dK, dV, stream=None):
         _check(lib.mesh_attn_backward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(dO), _ptr(lse), _ptr(bwd_ws),

@@ -117,9 +117,9 @@ int upload_plan(mesh_attn_plan* p)
     const size_t b0 = al(p->fwd_items.size() * sizeof(FwdItem)), b1 = al(p->bwd_items.size() * sizeof(BwdItem)),
                  b2 = al(p->fwd_segs.size() * sizeof(Seg)), b3 = al(p->bwd_segs.size() * sizeof(Seg)),
                  b4 = al(p->fwd_seglists.size() * sizeof(SegList)), b5 = al(p->bwd_seglists.size() * sizeof(SegList)),
-                 b6 = al(p->goo_items.size() * sizeof(FwdItem));
+                 b6 = al(p->goo_items.size() * sizeof(FwdItem)), b7 = al(p->goo_bwd_items.size() * sizeof(BwdItem));
     char* d = nullptr;
-    cudaError_t e = cudaMalloc(&d, b0 + b1 + b2 + b3 + b4 + b5 + b6 + 256);
+    cudaError_t e = cudaMalloc(&d, b0 + b1 + b2 + b3 + b4 + b5 + b6 + b7 + 256);
     if (e != cudaSuccess) return cuda_fail("cudaMalloc(work lists)", (int)e);
     p->d_blob = d;
     auto put = [&](const void* src, size_t bytes, size_t cap) {
@@ -135,6 +135,7 @@ int upload_plan(mesh_attn_plan* p)
     p->d_fwd_seglists = (const SegList*)put(p->fwd_seglists.data(), p->fwd_seglists.size() * sizeof(SegList), b4);
     p->d_bwd_seglists = (const SegList*)put(p->bwd_seglists.data(), p->bwd_seglists.size() * sizeof(SegList), b5);
     p->d_goo_items = (const FwdItem*)put(p->goo_items.data(), p->goo_items.size() * sizeof(FwdItem), b6);
+    p->d_goo_bwd_items = (const BwdItem*)put(p->goo_bwd_items.data(), p->goo_bwd_items.size() * sizeof(BwdItem), b7);
     if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
     // step_host's copy engines: one stream per direction, events for the chunk hand-offs
     cudaStream_t s0 = nullptr, s1 = nullptr;
@@ -272,13 +273,17 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
 }
 
 static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count, const void* Q, const void* K, const void* V,
-                      const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream, bool local)
+                      const void* dO, const float* bwd_ws, float* dQ, float* dK, float* dV, void* stream, bool local,
+                      const BwdItem* items = nullptr, int items_per_gpu = -1)
 {
+    const bool own_list = items != nullptr;                 // a compute task of the GOO executor: single-CTA kernel
+    if (!own_list) { items = p->d_bwd_items; items_per_gpu = (int)p->bwd_items.size(); }
+    if (items_per_gpu == 0) return MESH_ATTN_OK;
     if (int rc = check_device(p, "tile_bwd")) return rc;
     if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "tile_bwd: null pointer");
     Lane ln;
     if (!lane_of_range(p, g_first, g_count, &ln)) return fail(MESH_ATTN_EINVAL, "tile_bwd: simulated GPU range out of bounds (or crossing a USP lane)");
-    if ((long long)g_count * (long long)p->bwd_items.size() >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
+    if ((long long)g_count * (long long)items_per_gpu >= (1ll << 31)) return fail(MESH_ATTN_EINVAL, "tile_bwd: too many work items in one call");
     CUtensorMap tmQ, tmK, tmV, tmdO, tmdQ;
     const long long N = local ? (long long)p->geom.a * p->geom.L : (long long)p->geom.n * p->geom.L;     // query-shaped rows
     const long long Nk = local ? (long long)p->geom.b * p->geom.L : (long long)p->geom.n * p->geom.L;   // key-shaped rows
@@ -287,7 +292,7 @@ static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count,
     dK = head_slice(dK, ln.hk0, sdk, 4);
     dV = head_slice(dV, ln.hk0, sdk, 4);
     // paired items (2-CTA clusters): each CTA loads 64-row halves of the Q / dO tiles and multicasts them
-    const bool pair = p->bwd_pairable && ((long long)g_count * (long long)p->bwd_items.size()) >= 2 && !p->no_pair;
+    const bool pair = !own_list && p->bwd_pairable && ((long long)g_count * (long long)items_per_gpu) >= 2 && !p->no_pair;
     const int qbox = pair ? kBlock / 2 : kBlock;
     if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox, N) ||
         !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, Nk) ||
@@ -298,10 +303,10 @@ static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count,
     BwdParams bp;
     bp.gm = p->geom;
     if (local) { bp.gm.local = 1; bp.gm.rows_q = (int32_t)N; bp.gm.rows_kv = (int32_t)Nk; }
-    bp.items = p->d_bwd_items;
+    bp.items = items;
     bp.segs = p->d_bwd_segs;
     bp.seglists = p->d_bwd_seglists;
-    bp.items_per_gpu = (int)p->bwd_items.size();
+    bp.items_per_gpu = items_per_gpu;
     bp.g_first = g_first % p->geom.n;
     bp.g_count = g_count;
     bp.split = p->desc.precision;
@@ -532,6 +537,72 @@ int mesh_attn_forward_goo(const mesh_attn_plan* p, int32_t q_group, const void* 
         at = k;
     }
     return launch_merge_slots(p, q_group, p->k_kv, slots, partial_O, partial_lse, O, lse, stream);
+}
+
+int mesh_attn_backward_goo(const mesh_attn_plan* p, int32_t q_group, const void* Q, const void* K, const void* V, const void* dO,
+                           const float* bwd_ws, float* dQ, float* dK, float* dV, void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat,
+                           int32_t overlap, void* stream)
+{
+    if (int rc = check_device(p, "backward_goo")) return rc;
+    if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward_goo: null pointer");
+    if (comm_repeat < 0 || (comm_repeat > 0 && (!comm_ws || comm_ws_bytes < 4096))) return fail(MESH_ATTN_EINVAL, "backward_goo: comm_ws too small");
+    const Geom& gm = p->geom;
+    if (q_group < 0 || q_group >= gm.b * lanes_of(p)) return fail(MESH_ATTN_EINVAL, "backward_goo: q_group out of range");
+    const int lane = q_group / gm.b, r = q_group % gm.b, g_first = lane * gm.n + r * gm.a;
+    cudaStream_t st = (cudaStream_t)stream, cs = overlap ? (cudaStream_t)p->s_h2d : st;
+    cudaEvent_t ev_fork = (cudaEvent_t)p->copy_events[2 * gm.b + 6], ev_join = (cudaEvent_t)p->copy_events[2 * gm.b + 7];
+    const long long q_bytes = (long long)gm.batch * gm.n * gm.L * p->desc.heads_q * gm.head_dim * 2;
+    const long long kv_bytes = (long long)gm.batch * gm.n * gm.L * p->desc.heads_kv * gm.head_dim * 2;
+    auto copy_bytes = [&](const void* src, long long src_bytes, long long bytes) -> cudaError_t {
+        const long long chunk = std::min<long long>(std::min<long long>(src_bytes, comm_ws_bytes), bytes);
+        for (int rep = 0; rep < comm_repeat; ++rep)
+            for (long long done = 0; done < bytes; done += chunk) {
+                const cudaError_t e = cudaMemcpyAsync(comm_ws, src, (size_t)std::min(chunk, bytes - done), cudaMemcpyDeviceToDevice, cs);
+                if (e != cudaSuccess) return e;
+            }
+        return cudaSuccess;
+    };
+    const std::vector<int32_t>& rows = p->steps_bwd;
+    const size_t nrows = rows.size() / 4;
+    for (size_t at = 0; at < nrows;) {
+        const int step = rows[4 * at];
+        cudaError_t e = cudaSuccess;
+        if (overlap) {
+            e = cudaEventRecord(ev_fork, st);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(cs, ev_fork, 0);
+        }
+        // bytes in units of the bf16 inputs, as the paper counts them: AG of Q, O, dO = 3 Q units per chunk,
+        // RS-dQ one, AG-KV and RS-dKV a K and a V unit each
+        for (size_t k = at; k < nrows && rows[4 * k] == step && e == cudaSuccess; ++k) {
+            const int kind = rows[4 * k + 1];
+            if (comm_repeat == 0 || kind == MESH_ATTN_TASK_C) continue;
+            if (kind == MESH_ATTN_TASK_AG_Q) {
+                const long long bytes = goo_task_bytes(p, MESH_ATTN_TASK_AG_Q);
+                e = copy_bytes(Q, q_bytes, bytes);
+                if (e == cudaSuccess) e = copy_bytes(dO, q_bytes, 2 * bytes);
+            } else if (kind == MESH_ATTN_TASK_RS_Q) {
+                e = copy_bytes(dQ, 2 * q_bytes, goo_task_bytes(p, MESH_ATTN_TASK_RS_Q));
+            } else {                                          // AG-KV, RS-dKV
+                const long long bytes = goo_task_bytes(p, MESH_ATTN_TASK_AG_KV);
+                e = copy_bytes(kind == MESH_ATTN_TASK_AG_KV ? K : (const void*)dK, kv_bytes, bytes / 2);
+                if (e == cudaSuccess) e = copy_bytes(kind == MESH_ATTN_TASK_AG_KV ? V : (const void*)dV, kv_bytes, bytes / 2);
+            }
+        }
+        if (e != cudaSuccess) return cuda_fail("backward_goo: communication stand-in", (int)e);
+        size_t k = at;
+        for (; k < nrows && rows[4 * k] == step; ++k) {
+            if (rows[4 * k + 1] != MESH_ATTN_TASK_C) continue;
+            const SegList task = p->goo_bwd_task[(size_t)rows[4 * k + 2] * p->k_kv + rows[4 * k + 3]];
+            if (int rc = launch_bwd(p, g_first, gm.a, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream, false, p->d_goo_bwd_items + task.offset, task.count)) return rc;
+        }
+        if (overlap) {
+            e = cudaEventRecord(ev_join, cs);
+            if (e == cudaSuccess) e = cudaStreamWaitEvent(st, ev_join, 0);
+            if (e != cudaSuccess) return cuda_fail("backward_goo: step barrier", (int)e);
+        }
+        at = k;
+    }
+    return MESH_ATTN_OK;
 }
 
 int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const float* O, const void* dO,

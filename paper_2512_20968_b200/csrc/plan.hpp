@@ -116,6 +116,10 @@ struct mesh_attn_plan {
     // goo_items[goo_task[i*k_kv+j].offset .. +count), partial slot = u_local*k_kv + j
     std::vector<mesh_attn::FwdItem> goo_items;
     std::vector<mesh_attn::SegList> goo_task;
+    // the same for the backward executor (mesh_attn_backward_goo): items of C-i-j = the 128-key blocks of KV chunk j of every
+    // KV partition, each walking Q chunk i of every Q partition (their seg lists are appended to bwd_segs / bwd_seglists)
+    std::vector<mesh_attn::BwdItem> goo_bwd_items;
+    std::vector<mesh_attn::SegList> goo_bwd_task;
     // backward items 2k and 2k+1 visit the same Q blocks on every simulated GPU (tile_bwd then runs 2-CTA clusters that
     // share the Q / dO tile loads); no_pair = environment override MESH_ATTN_NO_PAIR=1 (A/B measurements)
     bool bwd_pairable = false, no_pair = false;
@@ -126,6 +130,7 @@ struct mesh_attn_plan {
     void* d_blob = nullptr;
     const mesh_attn::FwdItem* d_fwd_items = nullptr;
     const mesh_attn::FwdItem* d_goo_items = nullptr;
+    const mesh_attn::BwdItem* d_goo_bwd_items = nullptr;
     const mesh_attn::BwdItem* d_bwd_items = nullptr;
     const mesh_attn::Seg* d_fwd_segs = nullptr;
     const mesh_attn::Seg* d_bwd_segs = nullptr;

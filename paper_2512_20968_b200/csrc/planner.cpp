@@ -237,6 +237,30 @@ void build_worklists(mesh_attn_plan* p)
                 p->bwd_items.insert(p->bwd_items.end(), grp.begin(), grp.end());
             }
         }
+
+    // ---------- backward, chunk-granular (GOO executor): one item list per compute task C-i-j ----------
+    p->goo_bwd_task.assign((size_t)p->k_q * p->k_kv, SegList{0, 0});
+    for (int i = 0; i < p->k_q; ++i)
+        for (int j = 0; j < p->k_kv; ++j) {
+            SegList range{(int32_t)p->goo_bwd_items.size(), 0};
+            for (int bt = 0; bt < gm.batch; ++bt) {
+                SegList sl{(int32_t)p->bwd_segs.size(), 0};
+                for (int ul = 0; ul < gm.a; ++ul) { p->bwd_segs.push_back(Seg{ul, i * Lq, (i + 1) * Lq}); ++sl.count; }
+                const int list_id = (int)p->bwd_seglists.size();
+                p->bwd_seglists.push_back(sl);
+                for (int hk = 0; hk < gm.heads_kv; ++hk) {
+                    std::vector<BwdItem> grp;
+                    for (int jj = 0; jj < gm.b; ++jj)
+                        for (int t0 = j * Lkv; t0 < (j + 1) * Lkv; t0 += kBlock)
+                            grp.push_back(BwdItem{(int16_t)bt, (int16_t)jj, (int16_t)hk, (int16_t)list_id, t0, 0});
+                    if (gm.causal)
+                        std::stable_sort(grp.begin(), grp.end(), [](const BwdItem& x, const BwdItem& y) { return x.t0 < y.t0; });
+                    p->goo_bwd_items.insert(p->goo_bwd_items.end(), grp.begin(), grp.end());
+                }
+            }
+            range.count = (int32_t)p->goo_bwd_items.size() - range.offset;
+            p->goo_bwd_task[(size_t)i * p->k_kv + j] = range;
+        }
 }
 
 // First Q block of segment sg that item (kv_local, t0) of simulated GPU g visits (the rule of tile_bwd.cu's QWalk).
