@@ -29,9 +29,43 @@ if str(ROOT) not in sys.path:
 METRIC = "attention_fwd_bwd_tflops"
 UNIT = "TFLOP/s"
 FALLBACK_PEAKS = {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0}
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from one ncu capture of this command
-# (profiles/r01_v6_traffic_c5_tile_bwd.csv; profiles/r01_v6_ncu_c2_bwd.txt, r01_v5_ncu_c2_fwd.txt): workload -> kernel -> bytes
-NCU_TRAFFIC = {"C5": {"tile_bwd": 2134681542144 + 1102663412992}, "C2": {"tile_bwd": 3047004000 + 1805074000, "tile_fwd": 908874752 + 569961216}}
+
+
+def load_traffic(workload: str, kernel: str):
+    """roofline.traffic = dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of `kernel` on `workload`, read from the
+    newest ncu capture under profiles/ (`*_traffic_<workload>_<kernel>.csv`, written by `ncu --csv --metrics dram__bytes_read.sum,
+    dram__bytes_write.sum,...`; its sidecar `.md` names the command, the commit and the hash of the kernel sources it was taken
+    at).  Nothing is embedded in this file: no capture -> (None, reason)."""
+    import csv
+    import re
+
+    from paper_2512_20968_b200.build import kernel_source_hash
+
+    files = sorted((ROOT / "profiles").glob(f"*_traffic_{workload.lower()}_{kernel}.csv"),
+                   key=lambda f: [int(x) for x in re.findall(r"\d+", f.name)[:2]])
+    if not files:
+        return None, {"reason": f"no profiles/*_traffic_{workload.lower()}_{kernel}.csv capture for this workload and kernel"}
+    f = files[-1]
+    vals = {}
+    with open(f, newline="") as fh:
+        for row in csv.DictReader(fh):
+            try:
+                vals[row["Metric Name"]] = float(row["Metric Value"].replace(",", ""))
+            except (KeyError, ValueError, TypeError):
+                continue
+    if "dram__bytes_read.sum" not in vals or "dram__bytes_write.sum" not in vals:
+        return None, {"reason": f"{f.name} holds no dram__bytes_read.sum / dram__bytes_write.sum"}
+    src = {"file": f"profiles/{f.name}", "dram_read_bytes": vals["dram__bytes_read.sum"], "dram_write_bytes": vals["dram__bytes_write.sum"]}
+    if "lts__t_sector_hit_rate.pct" in vals:
+        src["l2_hit_pct"] = vals["lts__t_sector_hit_rate.pct"]
+    side = f.with_suffix(".md")
+    meta = side.read_text() if side.exists() else ""
+    for key in ("commit", "kernel_sha16"):
+        m = re.search(rf"^{key}:\s*(\S+)", meta, flags=re.M)
+        src[key] = m.group(1) if m else "unrecorded (captured before the sidecar files existed)"
+    src["kernel_sha16_now"] = kernel_source_hash(kernel)
+    src["matches_current_kernel"] = src["kernel_sha16"] == src["kernel_sha16_now"]
+    return vals["dram__bytes_read.sum"] + vals["dram__bytes_write.sum"], src
 
 
 def parse_args():
@@ -46,6 +80,9 @@ def parse_args():
     ap.add_argument("--goo-executor", type=int, default=-1, metavar="R",
                     help="separate mode (not the driver's bench line): time the GOO executor (mesh_attn_forward_goo) on --workload with every "
                          "communication stand-in copied R times, overlapped vs serialised, against the fused forward")
+    ap.add_argument("--bwd-pairing", type=int, default=0, choices=[0, 1, 2],
+                    help="plan desc field bwd_pairing (A/B runs): 0 auto (2-CTA clusters + dQ exchange), 1 single CTAs, 2 clusters without the exchange")
+    ap.add_argument("--bwd-piece-blocks", type=int, default=0, help="plan desc field bwd_piece_blocks (A/B runs): Q blocks per tile_bwd work item, 0 = default")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -141,10 +178,12 @@ def oracle_inputs_from_device(w, inp):
 
 class OracleSample:
     """The oracle as it stands (oracle/attn_oracle.py, fp64, OpenMP over sampled rows) on a bounded sample of the
-    workload: R random query rows of query head 0 -> forward (O, LSE from the definition) and, for workloads with a
-    backward pass, the query-side backward (LSE, Delta, dQ).  Algorithmic FLOPs counted for the sample: 4*D per
-    visible (q,k) pair forward; 6*D backward (the S, dP and dQ contractions; the key-side dK/dV sums, 4*D, need
-    every query row per key and are not in the sample)."""
+    workload: R random query rows of query head 0 -> forward (O, LSE from the definition), the query-side backward
+    (LSE, Delta, dQ) and the key-side backward (dK, dV of KSAMPLE random keys, summed over those R rows).  Algorithmic FLOPs
+    of the sample: 4*D per visible (q,k) pair forward, 6*D query side (the S, dP and dQ contractions), 4*D per visible pair
+    of the (R rows x KSAMPLE keys) key-side sample (the dV and dK contractions): all 10*D of the backward are sampled."""
+
+    KSAMPLE = 8192
 
     def __init__(self, w, host, seconds: float):
         import numpy as np
@@ -156,6 +195,7 @@ class OracleSample:
         self.threads = oracle.num_threads()
         self.pos = oracle.positions(w.n, w.L, w.seq_layout)
         self.rng = np.random.default_rng(20968)
+        self.last = {}
         dt, _ = self.run(self.rows(self.threads))                      # calibration pass
         per_round = max(dt, 1e-3)
         self.R = int(max(1, min(4096, round(seconds / per_round)))) * self.threads
@@ -166,21 +206,58 @@ class OracleSample:
     def run(self, rows):
         np, w, h = self.np, self.w, self.host
         heads = np.zeros(len(rows), dtype=np.int32)
+        D = w.head_dim
         t0 = time.perf_counter()
         self.oracle.fwd_rows(h["q"], h["k"], h["v"], w.scale, w.causal, self.pos, rows, heads)
+        t1 = time.perf_counter()
+        vis = int((self.pos[rows] + 1).sum()) if w.causal else len(rows) * w.seq_total
+        flops = vis * D * 4.0
+        part = {"rows": len(rows), "pairs_rows": vis, "s_fwd": t1 - t0, "s_dq": 0.0, "s_dkv_call": 0.0, "pairs_keys": 0}
         if w.backward:
             self.oracle.bwd_dq_rows(h["q"], h["k"], h["v"], h["do"], w.scale, w.causal, self.pos, rows, heads)
-        dt = time.perf_counter() - t0
-        vis = int((self.pos[rows] + 1).sum()) if w.causal else len(rows) * w.seq_total
-        return dt, vis * w.head_dim * (4.0 + (6.0 if w.backward else 0.0))
+            t2 = time.perf_counter()
+            keys = np.sort(self.rng.integers(0, w.seq_total, min(self.KSAMPLE, w.seq_total))).astype(np.int64)
+            # query head 0 only: a one-head view keeps the key side at the sampled head (GQA: head 0 of KV head 0's group)
+            q1, do1 = h["q"][:, :1], h["do"][:, :1]
+            self.oracle.bwd_dkv_keys(q1, h["k"], h["v"], do1, w.scale, w.causal, self.pos, keys, np.zeros(len(keys), np.int32), qs_rows=rows)
+            t3 = time.perf_counter()
+            if w.causal:
+                pk = np.sort(self.pos[keys])
+                vis_k = int(np.searchsorted(pk, self.pos[rows], side="right").sum())     # keys of the sample each sampled row sees
+            else:
+                vis_k = len(rows) * len(keys)
+            flops += vis * D * 6.0 + vis_k * D * 4.0
+            part.update(s_dq=t2 - t1, s_dkv_call=t3 - t2, pairs_keys=vis_k)
+        self.last = part
+        return time.perf_counter() - t0, flops
 
     def timed(self):
         dt, flops = self.run(self.rows(self.R))
         return dt, flops
 
+    def extrapolate(self):
+        """Full-problem time of the oracle from the last sample: each leg scaled by (all visible pairs x all query heads) /
+        (the pairs that leg sampled).  bwd_dkv_keys recomputes LSE and Delta of its query rows with bwd_dq_rows before its
+        own loop (the oracle as it stands), so its call is split into that pass (it scales with the rows) and the key-side
+        loop proper (it scales with the (row, key) pairs)."""
+        w, p = self.w, self.last
+        if not p or not p["pairs_rows"]:
+            return {}
+        all_pairs = float(w.visible_pairs()) * w.heads_q * w.batch
+        per_row_legs = p["s_fwd"] + p["s_dq"] + (min(p["s_dq"], p["s_dkv_call"]) if w.backward else 0.0)
+        sec = per_row_legs * all_pairs / p["pairs_rows"]
+        if w.backward and p["pairs_keys"]:
+            sec += max(p["s_dkv_call"] - p["s_dq"], 0.0) * all_pairs / p["pairs_keys"]
+        fl = w.flops_fwd() + (w.flops_bwd() if w.backward else 0.0)
+        return {"extrapolated_full_problem_seconds": sec, "extrapolated_tokens_per_s": w.seq_total * w.batch / sec,
+                "extrapolated_tflops": fl / sec / 1e12, "sample_seconds": {k: p[k] for k in ("s_fwd", "s_dq", "s_dkv_call")},
+                "sampled_pairs": {"query_rows_x_all_keys": p["pairs_rows"], "query_rows_x_sampled_keys": p["pairs_keys"]},
+                "all_visible_pairs_x_heads": all_pairs}
+
     def describe(self):
         return (f"{self.R} random query rows of head 0 of {self.w.name}: fp64 forward rows"
-                + (" + query-side backward rows (dQ, Delta)" if self.w.backward else "") + ", all keys")
+                + (f" + query-side backward rows (dQ, Delta), all keys + key-side backward (dK, dV) of {min(self.KSAMPLE, self.w.seq_total)} random keys over those rows"
+                   if self.w.backward else "") + "; all keys for the row legs")
 
 
 def run_reference(args):
@@ -205,7 +282,7 @@ def run_reference(args):
         "warmup": args.warmup, "ms_per_step": 1e3 * tot_t / max(1, args.steps), "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "config": workload_config(w, "oracle sample per step: " + smp.describe()),
-        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.threads, "kind": "oracle", "sample": smp.describe()},
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": smp.threads, "kind": "oracle", "sample": smp.describe(), **smp.extrapolate()},
         "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -264,12 +341,16 @@ def alloc_host(shape, dtype, torch):
 
 def run_e2e(plan, w, inp, buf, torch, steps):
     """The public host-buffer call (mesh_attn_step_host): H2D of Q,K,V(,dO), the whole hot path, D2H of O, LSE
-    (and dQ,dK,dV), all inside the timed region."""
-    host_in, host_out, pinned = {}, {}, True
+    (and dQ,dK,dV), all inside the timed region.  The device staging buffers are SEPARATE from the resident inputs and
+    NaN-filled before every timed call, so the kernels can only have seen what the timed copies brought; afterwards the O that
+    came back to the host is compared bit for bit with a device-resident forward on the original inputs (the forward has no
+    atomics: same bits), which proves the copy -> kernel -> copy chain of the timed call."""
+    host_in, host_out, stage, pinned = {}, {}, {}, True
     for k, t in inp.items():
         host_in[k], p = alloc_host(t.shape, t.dtype, torch)
         pinned &= p
         host_in[k].copy_(t)
+        stage[k] = torch.empty_like(t)
     outs = {"O": buf.O, "lse": buf.lse}
     if w.backward:
         outs.update(dQ=buf.dQ, dK=buf.dK, dV=buf.dV)
@@ -278,22 +359,38 @@ def run_e2e(plan, w, inp, buf, torch, steps):
         pinned &= p
         host_out[k].zero_()                                   # touch the pages before timing
     kw = dict(Q_host=host_in["q"], K_host=host_in["k"], V_host=host_in["v"], O_host=host_out["O"], lse_host=host_out["lse"],
-              d_Q=inp["q"], d_K=inp["k"], d_V=inp["v"], d_O=buf.O, d_lse=buf.lse, d_partial_O=buf.partial_O,
+              d_Q=stage["q"], d_K=stage["k"], d_V=stage["v"], d_O=buf.O, d_lse=buf.lse, d_partial_O=buf.partial_O,
               d_partial_lse=buf.partial_lse)
     if w.backward:
-        kw.update(dO_host=host_in["do"], dQ_host=host_out["dQ"], dK_host=host_out["dK"], dV_host=host_out["dV"], d_dO=inp["do"],
+        kw.update(dO_host=host_in["do"], dQ_host=host_out["dQ"], dK_host=host_out["dK"], dV_host=host_out["dV"], d_dO=stage["do"],
                   d_bwd_ws=buf.bwd_ws, d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    ms = 0.0
     for _ in range(steps):
+        for t in stage.values():
+            t.view(torch.int16).fill_(0x7FC0)                 # bf16 NaN: nothing of the resident inputs survives in the staging
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
         plan.step_host(**kw)                                  # synchronises its stream before returning
-    e1.record()
-    torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / steps
+        e1.record()
+        torch.cuda.synchronize()
+        ms += e0.elapsed_time(e1)
+    ms /= steps
     h2d = sum(t.numel() * t.element_size() for t in host_in.values())
     d2h = sum(t.numel() * t.element_size() for t in host_out.values())
-    return ms, h2d, d2h, pinned
+    # ---- check: the staging now holds the inputs, and the host O equals a resident forward's O
+    checked = all(torch.equal(stage[k].view(torch.int16), inp[k].view(torch.int16)) for k in inp)
+    del stage
+    plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+    torch.cuda.synchronize()
+    rows = 1 << 15
+    for r0 in range(0, w.seq_total, rows):
+        r1 = min(w.seq_total, r0 + rows)
+        checked = checked and bool(torch.equal(host_out["O"][:, r0:r1].cuda(), buf.O[:, r0:r1]))
+    if w.backward:                                            # atomics reorder the gradient sums: finite and non-trivial is what can be said
+        checked = checked and all(bool(torch.isfinite(host_out[k][:, :rows]).all().item()) and bool(host_out[k][:, :rows].abs().max().item() > 0)
+                                  for k in ("dQ", "dK", "dV"))
+    return ms, h2d, d2h, pinned, checked
 
 
 def run_ours(args):
@@ -328,7 +425,7 @@ def run_ours(args):
     w = W.CONFIGS[args.workload]
     peaks, peak_src = load_peaks()
     inp = W.make_inputs(w, "cuda", ("q", "k", "v", "do") if w.backward else ("q", "k", "v"))
-    plan = plan_for(w, usp_lanes=args.usp_lanes)
+    plan = plan_for(w, usp_lanes=args.usp_lanes, bwd_pairing=args.bwd_pairing, bwd_piece_blocks=args.bwd_piece_blocks)
     buf = Buffers(plan, w, backward=w.backward)
 
     def step():
@@ -372,12 +469,14 @@ def run_ours(args):
     if not args.no_e2e:
         try:
             e2e_steps = 1 if ms_total / K > 2000 else min(K, 5)
-            ms_e, h2d, d2h, pinned = run_e2e(plan, w, inp, buf, torch, e2e_steps)
+            ms_e, h2d, d2h, pinned, checked = run_e2e(plan, w, inp, buf, torch, e2e_steps)
             ms_e = max_over_ranks(ms_e, dist, "cuda")
             e2e = {"value": whole_job_tflops(fl_fwd + fl_bwd, world, 1, ms_e), "unit": UNIT, "h2d_bytes_per_step": h2d,
                    "d2h_bytes_per_step": d2h, "ms_per_step": ms_e, "steps": e2e_steps, "pinned": pinned,
-                   "api": "mesh_attn_step_host"}
-        except (RuntimeError, MemoryError) as ex:                # host memory too small for the host mirrors
+                   "api": "mesh_attn_step_host", "checked": checked,
+                   "check": "device staging separate from the resident inputs and NaN-filled before the timed call; afterwards staging == inputs "
+                            "and the host O == a resident forward's O bit for bit; host gradients finite and non-zero"}
+        except (RuntimeError, MemoryError) as ex:                # host or device memory too small for the mirrors / the staging
             e2e = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0, "error": str(ex)[:200]}
     if rank != 0:
         if dist is not None:
@@ -391,8 +490,9 @@ def run_ours(args):
     long_step = sec >= 2.0
     peak = peaks["bf16_tflops_sustained"] if long_step else peaks["bf16_tflops"]
     ach = dom_flops / (dom_ms / 1e3) / 1e12 if dom_ms > 0 else 0.0
+    traffic, traffic_src = load_traffic(w.name, dom)
     roofline = {"kernel": f"mesh_attn_{dom}", "bound": "tensor", "achieved": ach, "peak": peak, "unit": "TFLOP/s",
-                "frac": ach / peak, "traffic": NCU_TRAFFIC.get(w.name, {}).get(dom), "launches": dom_n, "avg_launch_ms": dom_ms / max(1, dom_n),
+                "frac": ach / peak, "traffic": traffic, "traffic_source": traffic_src, "launches": dom_n, "avg_launch_ms": dom_ms / max(1, dom_n),
                 "algorithmic_flops_per_launch": dom_flops / max(1, dom_n),
                 "peak_kind": f"{peak_src} dense bf16, " + ("sustained (kernel timed inside a long step)" if long_step else "burst"),
                 "share_of_step": dom_ms / ms_total}
@@ -422,7 +522,7 @@ def run_ours(args):
         smp = OracleSample(w, oracle_inputs_from_device(w, inp), args.cpu_seconds)
         dt, fl = smp.timed()
         cpu = {"value": fl / dt / 1e12, "unit": UNIT, "cores": smp.threads, "kind": "oracle", "sample": smp.describe(),
-               "seconds": dt}
+               "seconds": dt, **smp.extrapolate()}
 
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": args.warmup,
@@ -433,6 +533,7 @@ def run_ours(args):
     }
     if args.usp_lanes > 1:
         line["config"]["usp_lanes"] = args.usp_lanes
+    line["config"]["tile_bwd_kernel"] = {0: "single CTAs", 1: "2-CTA clusters, shared Q/dO tile loads", 2: "2-CTA clusters, shared tile loads + dQ exchange"}[plan.query(B.Q_BWD_PAIRED)]
     print(json.dumps(line), flush=True)
     if dist is not None:
         dist.destroy_process_group()
@@ -484,7 +585,7 @@ def run_goo_executor(args):
     steps = plan.steps()
     line = {
         "mode": "goo_executor", "config": workload_config(w), "comm_repeat": R,
-        "comm_bytes_per_q_group": plan.query(B.Q_GOO_COMM_BYTES), "steps": int(steps[:, 0].max()) + 1 if len(steps) else 0,
+        "comm_bytes_per_q_group": plan.query(B.Q_GOO_COMM_BYTES), "steps": int(steps[:, 0].max()) if len(steps) else 0,   # step numbers are 1-based
         "compute_tasks_per_q_group": w.k_q * w.k_kv,
         "ms": {"fused_forward": t_fused, "executor_no_comm": t_compute, "executor_overlapped": t_overlap, "executor_serialised": t_serial},
         "exposed_comm_ms": {"overlapped": t_overlap - t_compute, "serialised": t_serial - t_compute},

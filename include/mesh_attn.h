@@ -23,8 +23,8 @@
  *     everything is enqueued on `stream`.
  *   - Every function returns a mesh_attn_status (0 = OK, negative = error) and never
  *     throws or aborts; mesh_attn_last_error() gives a thread-local detail string.
- *   - There is no CPU fallback: on a machine without a CUDA device the planner calls
- *     work, every compute call returns MESH_ATTN_ECUDA.
+ *   - There is no CPU fallback: on a machine without an sm_100 CUDA device (none at all, or another
+ *     architecture) the planner calls work, every compute call returns MESH_ATTN_ECUDA.
  *
  * Tensor layouts (rows in PARTITION-MAJOR order: partition p, local row s -> row p*L+s,
  * L = seq_total / n):
@@ -49,7 +49,12 @@
 extern "C" {
 #endif
 
-typedef struct mesh_attn_plan mesh_attn_plan; /* opaque, library-owned, immutable after create */
+typedef struct mesh_attn_plan mesh_attn_plan; /* opaque, library-owned, immutable after create.  A plan serves ONE in-flight
+                                                 call at a time: mesh_attn_step_host and the *_goo executors order their copies
+                                                 with plan-owned streams and events, so two concurrent calls on the same plan
+                                                 (from two host threads or two caller streams) would race on them; use one plan
+                                                 per concurrent caller (plans are cheap).  The profiling calls are process-global
+                                                 and not thread-safe. */
 
 typedef enum {
     MESH_ATTN_OK = 0,
@@ -81,7 +86,18 @@ typedef struct {
                                  Mesh-Attention on its own a x b mesh.  There are n*U simulated GPUs: g in [0, n*U) is
                                  mesh GPU g % n of lane g / n; Q group q in [0, b*U) is group q % b of lane q / b.
                                  The partial workspace of a simulated GPU shrinks by U.  heads_kv % U == 0.   */
-    int32_t reserved[4];      /* must be 0                                                             */
+    int32_t bwd_pairing;      /* tile_bwd as 2-CTA clusters over work items 2k, 2k+1 (MESH_ATTN_Q_BWD_PAIRED): 0 auto (paired when the
+                                 planner finds the items pairable: shared Q / dO tile loads AND the pair's dQ exchange, which
+                                 halves the dQ atomics; precision 1 pairs without the exchange), 1 never (single-CTA kernel),
+                                 2 paired, shared tile loads only (no dQ exchange).  1 and 2 exist for A/B measurements
+                                 and for callers that want the dQ sums free of the exchange's bf16 rounding */
+    int32_t bwd_piece_blocks; /* tile_bwd work items: > 0 cuts the Q sweep of a 128-key block (all Q partitions of the tile) into pieces of
+                                 at most this many 128-row Q blocks (whole segments = Q chunks of one partition), one work item per
+                                 (key block, piece), the key blocks of a piece adjacent in the list; 0 (default) = one item per key
+                                 block.  Short sweeps keep the Q / dO / dQ rows the running CTAs share in L2, very short ones pay the
+                                 per-item K / V load and dK / dV epilogue more often (measured: DESIGN.md 6.3).  The results are
+                                 the same sums in another order.                                                       */
+    int32_t reserved[2];      /* must be 0                                                             */
 } mesh_attn_plan_desc;
 
 /* what = ... for mesh_attn_plan_query */
@@ -107,8 +123,8 @@ enum {
     MESH_ATTN_Q_USP_LANES = 16,            /* U                                                                          */
     MESH_ATTN_Q_BWD_PAIRED = 18,           /* 1 if tile_bwd runs as 2-CTA clusters sharing the Q / dO tile loads: backward work items
                                               2k and 2k+1 visit the same Q blocks on every simulated GPU (holds for non-causal and
-                                              striped-causal plans with an even item count; MESH_ATTN_NO_PAIR=1 in the environment
-                                              at plan_create forces 0) */
+                                              striped-causal plans with an even item count; desc.bwd_pairing = 1 forces 0); 2 if the
+                                              pair also exchanges dQ partial sums (half the dQ atomics) */
     MESH_ATTN_Q_GOO_PARTIAL_O_BYTES = 19,  /* mesh_attn_forward_goo: bytes of partial_O for ONE simulated GPU (a*k_kv slots); x a */
     MESH_ATTN_Q_GOO_PARTIAL_LSE_BYTES = 20,
     MESH_ATTN_Q_GOO_COMM_BYTES = 21,       /* bytes the forward step list's collectives move for the a GPUs of one Q group:
@@ -313,6 +329,14 @@ typedef struct {
     float *d_O, *d_lse, *d_bwd_ws, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;
 } mesh_attn_host_io;
 int mesh_attn_step_host(const mesh_attn_plan* plan, const mesh_attn_host_io* io, void* stream);
+
+/* Kernel watchdog.  Every wait inside the tile kernels is bounded (~4 s): a wait that does not complete is a protocol bug,
+ * and instead of hanging the GPU or trapping (which would destroy the caller's CUDA context) the kernel records the fault in
+ * status words owned by the plan (pinned host memory mapped into the device) and runs to its end with invalid results.
+ * Every hot call checks those words on entry and mesh_attn_step_host after its synchronisation; mesh_attn_plan_health
+ * checks them on demand (call it after synchronising the stream): MESH_ATTN_OK, or MESH_ATTN_ECUDA with the block, thread
+ * and barrier in mesh_attn_last_error().  A faulted plan stays faulted: destroy it.  Host-only plans are always OK. */
+int mesh_attn_plan_health(const mesh_attn_plan* plan);
 
 /* number of kernels launched by this library in the calling process so far (bench bookkeeping) */
 int64_t mesh_attn_launch_count(void);

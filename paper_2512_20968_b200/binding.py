@@ -37,7 +37,7 @@ class PlanDesc(C.Structure):
         ("gamma", C.c_float), ("t_ag_q", C.c_float), ("t_ag_kv", C.c_float), ("t_rs_q", C.c_float), ("t_c", C.c_float),
         ("softmax_scale", C.c_float),
         ("tensor_layout", C.c_int32), ("partial_mode", C.c_int32), ("precision", C.c_int32),
-        ("usp_lanes", C.c_int32), ("reserved", C.c_int32 * 4),
+        ("usp_lanes", C.c_int32), ("bwd_pairing", C.c_int32), ("bwd_piece_blocks", C.c_int32), ("reserved", C.c_int32 * 2),
     ]
 
 
@@ -74,6 +74,7 @@ lib.mesh_attn_rank_bwd_preprocess.argtypes = [_P] * 6
 lib.mesh_attn_rank_sum_peers.argtypes = [_P, C.POINTER(_P), C.c_int32, C.c_int64, _P, _P]
 lib.mesh_attn_rank_bwd.argtypes = [_P, C.c_int32] + [_P] * 9
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
+lib.mesh_attn_plan_health.argtypes = [_P]
 lib.mesh_attn_launch_count.restype = C.c_int64
 lib.mesh_attn_profile_enable.argtypes = [C.c_int32, C.c_int32]
 lib.mesh_attn_profile_read.argtypes = [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -84,7 +85,7 @@ lib.mesh_attn_last_error.restype = C.c_char_p
 EXPORTED = [
     "mesh_attn_plan_create", "mesh_attn_plan_destroy", "mesh_attn_plan_am", "mesh_attn_plan_footprint", "mesh_attn_plan_tiles",
     "mesh_attn_plan_steps", "mesh_attn_plan_query", "mesh_attn_plan_tam_units", "mesh_attn_plan_timeline", "mesh_attn_tile_fwd", "mesh_attn_merge", "mesh_attn_bwd_preprocess",
-    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count",
+    "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count", "mesh_attn_plan_health",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
     "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_sum_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
 ]
@@ -148,6 +149,10 @@ class Plan:
         v = C.c_int64()
         _check(lib.mesh_attn_plan_query(self._h, what, C.byref(v)))
         return v.value
+
+    def health(self):
+        """raises MeshAttnError(ECUDA) if a kernel of this plan reported a fault (synchronise the stream first)"""
+        _check(lib.mesh_attn_plan_health(self._h))
 
     def timeline(self, backward: bool = False):
         """(makespan, serial time, exposed communication) of the step list in the plan's cost units"""

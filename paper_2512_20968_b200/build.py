@@ -66,5 +66,21 @@ def build(force: bool = False, verbose: bool = False) -> Path:
     return LIB
 
 
+def kernel_source_hash(kernel: str) -> str:
+    """sha256 (first 16 hex digits) of the sources that define `kernel` ("tile_fwd", "tile_bwd", "merge", ...): its .cu file and
+    the shared headers.  profiles/*_traffic_*.md record it, so that bench.py can say whether a stored ncu capture still
+    describes the kernel that runs."""
+    import hashlib
+
+    main = {"tile_fwd": "tile_fwd.cu", "tile_bwd": "tile_bwd.cu"}.get(kernel, "aux_kernels.cu")
+    h = hashlib.sha256()
+    for name in (main, "sm100.cuh", "tile_kernels.hpp", "plan.hpp"):
+        h.update((CSRC / name).read_bytes())
+    return h.hexdigest()[:16]
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--hash" in sys.argv:
+        print(kernel_source_hash(sys.argv[sys.argv.index("--hash") + 1]))
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

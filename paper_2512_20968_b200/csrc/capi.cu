@@ -88,11 +88,26 @@ struct ProfScope {                   // records begin at construction, end at de
     }
 };
 
+// a kernel of this plan reported a fault through its status words (sm100.cuh watchdog): every later call fails loudly
+int check_health(const mesh_attn_plan* p, const char* who)
+{
+    if (!p->h_status) return MESH_ATTN_OK;
+    const volatile int* st = p->h_status;
+    if (st[0] == 0) return MESH_ATTN_OK;
+    char buf[256];
+    if (st[0] == 1)
+        std::snprintf(buf, sizeof buf, ": an earlier kernel of this plan timed out in an mbarrier wait (block %d, thread %d, barrier 0x%x, parity %d); "
+                      "its results are invalid; destroy the plan", st[1], st[2], (unsigned)st[3], st[4]);
+    else
+        std::snprintf(buf, sizeof buf, ": an earlier kernel of this plan found its dynamic shared memory misaligned (block %d) and did not run", st[1]);
+    return fail(MESH_ATTN_ECUDA, std::string(who) + buf);
+}
+
 int check_device(const mesh_attn_plan* p, const char* who)
 {
     if (!p) return fail(MESH_ATTN_EINVAL, std::string(who) + ": null plan");
-    if (!p->d_blob) return fail(MESH_ATTN_ECUDA, std::string(who) + ": plan has no device work lists (no CUDA device at plan_create); there is no CPU fallback");
-    return MESH_ATTN_OK;
+    if (!p->d_blob) return fail(MESH_ATTN_ECUDA, std::string(who) + ": plan has no device work lists (no sm_100 CUDA device at plan_create); there is no CPU fallback");
+    return check_health(p, who);
 }
 }  // namespace
 
@@ -110,7 +125,7 @@ int upload_plan(mesh_attn_plan* p)
     if (cudaGetDevice(&dev) != cudaSuccess) return cuda_fail("cudaGetDevice", (int)cudaGetLastError());
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return cuda_fail("cudaGetDeviceProperties", (int)cudaGetLastError());
-    if (prop.major != 10) return fail(MESH_ATTN_EUNSUPPORTED, "plan_create: kernels are built for sm_100a (B200) only");
+    if (prop.major != 10) return MESH_ATTN_OK;   // not a B200: like no device at all -- a host-only plan whose compute calls return ECUDA
     p->device = dev;
     p->num_sms = prop.multiProcessorCount;
     auto al = [](size_t x) { return (x + 255) & ~size_t(255); };
@@ -124,7 +139,7 @@ int upload_plan(mesh_attn_plan* p)
     p->d_blob = d;
     auto put = [&](const void* src, size_t bytes, size_t cap) {
         char* at = d;
-        if (bytes) e = cudaMemcpy(at, src, bytes, cudaMemcpyHostToDevice);
+        if (bytes && e == cudaSuccess) e = cudaMemcpy(at, src, bytes, cudaMemcpyHostToDevice);   // the first error is the one reported
         d += cap;
         return at;
     };
@@ -137,6 +152,13 @@ int upload_plan(mesh_attn_plan* p)
     p->d_goo_items = (const FwdItem*)put(p->goo_items.data(), p->goo_items.size() * sizeof(FwdItem), b6);
     p->d_goo_bwd_items = (const BwdItem*)put(p->goo_bwd_items.data(), p->goo_bwd_items.size() * sizeof(BwdItem), b7);
     if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
+    // watchdog status words: pinned host memory the kernels write through its device mapping (no host sync needed to read it)
+    e = cudaHostAlloc((void**)&p->h_status, 8 * sizeof(int), cudaHostAllocMapped);
+    if (e == cudaSuccess) {
+        std::memset(p->h_status, 0, 8 * sizeof(int));
+        e = cudaHostGetDevicePointer((void**)&p->d_status, p->h_status, 0);
+    }
+    if (e != cudaSuccess) { free_plan_device(p); return cuda_fail("plan_create: status words", (int)e); }
     // step_host's copy engines: one stream per direction, events for the chunk hand-offs
     cudaStream_t s0 = nullptr, s1 = nullptr;
     e = cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking);
@@ -155,6 +177,8 @@ void free_plan_device(mesh_attn_plan* p)
 {
     if (p->d_blob) cudaFree(p->d_blob);
     p->d_blob = nullptr;
+    if (p->h_status) cudaFreeHost(p->h_status);
+    p->h_status = p->d_status = nullptr;
     for (void* ev : p->copy_events) cudaEventDestroy((cudaEvent_t)ev);
     p->copy_events.clear();
     if (p->s_h2d) cudaStreamDestroy((cudaStream_t)p->s_h2d);
@@ -195,6 +219,7 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
     fp.split = p->desc.precision;
     fp.partial_O = partial_O;
     fp.partial_lse = partial_lse;
+    fp.status = p->d_status;
     ProfScope prof(MESH_ATTN_K_TILE_FWD, (cudaStream_t)stream);
     const int e = launch_tile_fwd(fp, tmQ, tmK, tmV, p->num_sms, (cudaStream_t)stream);
     if (e) return cuda_fail(who, e);
@@ -292,13 +317,13 @@ static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count,
     dK = head_slice(dK, ln.hk0, sdk, 4);
     dV = head_slice(dV, ln.hk0, sdk, 4);
     // paired items (2-CTA clusters): each CTA loads 64-row halves of the Q / dO tiles and multicasts them
-    const bool pair = !own_list && p->bwd_pairable && ((long long)g_count * (long long)items_per_gpu) >= 2 && !p->no_pair;
+    const int pair = (!own_list && ((long long)g_count * (long long)items_per_gpu) >= 2) ? p->bwd_pair_mode() : 0;
     const int qbox = pair ? kBlock / 2 : kBlock;
     if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox, N) ||
         !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, Nk) ||
         !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, Nk) ||
         !make_map(p, &tmdO, dO, p->geom.heads_q, p->desc.heads_q, ln.hq0, qbox, N) ||
-        !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)N, p->geom.batch, sdq.h * 4, sdq.row * 4, sdq.b * 4, 16))
+        !make_tmap_f32_4d(&tmdQ, dQ, p->geom.head_dim, p->geom.heads_q, (uint64_t)N, p->geom.batch, sdq.h * 4, sdq.row * 4, sdq.b * 4, pair == 2 ? kBwdStgRowsExch : kBwdStgRows))
         return fail(MESH_ATTN_ECUDA, "tile_bwd: cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     BwdParams bp;
     bp.gm = p->geom;
@@ -310,7 +335,8 @@ static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count,
     bp.g_first = g_first % p->geom.n;
     bp.g_count = g_count;
     bp.split = p->desc.precision;
-    bp.pair = pair ? 1 : 0;
+    bp.pair = pair;
+    bp.status = p->d_status;
     bp.ws = bwd_ws + ln.hq0 * N;
     bp.ws_plane = (long long)p->geom.batch * p->desc.heads_q * N;
     bp.vec_stride_b = (long long)p->desc.heads_q * N;
@@ -708,10 +734,16 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
     if (ok()) e = cudaStreamWaitEvent(st, ev(5), 0);
     if (ok()) e = cudaStreamSynchronize(st);
     if (!ok()) return cuda_fail("step_host D2H", (int)e);
-    return MESH_ATTN_OK;
+    return check_health(p, "step_host");
 }
 
 int64_t mesh_attn_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int mesh_attn_plan_health(const mesh_attn_plan* p)
+{
+    if (!p) return fail(MESH_ATTN_EINVAL, "plan_health: null plan");
+    return check_health(p, "plan_health");
+}
 
 int mesh_attn_profile_enable(int32_t on, int32_t capacity)
 {

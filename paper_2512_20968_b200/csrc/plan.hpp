@@ -121,13 +121,22 @@ struct mesh_attn_plan {
     std::vector<mesh_attn::BwdItem> goo_bwd_items;
     std::vector<mesh_attn::SegList> goo_bwd_task;
     // backward items 2k and 2k+1 visit the same Q blocks on every simulated GPU (tile_bwd then runs 2-CTA clusters that
-    // share the Q / dO tile loads); no_pair = environment override MESH_ATTN_NO_PAIR=1 (A/B measurements)
-    bool bwd_pairable = false, no_pair = false;
+    // share the Q / dO tile loads); desc.bwd_pairing selects never / shared loads only / shared loads + dQ exchange
+    bool bwd_pairable = false;
+    int bwd_pair_mode() const    // 0 single-CTA kernel, 1 paired (multicast Q / dO tiles), 2 paired + dQ exchange
+    {
+        if (!bwd_pairable || desc.bwd_pairing == 1) return 0;
+        return (desc.bwd_pairing == 2 || desc.precision == 1) ? 1 : 2;
+    }
 
     // device copies (null when no CUDA device was present at creation)
     int device = -1;
     int num_sms = 0;
     void* d_blob = nullptr;
+    // status words of the kernels' watchdog (sm100.cuh): pinned host memory mapped into the device; [0] != 0 = a kernel of this
+    // plan reported a fault (1: mbarrier wait timed out, 2: misaligned shared memory), [1..4] = block, thread, barrier, parity
+    int* h_status = nullptr;
+    int* d_status = nullptr;
     const mesh_attn::FwdItem* d_fwd_items = nullptr;
     const mesh_attn::FwdItem* d_goo_items = nullptr;
     const mesh_attn::BwdItem* d_goo_bwd_items = nullptr;

@@ -12,7 +12,6 @@
 // No CUDA calls here except through mesh_attn::upload_plan (capi.cu).
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <set>
@@ -140,25 +139,30 @@ void build_worklists(mesh_attn_plan* p)
     // Q chunks in order of first appearance in the compute order; for Q chunk i the KV chunks
     // in the order C-i-j tasks execute.
     const std::vector<int> q_chunks = first_appearance<int>(p->order_fwd, true);
+    // seg lists: fused mode -> one list per Q chunk (all b partitions per KV chunk, partition-major inside a
+    // chunk as in tile_list); per-pair mode -> one list per (Q chunk, kv_local).  They do not depend on the batch
+    // index: built once (FwdItem::seglist is 16 bits; plan_create rejects plans with more than 32767 lists).
+    const int n_lists = per_pair ? gm.b : 1;
+    std::vector<std::vector<int>> fwd_list_ids(p->k_q);
+    for (int i : q_chunks) {
+        std::vector<int> kv_chunks;
+        for (auto& t : p->order_fwd) if (t.first == i) kv_chunks.push_back(t.second);
+        fwd_list_ids[i].resize(n_lists);
+        for (int l = 0; l < n_lists; ++l) {
+            SegList sl{(int32_t)p->fwd_segs.size(), 0};
+            for (int j : kv_chunks)
+                for (int jj = 0; jj < gm.b; ++jj) {
+                    if (per_pair && jj != l) continue;
+                    p->fwd_segs.push_back(Seg{jj, j * Lkv, (j + 1) * Lkv});
+                    ++sl.count;
+                }
+            fwd_list_ids[i][l] = (int)p->fwd_seglists.size();
+            p->fwd_seglists.push_back(sl);
+        }
+    }
     for (int bt = 0; bt < gm.batch; ++bt)
         for (int i : q_chunks) {
-            std::vector<int> kv_chunks;
-            for (auto& t : p->order_fwd) if (t.first == i) kv_chunks.push_back(t.second);
-            // seg lists: fused mode -> one list (all b partitions per KV chunk, partition-major inside a
-            // chunk as in tile_list); per-pair mode -> one list per kv_local
-            const int n_lists = per_pair ? gm.b : 1;
-            std::vector<int> list_ids(n_lists);
-            for (int l = 0; l < n_lists; ++l) {
-                SegList sl{(int32_t)p->fwd_segs.size(), 0};
-                for (int j : kv_chunks)
-                    for (int jj = 0; jj < gm.b; ++jj) {
-                        if (per_pair && jj != l) continue;
-                        p->fwd_segs.push_back(Seg{jj, j * Lkv, (j + 1) * Lkv});
-                        ++sl.count;
-                    }
-                list_ids[l] = (int)p->fwd_seglists.size();
-                p->fwd_seglists.push_back(sl);
-            }
+            const std::vector<int>& list_ids = fwd_list_ids[i];
             for (int hk = 0; hk < gm.heads_kv; ++hk) {
                 std::vector<FwdItem> grp;
                 for (int l = 0; l < n_lists; ++l)
@@ -216,38 +220,70 @@ void build_worklists(mesh_attn_plan* p)
     }
 
     // ---------- backward: item = (batch, kv_local, kv head, 128-key block) ----------
+    // The Q sweep of a key block (every Q chunk of every Q partition of the tile, in the order the C-i-j tasks of KV chunk j
+    // execute) can be cut into PIECES of at most bwd_piece_blocks 128-row blocks, a piece being a run of consecutive segments; a
+    // work item is (key block, piece), and all key blocks of a (KV chunk, head, piece) are adjacent in the list, so that the
+    // CTAs running at the same time sweep the same few MB of Q / dO / dQ rows.  dK / dV of a key block are then accumulated per
+    // piece and added atomically like every other partial sum (Alg.3 l.7).  Default: one piece (the whole sweep).
+    // Measured (profiles/r02_v1_README.md): on a 131 072-token probe 128-block pieces beat 512-block sweeps by 18 %, at
+    // BASELINE.json configs[4] they do not (864 vs 874 TFLOP/s): there the persistent CTAs, which take items round-robin, drift
+    // apart by many pieces, so the shorter sweep does not make them share L2 lines.
+    const int piece_blocks = p->desc.bwd_piece_blocks > 0 ? p->desc.bwd_piece_blocks : (1 << 30);
     const std::vector<int> kv_chunks_b = first_appearance<int>(p->order_bwd, false);
-    for (int bt = 0; bt < gm.batch; ++bt)
-        for (int j : kv_chunks_b) {
-            std::vector<int> qc;
-            for (auto& t : p->order_bwd) if (t.second == j) qc.push_back(t.first);
+    struct Piece { int list_id, max_end; };
+    std::vector<std::vector<Piece>> bwd_pieces(p->k_kv);   // seg lists per KV chunk, shared by every batch index
+    for (int j : kv_chunks_b) {
+        std::vector<int> qc;
+        for (auto& t : p->order_bwd) if (t.second == j) qc.push_back(t.first);
+        std::vector<Seg> segs;
+        for (int i : qc)
+            for (int ul = 0; ul < gm.a; ++ul) segs.push_back(Seg{ul, i * Lq, (i + 1) * Lq});
+        for (size_t s0 = 0; s0 < segs.size();) {
             SegList sl{(int32_t)p->bwd_segs.size(), 0};
-            for (int i : qc)
-                for (int ul = 0; ul < gm.a; ++ul) { p->bwd_segs.push_back(Seg{ul, i * Lq, (i + 1) * Lq}); ++sl.count; }
-            const int list_id = (int)p->bwd_seglists.size();
-            p->bwd_seglists.push_back(sl);
-            for (int hk = 0; hk < gm.heads_kv; ++hk) {
-                std::vector<BwdItem> grp;
-                for (int jj = 0; jj < gm.b; ++jj)
-                    for (int t0 = j * Lkv; t0 < (j + 1) * Lkv; t0 += kBlock)
-                        grp.push_back(BwdItem{(int16_t)bt, (int16_t)jj, (int16_t)hk, (int16_t)list_id, t0, 0});
-                // causal: early keys are seen by more queries -> longest first
-                if (gm.causal)
-                    std::stable_sort(grp.begin(), grp.end(), [](const BwdItem& x, const BwdItem& y) { return x.t0 < y.t0; });
-                p->bwd_items.insert(p->bwd_items.end(), grp.begin(), grp.end());
+            int blocks = 0, max_end = 0;
+            while (s0 < segs.size() && (sl.count == 0 || blocks + Lq / kBlock <= piece_blocks)) {
+                p->bwd_segs.push_back(segs[s0]);
+                max_end = std::max(max_end, (int)segs[s0].end);
+                blocks += Lq / kBlock;
+                ++sl.count;
+                ++s0;
             }
+            bwd_pieces[j].push_back(Piece{(int)p->bwd_seglists.size(), max_end});
+            p->bwd_seglists.push_back(sl);
         }
+    }
+    for (int bt = 0; bt < gm.batch; ++bt)
+        for (int j : kv_chunks_b)
+            for (int hk = 0; hk < gm.heads_kv; ++hk)
+                for (const Piece& pc : bwd_pieces[j]) {
+                    std::vector<BwdItem> grp;
+                    for (int jj = 0; jj < gm.b; ++jj)
+                        for (int t0 = j * Lkv; t0 < (j + 1) * Lkv; t0 += kBlock) {
+                            // striped causal layout: key row t is seen by the local query rows >= t (offset 0 or -1, plan.hpp
+                            // causal_off), whatever the partitions: a piece that ends at or before t0 has no step for this block
+                            if (gm.causal && gm.striped && t0 >= pc.max_end) continue;
+                            grp.push_back(BwdItem{(int16_t)bt, (int16_t)jj, (int16_t)hk, (int16_t)pc.list_id, t0, 0});
+                        }
+                    // causal: early keys are seen by more queries -> longest first
+                    if (gm.causal)
+                        std::stable_sort(grp.begin(), grp.end(), [](const BwdItem& x, const BwdItem& y) { return x.t0 < y.t0; });
+                    p->bwd_items.insert(p->bwd_items.end(), grp.begin(), grp.end());
+                }
 
     // ---------- backward, chunk-granular (GOO executor): one item list per compute task C-i-j ----------
     p->goo_bwd_task.assign((size_t)p->k_q * p->k_kv, SegList{0, 0});
+    std::vector<int> goo_list_id(p->k_q);                  // the Q rows of chunk i of every Q partition: one list per Q chunk
+    for (int i = 0; i < p->k_q; ++i) {
+        SegList sl{(int32_t)p->bwd_segs.size(), 0};
+        for (int ul = 0; ul < gm.a; ++ul) { p->bwd_segs.push_back(Seg{ul, i * Lq, (i + 1) * Lq}); ++sl.count; }
+        goo_list_id[i] = (int)p->bwd_seglists.size();
+        p->bwd_seglists.push_back(sl);
+    }
     for (int i = 0; i < p->k_q; ++i)
         for (int j = 0; j < p->k_kv; ++j) {
             SegList range{(int32_t)p->goo_bwd_items.size(), 0};
             for (int bt = 0; bt < gm.batch; ++bt) {
-                SegList sl{(int32_t)p->bwd_segs.size(), 0};
-                for (int ul = 0; ul < gm.a; ++ul) { p->bwd_segs.push_back(Seg{ul, i * Lq, (i + 1) * Lq}); ++sl.count; }
-                const int list_id = (int)p->bwd_seglists.size();
-                p->bwd_seglists.push_back(sl);
+                const int list_id = goo_list_id[i];
                 for (int hk = 0; hk < gm.heads_kv; ++hk) {
                     std::vector<BwdItem> grp;
                     for (int jj = 0; jj < gm.b; ++jj)
@@ -334,6 +370,8 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     if (d->head_dim != 64 && d->head_dim != 128) return fail(MESH_ATTN_EUNSUPPORTED, "plan_create: head_dim must be 64 or 128");
     for (int v : {d->causal, d->kvr, d->order, d->seq_layout, d->tensor_layout, d->partial_mode, d->precision})
         if (v != 0 && v != 1) return fail(MESH_ATTN_EINVAL, "plan_create: flag fields must be 0 or 1");
+    if (d->bwd_piece_blocks < 0) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_piece_blocks must be >= 0 (0 = default)");
+    if (d->bwd_pairing < 0 || d->bwd_pairing > 2) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_pairing must be 0 (auto), 1 (never) or 2 (shared tile loads only)");
     for (int v : d->reserved) if (v != 0) return fail(MESH_ATTN_EINVAL, "plan_create: reserved fields must be 0");
     const int k_q = d->k_q <= 0 ? 1 : d->k_q, k_kv = d->k_kv <= 0 ? 1 : d->k_kv;
     if (k_q * k_kv > 16) return fail(MESH_ATTN_EINVAL, "plan_create: k_q*k_kv must be <= 16 (PAPER.md L206)");
@@ -391,7 +429,10 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     }
     build_worklists(p);
     p->bwd_pairable = bwd_items_pairable(p);
-    if (const char* e = std::getenv("MESH_ATTN_NO_PAIR")) p->no_pair = e[0] == '1';
+    if (p->fwd_seglists.size() > 32767 || p->bwd_seglists.size() > 32767) {     // FwdItem / BwdItem::seglist are 16 bits
+        delete p;
+        return fail(MESH_ATTN_EINVAL, "plan_create: too many segment lists (k_q, k_kv, b too large for partial_mode 1)");
+    }
 
     const int rc = upload_plan(p);
     if (rc != MESH_ATTN_OK) { delete p; return rc; }
@@ -586,7 +627,7 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             *value = (int64_t)gm.a * (2ll * p->k_q * (gm.a - 1) * unit_q + 2ll * p->k_kv * (gm.b - 1) * unit_kv);
             break;
         }
-        case MESH_ATTN_Q_BWD_PAIRED: *value = (p->bwd_pairable && !p->no_pair) ? 1 : 0; break;
+        case MESH_ATTN_Q_BWD_PAIRED: *value = p->bwd_pair_mode(); break;
         case MESH_ATTN_Q_USP_A2A_BYTES_FWD: {
             // the GPU holds N/(n U) tokens of all heads before the all-to-all and keeps 1/U of them
             const long double tokens = (long double)gm.batch * gm.n * gm.L / ((long double)gm.n * U);

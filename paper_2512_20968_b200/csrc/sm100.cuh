@@ -7,7 +7,7 @@
 #include <stdint.h>
 
 #ifndef MESH_ATTN_WATCHDOG
-#define MESH_ATTN_WATCHDOG 1   // bounded mbarrier waits: a protocol bug traps instead of hanging the GPU
+#define MESH_ATTN_WATCHDOG 1   // bounded mbarrier waits: a protocol bug is reported to the host instead of hanging the GPU
 #endif
 
 // optional per-phase clock accounting of one thread per role (tuning builds only: -DMESH_ATTN_PHASE_TIMING)
@@ -58,16 +58,42 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity)
         : "memory");
     return ok != 0;
 }
+// Watchdog.  A wait that has not completed after ~4 s is a protocol bug (never seen in a correct run).  It does not
+// trap (a trap kills the caller's CUDA context, and the C ABI promises never to abort): the first thread of the launch
+// to time out records (1, block, thread, barrier, parity) in the launch's status words -- host-mapped memory owned by the
+// plan, which every C-ABI call checks -- and raises the CTA's abort word; from then on every wait of the CTA returns at
+// once, so the kernel runs to its end (with garbage results the host has been told about) instead of hanging.
+// The state lives in the LAST 16 bytes of the kernel's dynamic shared memory (kernels using these waits reserve them):
+// a static __shared__ object would push the 1024-byte aligned dynamic region up by a full KB.
+struct Watchdog { int abort; int pad; int* status; };
+constexpr int kWatchdogBytes = 16;
+__device__ __forceinline__ Watchdog& watchdog()
+{
+    extern __shared__ __align__(16) uint8_t wd_dynamic_smem[];
+    uint32_t size;
+    asm("mov.u32 %0, %%dynamic_smem_size;" : "=r"(size));
+    return *reinterpret_cast<Watchdog*>(wd_dynamic_smem + size - kWatchdogBytes);
+}
+// one thread, before the __syncthreads() that publishes the barrier initialisation
+__device__ __forceinline__ void watchdog_init(int* status) { watchdog().abort = 0; watchdog().status = status; }
+__device__ __forceinline__ void watchdog_report(int code, uint32_t what, uint32_t detail)
+{
+    Watchdog& w = watchdog();
+    if (atomicExch(&w.abort, 1) == 0 && w.status != nullptr && atomicCAS_system(w.status, 0, code) == 0) {
+        w.status[1] = (int)blockIdx.x; w.status[2] = (int)threadIdx.x; w.status[3] = (int)what; w.status[4] = (int)detail;
+        __threadfence_system();
+    }
+}
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity)
 {
 #if MESH_ATTN_WATCHDOG
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     while (!mbar_try_wait(bar, parity)) {
+        if (*reinterpret_cast<volatile int*>(&watchdog().abort)) return;
         if (clock64() - t0 > 8000000000ll) {   // ~4 s: certainly a deadlock
-            printf("mesh_attn watchdog: mbarrier wait timed out (block %d thread %d bar 0x%x parity %u)\n", blockIdx.x,
-                   threadIdx.x, smem_u32(bar), parity);
-            __trap();
+            watchdog_report(1, smem_u32(bar), parity);
+            return;
         }
     }
 #else
@@ -177,6 +203,47 @@ __device__ __forceinline__ uint32_t cluster_ctarank()
 __device__ __forceinline__ void cluster_sync()
 {
     asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// ---- distributed shared memory (the peer CTA of a 2-CTA cluster)
+// shared::cluster address of the peer's copy of a shared-memory object of this CTA
+__device__ __forceinline__ uint32_t mapa(uint32_t smem_addr, uint32_t cta_rank)
+{
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(cta_rank));
+    return r;
+}
+// 16-byte asynchronous store into the peer's shared memory; completes 16 bytes of the peer's mbarrier transaction count
+__device__ __forceinline__ void st_async_v4(uint32_t remote_addr, uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t remote_bar)
+{
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v4.b32 [%0], {%1, %2, %3, %4}, [%5];"
+                 ::"r"(remote_addr), "r"(a), "r"(b), "r"(c), "r"(d), "r"(remote_bar) : "memory");
+}
+// arrive on a barrier of the peer CTA (a consumer handing a buffer back to its remote producer)
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t remote_bar)
+{
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(remote_bar) : "memory");
+}
+// wait that acquires at cluster scope: the data the peer's st.async delivered is visible afterwards
+__device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t* bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n.reg .pred P;\nmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2, %3;\nselp.b32 %0, 1, 0, P;\n}"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity), "r"(10000000u)
+        : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait_cluster(uint64_t* bar, uint32_t parity)
+{
+    if (mbar_try_wait_cluster(bar, parity)) return;
+    const long long t0 = clock64();
+    while (!mbar_try_wait_cluster(bar, parity)) {
+#if MESH_ATTN_WATCHDOG
+        if (*reinterpret_cast<volatile int*>(&watchdog().abort)) return;
+        if (clock64() - t0 > 8000000000ll) { watchdog_report(1, smem_u32(bar), parity); return; }
+#endif
+    }
 }
 // TMA tile load delivered to the same CTA-relative smem address (and mbarrier) of every CTA in `cta_mask`
 __device__ __forceinline__ void tma_load_4d_mc(void* smem_dst, const CUtensorMap* m, uint64_t* bar, int c0, int c1, int c2, int c3,

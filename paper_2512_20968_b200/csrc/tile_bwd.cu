@@ -41,6 +41,8 @@
 // needed when |dS| is large (outlier scores, BASELINE.json configs[2]).
 #include <cuda_bf16.h>
 
+#include <atomic>
+
 #include "plan.hpp"
 #include "sm100.cuh"
 #include "tile_kernels.hpp"
@@ -60,26 +62,34 @@ constexpr int kCtrlRegs = 80, kComputeRegs = 136, kDrainRegs = 160;
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
-template <int D, bool kSplit> struct BwdCfg {
+template <int D, bool kSplit, bool kExch> struct BwdCfg {
+    static_assert(!(kSplit && kExch), "the dQ exchange is built for the single-operand mode only");
     static_assert(D == 128, "backward kernel: dQ^T needs head_dim = UMMA M = 128");
     static constexpr int kBoxes = D / 64;
     static constexpr int kTileBytes = kBlock * D * 2;          // [128 x D] bf16
     static constexpr int kDsBytes = kBlock * kBlock * 2;        // dS^T [128 kv x 128 q] bf16
     static constexpr int kNumDs = kSplit ? 2 : 1;               // hi (+ lo)
     static constexpr int kStages = kSplit ? 1 : 2;              // Q ring; split mode trades the second Q stage for the dS lo tile
-    static constexpr int kStgRows = 16;                         // dQ staging: a ring of kStgBufs buffers of [16 queries][D] fp32
-    static constexpr int kStgBufs = 4;
-    static constexpr int kStgBytes = kStgBufs * kStgRows * D * 4;
+    static constexpr int kStgRows = kExch ? kBwdStgRowsExch : kBwdStgRows;   // dQ staging: a ring of kStgBufs buffers of [kStgRows queries][D] fp32
+    static constexpr int kStgBytes = kBwdStgBytes;
+    static constexpr int kStgBufs = kStgBytes / (kStgRows * D * 4);
+    static_assert(kStgBufs >= 1 && kStgBufs * kStgRows * D * 4 == kStgBytes, "staging rows must divide the staging memory");
+    static constexpr int kDrainRows = kExch ? kBlock / 2 : kBlock;   // query rows of a step this CTA reduces into global dQ
+    // kExch: the peer's dQ^T half for this CTA's queries arrives as bf16 ([8 octets of queries][D][8]) in the FIRST HALF of the
+    // staging memory, is added to the registers, and then the whole 64-row fp32 sum is staged over it
+    static constexpr int kRecvBytes = (kBlock / 2) * D * 2;
+    static_assert(!kExch || (kDrainRows * D * 4 == kStgBytes && 2 * kRecvBytes == kStgBytes), "the exchange stages a whole step at once");
     static constexpr int kOffK = 0;
     static constexpr int kOffV = kTileBytes;
     static constexpr int kOffQ = 2 * kTileBytes;                // kStages Q tiles
     static constexpr int kOffdO = kOffQ + kStages * kTileBytes; // ONE dO tile: dO(i+1) is only needed a full step after dV(i) freed it
     static constexpr int kOffDs = kOffdO + kTileBytes;
     static constexpr int kOffStg = kOffDs + kNumDs * kDsBytes;  // dQ staging for the TMA reduce
+    static constexpr int kOffRecv = kOffStg;                    // aliases the first half of the staging memory (kExch)
     static constexpr int kOffVec = kOffStg + kStgBytes;         // per Q stage: log2(scale)-lse*log2e [128], delta[128] fp32
     static constexpr int kOffBars = kOffVec + kStages * 1024;
-    static constexpr int kNumBars = 2 + 2 * kStages + 10;
-    static constexpr int kSmemBytes = kOffBars + kNumBars * 8 + 16;
+    static constexpr int kNumBars = 2 + 2 * kStages + 12;
+    static constexpr int kSmemBytes = kOffBars + kNumBars * 8 + 16 + kWatchdogBytes;   // + TMEM slot + watchdog state (last 16 bytes)
     static constexpr uint32_t kColS = 0, kColDP = 128, kColDK = 256, kColDV = 384;
 };
 
@@ -195,13 +205,25 @@ template <int D> __device__ __forceinline__ void drain_rows(uint32_t taddr, floa
 // (64 rows) and the TMA multicasts it into both CTAs' shared memory, which halves the L2 -> SM tile traffic; a tile slot
 // is released to both loaders (multicast tcgen05.commit) because either one writes into both CTAs.  tmQ / tmdO are then
 // tensor maps with 64-row boxes.
-template <int D, bool kSplit, bool kPair>
+//
+// kPairMode 2 (kExch) -- the pair's dQ exchange.  Both CTAs hold a dQ^T contribution [128 d x 128 queries] for the SAME 128
+// query rows (their key blocks differ).  Instead of adding both to global memory, each CTA keeps the half of its tile that
+// belongs to "its" 64 queries (CTA rank r: queries 64r .. 64r+63 of the step) and sends the other half to its peer through
+// distributed shared memory as bf16 (16 KB per step and direction; fp32 would be 32 KB, measured at ~10 B/clk: too slow,
+// profiles/r01_v6_README.md); the receiver adds the peer's half to its own fp32 half and reduces 64 instead of 128 query
+// rows into global dQ: HALF the L2 atomics per step, which is what bounds the kernel.  The exchanged half
+// is rounded to bf16 (2^-9 relative, the precision the dS^T operand already has); precision = 1 plans do not use it.
+// Drain thread d of CTA r holds dQ^T row d; element (d, query) travels from thread d to thread d of the peer, so the
+// exchange buffer is addressed [octet of queries][d] x 16 bytes: conflict-free 512-byte warp stores (st.async, which also
+// completes the receiver's transaction barrier) and loads.  `send_ok` is the receiver handing the buffer back.
+template <int D, bool kSplit, int kPairMode>
 __global__ void __launch_bounds__(kBwdThreads, 1)
 tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
                 const __grid_constant__ CUtensorMap tmV, const __grid_constant__ CUtensorMap tmdO,
                 const __grid_constant__ CUtensorMap tmdQ, const BwdParams p)
 {
-    using Cfg = BwdCfg<D, kSplit>;
+    constexpr bool kPair = kPairMode >= 1, kExch = kPairMode == 2;
+    using Cfg = BwdCfg<D, kSplit, kExch>;
     extern __shared__ __align__(1024) uint8_t smem[];
     uint8_t* sK = smem + Cfg::kOffK;
     uint8_t* sV = smem + Cfg::kOffV;
@@ -221,7 +243,9 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* dkv_empty = s_full + 7;
     uint64_t* do_full = s_full + 8;
     uint64_t* do_empty = s_full + 9;
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(s_full + 10);
+    uint64_t* send_ok = s_full + 10;                    // kExch: the peer's receive buffer is free for this step's half (remote arrive)
+    uint64_t* recv_full = s_full + 11;                  // kExch: the peer's dQ^T half for this CTA's queries has landed in sRecv (transaction count)
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(s_full + 12);
     uint8_t* sdO = smem + Cfg::kOffdO;
     float* sStg = reinterpret_cast<float*>(smem + Cfg::kOffStg);
     auto sQ = [&](int st) { return smem + Cfg::kOffQ + st * Cfg::kTileBytes; };
@@ -234,8 +258,12 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const long long N = gm.rows_q;
     constexpr int kCompute = 2 * kBlock;                // threads of the two compute groups
 
+    if (smem_u32(smem) & 1023u) {                       // the 128-byte swizzle needs a 1024-byte aligned base: report, do not trap
+        if (threadIdx.x == 0 && p.status != nullptr && atomicCAS_system(p.status, 0, 2) == 0) { p.status[1] = (int)blockIdx.x; __threadfence_system(); }
+        return;
+    }
     if (threadIdx.x == 0) {
-        if (smem_u32(smem) & 1023u) { printf("mesh_attn tile_bwd: dynamic smem base not 1024-byte aligned\n"); __trap(); }
+        watchdog_init(p.status);
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV); prefetch_tmap(&tmdO); prefetch_tmap(&tmdQ);
         mbar_init(kv_full, 1);
         mbar_init(kv_empty, 1);
@@ -250,6 +278,8 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(dkv_empty, kCompute);
         mbar_init(do_full, 1);
         mbar_init(do_empty, kPair ? 2 : 1);
+        mbar_init(recv_full, 1);
+        mbar_init(send_ok, 1);
         fence_mbar_init();
     }
     if (warp == 2) tmem_alloc<512>(tmem_slot);
@@ -597,6 +627,15 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const bool issuer = threadIdx.x == 12 * 32;
         const int dv = gm.head_dim;                      // 64: dQ^T rows 64..127 are zero and stay in the CTA
         uint32_t dq_ph = 0;
+        // kExch: this CTA reduces queries own0 .. own0+63 of every step and sends the others to the peer
+        const uint32_t own0 = kExch ? pair_rank * (kBlock / 2) : 0, peer0 = kBlock / 2 - own0;
+        const uint8_t* sRecv = smem + Cfg::kOffRecv;
+        const uint32_t my_slot = (uint32_t)d * 16u;                                       // + octet * (D * 16)
+        const uint32_t peer_recv = kExch ? mapa(smem_u32(sRecv), pair_rank ^ 1u) + my_slot : 0u;
+        const uint32_t peer_recv_full = kExch ? mapa(smem_u32(recv_full), pair_rank ^ 1u) : 0u;
+        constexpr int kSlices = Cfg::kDrainRows / Cfg::kStgRows;
+        const uint32_t peer_send_ok = kExch ? mapa(smem_u32(send_ok), pair_rank ^ 1u) : 0u;
+        uint32_t rf_ph = 0, sok_ph = 0;
         PT_DECL;
         for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
             const BwdItemCtx c = load_bwd_item(p, idx);
@@ -604,36 +643,102 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             QStep q;
             while (q.next(walk)) {
                 PT_MARK(0);
-                mbar_wait(dq_full, dq_ph);
-                dq_ph ^= 1;
-                tc_fence_after();
-                uint32_t r[kBlock];
+                if constexpr (kExch) {
+                    // One step of the exchange (see the kernel's header comment).  The staging memory is used twice per step: its
+                    // first half receives the peer's bf16 half, then all of it holds this CTA's 64 fp32 rows, reduced as kSlices
+                    // boxes in bulk groups of their own, the first-half boxes first.  The TMA works on them during the next step's
+                    // load / send / wait, so this group never waits for a reduce it has just issued.
+                    if (issuer) mbar_expect_tx(recv_full, Cfg::kRecvBytes);      // what the peer will send for this step
+                    mbar_wait(dq_full, dq_ph);
+                    dq_ph ^= 1;
+                    tc_fence_after();
+                    uint32_t r[kBlock / 2], rp[kBlock / 2];      // this CTA's / the peer's query columns of dQ^T row d
+                    tmem_ld_x32(tDQ + peer0, *reinterpret_cast<uint32_t(*)[32]>(&rp[0]));
+                    tmem_ld_x32(tDQ + peer0 + 32, *reinterpret_cast<uint32_t(*)[32]>(&rp[32]));
+                    tmem_ld_x32(tDQ + own0, *reinterpret_cast<uint32_t(*)[32]>(&r[0]));
+                    tmem_ld_x32(tDQ + own0 + 32, *reinterpret_cast<uint32_t(*)[32]>(&r[32]));
+                    tmem_ld_wait();
+                    tc_fence_before();
+                    mbar_arrive(dq_empty);           // TMEM columns free again: dP^T of the next step may start
+                    PT_MARK(1);
+                    if (issuer) {                    // the previous step's first-half boxes have been read: the peer may send into that half
+                        // (head_dim 64: the staged rows are half as long, all of them lie in the receive area: wait for every box)
+                        if (dv == D) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(kSlices / 2) : "memory");
+                        else asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");
+                        mbar_arrive_remote(peer_send_ok);
+                    }
+                    mbar_wait(send_ok, sok_ph);      // ... and the peer's first half is free for this CTA's data
+                    sok_ph ^= 1;
 #pragma unroll
-                for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tDQ + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[ch * 32]));
-                tmem_ld_wait();
-                tc_fence_before();
-                mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
-                PT_MARK(1);
+                    for (int o = 0; o < kBlock / 16; ++o)        // 8 queries = 16 bytes of bf16 per store
+                        st_async_v4(peer_recv + o * (D * 16),
+                                    pack_bf16x2(__uint_as_float(rp[8 * o + 0]), __uint_as_float(rp[8 * o + 1])),
+                                    pack_bf16x2(__uint_as_float(rp[8 * o + 2]), __uint_as_float(rp[8 * o + 3])),
+                                    pack_bf16x2(__uint_as_float(rp[8 * o + 4]), __uint_as_float(rp[8 * o + 5])),
+                                    pack_bf16x2(__uint_as_float(rp[8 * o + 6]), __uint_as_float(rp[8 * o + 7])), peer_recv_full);
+                    PT_MARK(2);
+                    mbar_wait_cluster(recv_full, rf_ph);         // the peer's half for this CTA's queries has landed: add it
+                    rf_ph ^= 1;
+                    PT_MARK(3);
 #pragma unroll
-                for (int k = 0; k < kBlock / Cfg::kStgRows; ++k) {   // 16-query slice k through staging buffer k % kStgBufs
-                    float* stg = sStg + (k % Cfg::kStgBufs) * (Cfg::kStgRows * D);      // rows of dv floats (the reduce's box)
-                    if (issuer) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(Cfg::kStgBufs - 1) : "memory");   // slice k - kStgBufs has been read
-                    named_bar_sync(1, kBlock);
+                    for (int o = 0; o < kBlock / 16; ++o) {
+                        const uint4 w = *reinterpret_cast<const uint4*>(sRecv + o * (D * 16) + my_slot);
+                        r[8 * o + 0] = __float_as_uint(__uint_as_float(r[8 * o + 0]) + __uint_as_float(w.x << 16));
+                        r[8 * o + 1] = __float_as_uint(__uint_as_float(r[8 * o + 1]) + __uint_as_float(w.x & 0xffff0000u));
+                        r[8 * o + 2] = __float_as_uint(__uint_as_float(r[8 * o + 2]) + __uint_as_float(w.y << 16));
+                        r[8 * o + 3] = __float_as_uint(__uint_as_float(r[8 * o + 3]) + __uint_as_float(w.y & 0xffff0000u));
+                        r[8 * o + 4] = __float_as_uint(__uint_as_float(r[8 * o + 4]) + __uint_as_float(w.z << 16));
+                        r[8 * o + 5] = __float_as_uint(__uint_as_float(r[8 * o + 5]) + __uint_as_float(w.z & 0xffff0000u));
+                        r[8 * o + 6] = __float_as_uint(__uint_as_float(r[8 * o + 6]) + __uint_as_float(w.w << 16));
+                        r[8 * o + 7] = __float_as_uint(__uint_as_float(r[8 * o + 7]) + __uint_as_float(w.w & 0xffff0000u));
+                    }
+                    PT_MARK(4);
+                    if (issuer) asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory");   // the previous step's second-half boxes too
+                    named_bar_sync(1, kBlock);       // every thread has consumed the received half: the sums may be staged over it
 #pragma unroll
-                    for (int j = 0; j < Cfg::kStgRows; ++j)
-                        if (d < dv) stg[j * dv + d] = __uint_as_float(r[k * Cfg::kStgRows + j]);
+                    for (int j = 0; j < kBlock / 2; ++j)
+                        if (d < dv) sStg[j * dv + d] = __uint_as_float(r[j]);
                     fence_proxy_async_smem();
                     named_bar_sync(1, kBlock);
                     if (issuer) {
-                        tma_reduce_add_4d(&tmdQ, stg, 0, q.h, q.u * gm.L + q.s0 + k * Cfg::kStgRows, c.it.batch);
-                        asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+#pragma unroll
+                        for (int k = 0; k < kSlices; ++k) {
+                            tma_reduce_add_4d(&tmdQ, sStg + k * (Cfg::kStgRows * dv), 0, q.h, q.u * gm.L + q.s0 + (int)own0 + k * Cfg::kStgRows, c.it.batch);
+                            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                        }
+                    }
+                } else {
+                    mbar_wait(dq_full, dq_ph);
+                    dq_ph ^= 1;
+                    tc_fence_after();
+                    uint32_t r[kBlock];
+#pragma unroll
+                    for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tDQ + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&r[ch * 32]));
+                    tmem_ld_wait();
+                    tc_fence_before();
+                    mbar_arrive(dq_empty);               // TMEM columns free again: dP^T of the next step may start
+                    PT_MARK(1);
+#pragma unroll
+                    for (int k = 0; k < kSlices; ++k) {   // 16-query slice k through staging buffer k % kStgBufs
+                        float* stg = sStg + (k % Cfg::kStgBufs) * (Cfg::kStgRows * D);      // rows of dv floats (the reduce's box)
+                        if (issuer) asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(Cfg::kStgBufs - 1) : "memory");   // slice k - kStgBufs has been read
+                        named_bar_sync(1, kBlock);
+#pragma unroll
+                        for (int j = 0; j < Cfg::kStgRows; ++j)
+                            if (d < dv) stg[j * dv + d] = __uint_as_float(r[k * Cfg::kStgRows + j]);
+                        fence_proxy_async_smem();
+                        named_bar_sync(1, kBlock);
+                        if (issuer) {
+                            tma_reduce_add_4d(&tmdQ, stg, 0, q.h, q.u * gm.L + q.s0 + k * Cfg::kStgRows, c.it.batch);
+                            asm volatile("cp.async.bulk.commit_group;" ::: "memory");
+                        }
                     }
                 }
-                PT_MARK(2);
+                PT_MARK(5);
             }
         }
         if (issuer) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");       // every reduce has landed before the CTA exits
-        PT_REPORT("bwd drain clocks per step: wait dQ + ld, staging + TMA reduce, 0, 0, 0");
+        PT_REPORT("bwd drain clocks per step: wait dQ + ld, wait send_ok + send, wait recv, add, staging + TMA reduce (no exchange: wait dQ + ld, 0, 0, 0, staging)");
     }
 
     tc_fence_before();
@@ -642,13 +747,13 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == 2) tmem_dealloc<512>(tmem);
 }
 
-template <int D, bool kSplit, bool kPair>
+template <int D, bool kSplit, int kPairMode>
 int launch_one(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, const CUtensorMap& tmdO,
                const CUtensorMap& tmdQ, int grid, cudaStream_t stream)
 {
-    using Cfg = BwdCfg<D, kSplit>;
+    using Cfg = BwdCfg<D, kSplit, kPairMode == 2>;
     static_assert(Cfg::kSmemBytes <= 227 * 1024, "tile_bwd shared memory over the 227 KB CTA limit");
-    auto kernel = tile_bwd_kernel<D, kSplit, kPair>;
+    auto kernel = tile_bwd_kernel<D, kSplit, kPairMode>;
     cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
     if (e != cudaSuccess) return (int)e;
     cudaLaunchConfig_t cfg{};
@@ -656,21 +761,26 @@ int launch_one(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tm
     cfg.dynamicSmemBytes = Cfg::kSmemBytes;
     cfg.stream = stream;
     cudaLaunchAttribute attr[1];
-    if (kPair) {
+    if (kPairMode) {
         attr[0].id = cudaLaunchAttributeClusterDimension;
         attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
         cfg.attrs = attr;
         cfg.numAttrs = 1;
-        static int max_clusters = -1;                   // co-resident 2-CTA clusters of this kernel (GPCs with an odd SM count leave one SM out)
-        if (max_clusters < 0) {
+        // co-resident 2-CTA clusters of this kernel (GPCs with an odd SM count leave one SM out), cached per device
+        constexpr int kMaxDevices = 64;
+        static std::atomic<int> max_clusters[kMaxDevices];      // 0 = not queried yet, else count + 1
+        int dev = 0;
+        e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return (int)e;
+        int n = (dev >= 0 && dev < kMaxDevices) ? max_clusters[dev].load(std::memory_order_relaxed) - 1 : -1;
+        if (n < 0) {
             cfg.gridDim = dim3(2);
-            int n = 0;
             e = cudaOccupancyMaxActiveClusters(&n, kernel, &cfg);
             if (e != cudaSuccess) return (int)e;
-            max_clusters = n;
+            if (dev >= 0 && dev < kMaxDevices) max_clusters[dev].store(n + 1, std::memory_order_relaxed);
         }
-        if (max_clusters <= 0) return (int)cudaErrorLaunchOutOfResources;
-        grid = (grid / 2 < max_clusters ? grid / 2 : max_clusters) * 2;
+        if (n <= 0) return (int)cudaErrorLaunchOutOfResources;
+        grid = (grid / 2 < n ? grid / 2 : n) * 2;
     }
     cfg.gridDim = dim3(grid);
     e = cudaLaunchKernelEx(&cfg, kernel, tmQ, tmK, tmV, tmdO, tmdQ, p);
@@ -687,11 +797,12 @@ int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
+    if (p.pair == 2 && !p.split) return launch_one<128, false, 2>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
     if (p.pair)
-        return p.split ? launch_one<128, true, true>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
-                       : launch_one<128, false, true>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
-    return p.split ? launch_one<128, true, false>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
-                   : launch_one<128, false, false>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
+        return p.split ? launch_one<128, true, 1>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
+                       : launch_one<128, false, 1>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
+    return p.split ? launch_one<128, true, 0>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream)
+                   : launch_one<128, false, 0>(p, tmQ, tmK, tmV, tmdO, tmdQ, grid, stream);
 }
 
 }  // namespace mesh_attn

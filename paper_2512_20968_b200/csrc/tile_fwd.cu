@@ -57,7 +57,7 @@ template <int D> struct FwdCfg {
     static constexpr int kSmemQ = 2 * kTileBytes;
     static constexpr int kSmemRing = kStages * kTileBytes;
     static constexpr int kNumBars = 2 + 2 * kStages + 8;
-    static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 1024;   // + alignment slack
+    static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 1024 + kWatchdogBytes;   // + TMEM slot, alignment slack, watchdog state (last 16 bytes)
     static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
 };
 
@@ -144,6 +144,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     if (warp == kLoaderWarp && lane == 0) {
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV);
+        watchdog_init(p.status);
         mbar_init(q_full, 1);
         mbar_init(q_empty, 1);
         for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }

@@ -7,6 +7,20 @@
 
 namespace mesh_attn {
 
+// tile_bwd's dQ staging: query rows per cp.reduce.async.bulk.tensor box (= box rows of the dQ tensor map built in capi.cu).
+// The TMA reduce costs a fixed ~210 clk per box on top of its bytes (measured: 8 KB boxes 509 clk, 4 KB boxes 360 clk each,
+// profiles/r02_v1_README.md), and its read of the staging memory completes ~1000-1500 clk after the issue (L2 atomics under load):
+// what bounds the drain is the bytes in flight.  Without the pair's dQ exchange: a ring of four 8 KB buffers (16 rows each);
+// with it: the step's 64 rows are staged at once and reduced as two 16 KB boxes while the next step's exchange runs.
+#ifndef MESH_ATTN_STG_ROWS
+#define MESH_ATTN_STG_ROWS 16
+#endif
+#ifndef MESH_ATTN_STG_ROWS_EXCH
+#define MESH_ATTN_STG_ROWS_EXCH 32
+#endif
+constexpr int kBwdStgRows = MESH_ATTN_STG_ROWS, kBwdStgRowsExch = MESH_ATTN_STG_ROWS_EXCH;
+constexpr int kBwdStgBytes = 32 * 1024;
+
 constexpr int kMaxPeers = 16;   // largest Q group the peer-memory merge takes (a <= 16: BASELINE.json's largest mesh)
 
 struct FwdParams {
@@ -19,6 +33,7 @@ struct FwdParams {
     int split;                 // precision: 1 = P fed to the PV MMA as hi + lo bf16
     float* partial_O;          // [g_count][slots][B][L][Hq][D]
     float* partial_lse;        // [g_count][slots][B][Hq][L]
+    int* status;               // the plan's host-mapped status words (sm100.cuh watchdog); may be null
 };
 
 struct BwdParams {
@@ -29,7 +44,10 @@ struct BwdParams {
     int items_per_gpu;
     int g_first, g_count;
     int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
-    int pair;                  // 1: items 2k, 2k+1 walk the same Q blocks -> 2-CTA clusters with multicast Q/dO tiles (tmQ, tmdO: 64-row boxes)
+    int pair;                  // 1: items 2k, 2k+1 walk the same Q blocks -> 2-CTA clusters with multicast Q/dO tiles (tmQ, tmdO: 64-row boxes);
+                               // 2: the pair also exchanges dQ^T halves (bf16, distributed shared memory) and each CTA reduces 64 of the
+                               //    step's 128 query rows (tmdQ: 8-row boxes)
+    int* status;               // the plan's host-mapped status words (sm100.cuh watchdog); may be null
     const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess); head 0 = first head of the lane
     long long ws_plane;        // elements between ws[0] and ws[1] (B * all heads * N)
     long long vec_stride_b;    // batch stride of the [B][Hq][N] vectors (all heads * N)

@@ -22,10 +22,13 @@ Two forms of the exchanges that FOLLOW a compute step (RS-O, RS-dQ, RS-dKV):
     separate collective.  Each partial is read exactly once, so peer reads cost no extra link traffic.  The all-gathers
     that PRECEDE a compute step stay NCCL copies into local HBM on purpose: every Q / K / V tile is re-read by dozens of
     work items, and peer memory is not cached in the reader's L2.
-Neither form has run on more than one GPU (this build's boxes have one): the per-rank kernels, the peer-memory reducers
-included, are parity-tested on one B200 by playing the n ranks one after the other (tests/test_gpu_rank_calls.py), the
-group construction / slot order / routing by world-size 2 and 4 gloo processes with stand-in compute
-(tests/test_multirank_cpu.py); the symmetric-memory rendezvous of ``peer_memory=True`` is unexecuted code.  Needs kvr = 1 (with KV partition rotation the ranks
+Neither form has run on more than one GPU (this build's boxes have one).  What has run: the per-rank kernels, the
+peer-memory reducers included, on one B200 with the n ranks played one after the other (tests/test_gpu_rank_calls.py); this
+class end to end, both forms, as a ONE-rank NCCL job on one B200 (a = b = 1: sub-communicators, all-gathers, all-to-all,
+reduce-scatter, ``symm_mem.empty`` / ``rendezvous`` / ``barrier`` and the peer reducers through the symmetric-memory handles)
+and the peer reducers on pointers that really belong to ANOTHER process (CUDA IPC between two processes on the one GPU)
+(tests/test_gpu_distributed_one_gpu.py); the group construction / slot order / routing by world-size 2 and 4 gloo processes
+with stand-in compute (tests/test_multirank_cpu.py).  Needs kvr = 1 (with KV partition rotation the ranks
 that share a KV footprint are exactly the owners of its partitions, L157-161), usp_lanes = 1, tensor_layout 0.
 """
 from __future__ import annotations
@@ -90,10 +93,10 @@ def _exchange_slots(send: torch.Tensor, ranks, own_index: int, group) -> torch.T
 
 
 class MeshAttnRank:
-    """One rank of the job.  ``kernels`` is the object whose ``rank_*`` methods do the arithmetic: the Plan itself
-    (default; there is no other product path), or a stand-in with the same four methods in the CPU tests."""
+    """One rank of the job.  Every compute step runs in the library's kernels through the plan's ``rank_*`` calls; there is
+    no other path (the CPU tests of the routing subclass this in tests/rank_standin.py and replace ``_kernels`` there)."""
 
-    def __init__(self, plan, rank: int | None = None, world_size: int | None = None, kernels=None, peer_memory: bool = False):
+    def __init__(self, plan, rank: int | None = None, world_size: int | None = None, peer_memory: bool = False):
         self.plan = plan
         self.peer_memory = peer_memory
         self.g = dist.get_rank() if rank is None else rank
@@ -101,7 +104,7 @@ class MeshAttnRank:
         d = plan.desc
         if max(d.usp_lanes, 1) != 1 or d.tensor_layout != 0 or d.partial_mode != 0:
             raise ValueError("MeshAttnRank needs usp_lanes = 1, tensor_layout 0, partial_mode 0")
-        self.kernels = plan if kernels is None else kernels
+        self._kernels = plan
         self.a, self.b, self.n = d.a, d.b, d.n
         self.B, self.L, self.Hq, self.Hkv, self.D = d.batch, d.seq_total // d.n, d.heads_q, d.heads_kv, d.head_dim
         q_groups, kv_groups = mesh_groups(plan, world)
@@ -152,17 +155,17 @@ class MeshAttnRank:
         if self.peer_memory:
             (partial_O, hO), (partial_lse, hl) = self._symmetric(dev)["pO"], self._symmetric(dev)["plse"]
             hO.barrier()                                                                # the members have merged the previous step's partials
-            self.kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)  # l.3-5
+            self._kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)  # l.3-5
             hO.barrier()                                                                # every member's partials are written
-            self.kernels.rank_merge_peers(self._slot_ptrs(hO, a, self.q_index, B * L * Hq * D),     # l.6 RS-O fused into the reducer
+            self._kernels.rank_merge_peers(self._slot_ptrs(hO, a, self.q_index, B * L * Hq * D),     # l.6 RS-O fused into the reducer
                                           self._slot_ptrs(hl, a, self.q_index, B * Hq * L), O_own, lse_own)
         else:
             partial_O = torch.empty((a, B, L, Hq, D), dtype=torch.float32, device=dev)
             partial_lse = torch.empty((a, B, Hq, L), dtype=torch.float32, device=dev)
-            self.kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)      # l.3-5
+            self._kernels.rank_fwd(self.g, Q_loc, K_loc, V_loc, partial_O, partial_lse)      # l.3-5
             recv_O = _exchange_slots(partial_O, self.q_ranks, self.q_index, self.q_group)   # l.6 RS-O: slot k -> member k
             recv_lse = _exchange_slots(partial_lse, self.q_ranks, self.q_index, self.q_group)
-            self.kernels.rank_merge(recv_O, recv_lse, O_own, lse_own)                       # ... with the online-softmax reducer
+            self._kernels.rank_merge(recv_O, recv_lse, O_own, lse_own)                       # ... with the online-softmax reducer
         self._saved = (Q_loc, K_loc, V_loc, O_own, lse_own)
         return O_own, lse_own
 
@@ -175,7 +178,7 @@ class MeshAttnRank:
         a, b, B, L, Hq, Hkv, D = self.a, self.b, self.B, self.L, self.Hq, self.Hkv, self.D
         dev = dO_own.device
         ws_own = torch.empty((2, B, Hq, L), dtype=torch.float32, device=dev)
-        self.kernels.rank_bwd_preprocess(O_own, dO_own.contiguous(), lse_own, ws_own)
+        self._kernels.rank_bwd_preprocess(O_own, dO_own.contiguous(), lse_own, ws_own)
         dO_loc = _gather_slots(dO_own, self.q_ranks, self.q_group)                       # l.1 (with Q_loc kept from the forward)
         ws_all = torch.empty((a, 2, B, Hq, L), dtype=torch.float32, device=dev)
         dist.all_gather(list(ws_all.unbind(0)), ws_own, group=self.q_group)
@@ -188,19 +191,19 @@ class MeshAttnRank:
             hQ.barrier(); hK.barrier()                                                  # the previous step's sums have been read
             for t in (dQ_loc, dK_loc, dV_loc):
                 t.zero_()
-            self.kernels.rank_bwd(self.g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc)   # l.3-5
+            self._kernels.rank_bwd(self.g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc)   # l.3-5
             hQ.barrier(); hK.barrier()
             dQ_own = torch.empty((B, L, Hq, D), dtype=torch.float32, device=dev)
             dK_own = torch.empty((B, L, Hkv, D), dtype=torch.float32, device=dev)
             dV_own = torch.empty((B, L, Hkv, D), dtype=torch.float32, device=dev)
-            self.kernels.rank_sum_peers(self._slot_ptrs(hQ, a, self.q_index, L * Hq * D), dQ_own)        # l.6 RS-dQ as peer reads
-            self.kernels.rank_sum_peers(self._slot_ptrs(hK, b, self.kv_index, L * Hkv * D), dK_own)      # l.7 RS-dKV
-            self.kernels.rank_sum_peers(self._slot_ptrs(hV, b, self.kv_index, L * Hkv * D), dV_own)
+            self._kernels.rank_sum_peers(self._slot_ptrs(hQ, a, self.q_index, L * Hq * D), dQ_own)        # l.6 RS-dQ as peer reads
+            self._kernels.rank_sum_peers(self._slot_ptrs(hK, b, self.kv_index, L * Hkv * D), dK_own)      # l.7 RS-dKV
+            self._kernels.rank_sum_peers(self._slot_ptrs(hV, b, self.kv_index, L * Hkv * D), dV_own)
             return dQ_own, dK_own, dV_own
         dQ_loc = torch.zeros((B, a * L, Hq, D), dtype=torch.float32, device=dev)
         dK_loc = torch.zeros((B, b * L, Hkv, D), dtype=torch.float32, device=dev)
         dV_loc = torch.zeros((B, b * L, Hkv, D), dtype=torch.float32, device=dev)
-        self.kernels.rank_bwd(self.g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc)   # l.3-5
+        self._kernels.rank_bwd(self.g, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc)   # l.3-5
         dQ_own = _reduce_scatter_slots(dQ_loc, self.q_ranks, self.q_index, self.q_group)             # l.6 RS-dQ
         dK_own = _reduce_scatter_slots(dK_loc, self.kv_ranks, self.kv_index, self.kv_group)          # l.7 RS-dKV
         dV_own = _reduce_scatter_slots(dV_loc, self.kv_ranks, self.kv_index, self.kv_group)

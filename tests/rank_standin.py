@@ -5,6 +5,16 @@ import math
 
 import torch
 
+from paper_2512_20968_b200.distributed import MeshAttnRank
+
+
+class StandInRank(MeshAttnRank):
+    """MeshAttnRank with its compute calls replaced by the stand-in below: the product class takes no such argument."""
+
+    def __init__(self, plan, standin, **kw):
+        super().__init__(plan, **kw)
+        self._kernels = standin
+
 
 class StandInKernels:
     def __init__(self, plan, seq_layout: str):

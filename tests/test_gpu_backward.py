@@ -81,9 +81,10 @@ def test_scaled_configs_full_keys(oracle, name, L, hq):
 
 
 @pytest.mark.parametrize("name", ["C2", "C5"])
-def test_paired_and_unpaired_kernel_variants(oracle, monkeypatch, name):
-    """tile_bwd as 2-CTA clusters with multicast Q / dO tiles (MESH_ATTN_Q_BWD_PAIRED) and as single CTAs
-    (MESH_ATTN_NO_PAIR=1 at plan creation): both against the oracle, and against each other."""
+def test_paired_and_unpaired_kernel_variants(oracle, name):
+    """The three tile_bwd kernels a pairable plan can run (plan desc field bwd_pairing): 2-CTA clusters with multicast Q / dO
+    tiles AND the pair's dQ exchange (0 = auto, MESH_ATTN_Q_BWD_PAIRED == 2), single CTAs (1), clusters without the exchange (2):
+    each against the oracle, and against each other (the exchange rounds half of the dQ partial sums to bf16)."""
     from paper_2512_20968_b200.binding import Q_BWD_PAIRED
 
     w = W.scaled_down(W.CONFIGS[name], 256, heads_q=2)
@@ -94,16 +95,74 @@ def test_paired_and_unpaired_kernel_variants(oracle, monkeypatch, name):
     rows = np.unique(np.concatenate([rng.integers(0, w.seq_total, 32), [0, w.seq_total - 1, w.L - 1, w.L]]))
     qrows, qheads = all_pairs(rows, range(w.heads_q))
     krows, kheads = all_pairs(rows[:16], range(w.heads_kv))
-    bufs = []
-    for no_pair in ("0", "1"):
-        monkeypatch.setenv("MESH_ATTN_NO_PAIR", no_pair)
+    bufs, errs = [], {}
+    for pairing, mode in ((0, 2), (1, 0), (2, 1)):
+        plan, buf = run_fwd_bwd(w, inp, bwd_pairing=pairing)
+        assert plan.query(Q_BWD_PAIRED) == mode
+        errs[mode] = check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
+        check_invariants(w, inp, buf)
+        plan.health()
+        bufs.append(buf)
+    print(f"\n{w.name} tile_bwd variants (2 = pair + dQ exchange, 0 = single CTA, 1 = pair): " + str({k: {a: float(f'{b:.3g}') for a, b in v.items()} for k, v in errs.items()}))
+    for other in bufs[1:]:
+        for x, y in ((bufs[0].dQ, other.dQ), (bufs[0].dK, other.dK), (bufs[0].dV, other.dV)):
+            assert (x - y).abs().max().item() <= (1e-2 if x is bufs[0].dQ else 1e-3)   # atomics: the summation order is run-dependent; dQ: + the exchange's bf16 rounding
+    with pytest.raises(Exception):
+        run_fwd_bwd(w, inp, bwd_pairing=3)
+
+
+def test_exchange_every_row_and_odd_paths(oracle):
+    """The dQ exchange on EVERY query row and key of a small problem, for the three kinds of pairable plans: non-causal
+    (items 2k, 2k+1 = neighbouring key blocks of one KV partition), striped causal (the same key block of two KV partitions,
+    offsets 0 / -1), GQA (the Q walk repeats per query head of the group); and a non-pairable plan (contiguous causal) still
+    runs the single-CTA kernel."""
+    from paper_2512_20968_b200.binding import Q_BWD_PAIRED
+
+    cases = [
+        replace(W.scaled_down(W.C2, 256, heads_q=2), a=2, b=2, seq_total=4 * 256),
+        replace(W.scaled_down(W.C4, 256, heads_q=4), a=2, b=2, seq_total=4 * 256, heads_kv=2),
+        replace(W.scaled_down(W.C5, 512, heads_q=1), a=2, b=2, seq_total=4 * 512),
+    ]
+    for w in cases:
+        inp = W.make_inputs(w, "cuda")
         plan, buf = run_fwd_bwd(w, inp)
-        assert plan.query(Q_BWD_PAIRED) == (1 if no_pair == "0" else 0)
+        assert plan.query(Q_BWD_PAIRED) == 2
+        qrows, qheads = all_pairs(np.arange(w.seq_total), range(w.heads_q))
+        krows, kheads = all_pairs(np.arange(0, w.seq_total, 7), range(w.heads_kv))
         check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
         check_invariants(w, inp, buf)
-        bufs.append(buf)
-    for x, y in ((bufs[0].dQ, bufs[1].dQ), (bufs[0].dK, bufs[1].dK), (bufs[0].dV, bufs[1].dV)):
-        assert (x - y).abs().max().item() <= 1e-3            # atomics: the summation order is run-dependent
+    w = replace(cases[1], seq_layout="contiguous")
+    inp = W.make_inputs(w, "cuda")
+    plan, buf = run_fwd_bwd(w, inp)
+    assert plan.query(Q_BWD_PAIRED) == 0
+    check_grads(oracle, w, inp, buf, *all_pairs(np.arange(0, w.seq_total, 3), range(w.heads_q)), *all_pairs(np.arange(0, w.seq_total, 7), range(w.heads_kv)))
+
+
+@pytest.mark.parametrize("pairing", [0, 1])
+def test_sweep_pieces(oracle, pairing):
+    """tile_bwd work items as (key block, piece of the Q sweep) (plan desc field bwd_piece_blocks): pieces of one segment, of two
+    blocks' worth and the whole sweep give the same gradients (the same sums in another order), each within tolerance of the
+    oracle on every row and key -- striped causal (pieces that end before a key block are pruned from the list), contiguous
+    causal (they stay, as zero-step items), GQA, two Q chunks in greedy order."""
+    from paper_2512_20968_b200.binding import Q_BWD_ITEMS_PER_GPU
+
+    for layout in ("striped", "contiguous"):
+        w = replace(W.scaled_down(W.C4, 512, heads_q=4), a=3, b=2, seq_total=6 * 512, heads_kv=2, seq_layout=layout, order="greedy", k_q=2, k_kv=2)
+        inp = W.make_inputs(w, "cuda")
+        qrows, qheads = all_pairs(np.arange(0, w.seq_total, 3), range(w.heads_q))
+        krows, kheads = all_pairs(np.arange(0, w.seq_total, 5), range(w.heads_kv))
+        ref, counts = None, []
+        for blocks in (1, 4, 1 << 20):
+            plan, buf = run_fwd_bwd(w, inp, bwd_piece_blocks=blocks, bwd_pairing=pairing)
+            counts.append(plan.query(Q_BWD_ITEMS_PER_GPU))
+            check_grads(oracle, w, inp, buf, qrows, qheads, krows, kheads)
+            check_invariants(w, inp, buf)
+            if ref is None:
+                ref = buf
+            else:
+                for x, y in ((ref.dQ, buf.dQ), (ref.dK, buf.dK), (ref.dV, buf.dV)):
+                    assert (x - y).abs().max().item() <= 1e-2
+        assert counts[0] > counts[1] > counts[2]
 
 
 @pytest.mark.parametrize("layout,kvr", [("contiguous", True), ("striped", False), ("striped", True)])

@@ -81,15 +81,14 @@ def _mesh_worker(rank: int, world: int, port: int, a: int, b: int, causal: bool,
     torch.set_num_threads(2)
     from paper_2512_20968_b200 import plan_for
     from paper_2512_20968_b200 import workloads as W
-    from paper_2512_20968_b200.distributed import MeshAttnRank
-    from tests.rank_standin import StandInKernels
+    from tests.rank_standin import StandInKernels, StandInRank
 
     L, D = 128, 64
     w = W.Workload("mesh", 7, causal, a, b, 1, L * a * b, heads_q, heads_kv, D, seq_layout="striped" if causal else "contiguous")
     plan = plan_for(w)
     inp = W.make_inputs(w, "cpu")                                # same seed on every rank
     own = {k: v[:, rank * L:(rank + 1) * L].contiguous() for k, v in inp.items()}
-    me = MeshAttnRank(plan, kernels=StandInKernels(plan, w.seq_layout))
+    me = StandInRank(plan, StandInKernels(plan, w.seq_layout))
     O, lse = me.forward(own["q"], own["k"], own["v"])
     dQ, dK, dV = me.backward(own["do"])
     torch.save({"O": O, "lse": lse, "dQ": dQ, "dK": dK, "dV": dV}, Path(out_dir, f"rank{rank}.pt"))

@@ -78,6 +78,28 @@ def test_goo_fig4_example():
     assert s2 == serial and m2 >= makespan and e2 >= exposed
 
 
+def _assert_same_tiles(got, ref, order):
+    """What the paper fixes about a GPU's tile list: the SEQUENCE of compute tasks C-i-j (the step list)
+    and, inside a task, the SET of pairs "for each gathered pair (Q_u, KV_v)" (Alg.2 l.3-5, L171-173) = I_g^Q x I_g^KV.
+    The order of the pairs inside one task is a free choice (any order gives the same attention; reading R17),
+    so it is compared as a set, not as a sequence."""
+    got = [tuple(r) for r in got.tolist()]
+    per = len(got) // len(order)
+    assert len(got) == len(ref) == per * len(order)
+    for t, ij in enumerate(order):
+        g_chunk, r_chunk = got[t * per:(t + 1) * per], ref[t * per:(t + 1) * per]
+        assert all(x[2:] == tuple(ij) for x in g_chunk)
+        assert len(set(g_chunk)) == per and set(g_chunk) == set(r_chunk)
+
+
+def test_tile_set_of_the_papers_example():
+    # PAPER.md L141 + L161: n = 9, a = b = 3, GPU 3: I^Q = {3,4,5}; KV footprint {0,1,2} (basic) / {0,3,6} (KVR)
+    for kvr, ikv in ((0, {0, 1, 2}), (1, {0, 3, 6})):
+        t = mk(3, 3, L=128, kvr=kvr).tiles(3)
+        assert {(int(u), int(v)) for u, v, _, _ in t.tolist()} == {(u, v) for u in (3, 4, 5) for v in ikv}
+        assert {(u, v) for u, v, _, _ in po.tile_list(9, 3, 3, bool(kvr), 3, [(0, 0)])} == {(u, v) for u in (3, 4, 5) for v in ikv}
+
+
 @pytest.mark.parametrize("kq,kkv", [(1, 1), (2, 2), (4, 4), (2, 8), (8, 2), (1, 16), (16, 1), (3, 5)])
 @pytest.mark.parametrize("costs", [(1.0, 0.5, 0.5, 0.5), (0.3, 0.7, 0.2, 1.0), (2.0, 2.0, 2.0, 0.1)])
 def test_goo_matches_oracle_and_tile_lists(kq, kkv, costs):
@@ -92,7 +114,7 @@ def test_goo_matches_oracle_and_tile_lists(kq, kkv, costs):
     assert abs(serial - (comm_total + kq * kkv * costs[3])) < 1e-6 and abs(exposed - (makespan - kq * kkv * costs[3])) < 1e-6
     order = po.compute_order(ref)
     for g in range(6):
-        assert [tuple(r) for r in p.tiles(g).tolist()] == po.tile_list(6, 2, 3, True, g, order)
+        _assert_same_tiles(p.tiles(g), po.tile_list(6, 2, 3, True, g, order), order)
 
 
 def test_backward_goo_is_valid():
@@ -126,7 +148,7 @@ def test_backward_goo_is_valid():
 def test_row_major_order_and_queries():
     p = mk(3, 3, L=256, kvr=1, heads_q=4, heads_kv=2, head_dim=128, batch=2)
     t = p.tiles(4)
-    assert [tuple(r) for r in t.tolist()] == po.tile_list(9, 3, 3, True, 4, [(0, 0)])
+    _assert_same_tiles(t, po.tile_list(9, 3, 3, True, 4, [(0, 0)]), [(0, 0)])
     N = 9 * 256
     assert p.query(B.Q_FLOPS_FWD) == 4 * 128 * 4 * 2 * N * N
     assert p.query(B.Q_FLOPS_BWD) == 10 * 128 * 4 * 2 * N * N
@@ -229,13 +251,37 @@ def test_backward_item_pairing_rule():
     non-causal plans, for striped-causal plans (same key block of two KV partitions: the causal offset 0 / -1 does not
     move the first visible Q block), never when the item count is odd or the contiguous causal layout shifts the walks."""
     kw = dict(batch=1, heads_q=2, heads_kv=1, head_dim=128)
-    assert Plan(a=2, b=2, seq_total=4 * 256, **kw).query(B.Q_BWD_PAIRED) == 1
-    assert Plan(a=2, b=2, seq_total=4 * 256, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 1
-    assert Plan(a=4, b=4, seq_total=16 * 256, causal=1, seq_layout=1, order=1, kvr=1, **kw).query(B.Q_BWD_PAIRED) == 1
+    # 2 = paired with the dQ exchange (bwd_pairing = 0, single-operand precision), 1 = paired, shared tile loads only, 0 = single CTAs
+    assert Plan(a=2, b=2, seq_total=4 * 256, **kw).query(B.Q_BWD_PAIRED) == 2
+    assert Plan(a=2, b=2, seq_total=4 * 256, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 2
+    assert Plan(a=4, b=4, seq_total=16 * 256, causal=1, seq_layout=1, order=1, kvr=1, **kw).query(B.Q_BWD_PAIRED) == 2
     assert Plan(a=2, b=2, seq_total=4 * 256, causal=1, seq_layout=0, **kw).query(B.Q_BWD_PAIRED) == 0
     assert Plan(a=1, b=1, seq_total=128, **kw).query(B.Q_BWD_PAIRED) == 0          # a single item
     assert Plan(a=3, b=3, seq_total=9 * 128, causal=1, seq_layout=1, **kw).query(B.Q_BWD_PAIRED) == 0   # 3 partitions per key block
-    assert Plan(a=3, b=3, seq_total=9 * 256, **kw).query(B.Q_BWD_PAIRED) == 1
+    assert Plan(a=3, b=3, seq_total=9 * 256, **kw).query(B.Q_BWD_PAIRED) == 2
+    # the plan descriptor's switch (no environment variable): never / shared loads only; split precision never exchanges
+    assert Plan(a=3, b=3, seq_total=9 * 256, bwd_pairing=1, **kw).query(B.Q_BWD_PAIRED) == 0
+    assert Plan(a=3, b=3, seq_total=9 * 256, bwd_pairing=2, **kw).query(B.Q_BWD_PAIRED) == 1
+    assert Plan(a=3, b=3, seq_total=9 * 256, precision=1, **kw).query(B.Q_BWD_PAIRED) == 1
+    with pytest.raises(MeshAttnError):
+        Plan(a=3, b=3, seq_total=9 * 256, bwd_pairing=3, **kw)
+
+
+def test_segment_lists_do_not_grow_with_batch_and_are_bounded():
+    """FwdItem / BwdItem::seglist are 16 bits: the lists are built once (not per batch index), and a plan that would
+    need more than 32767 of them is refused instead of wrapping to a negative index."""
+    kw = dict(heads_q=1, heads_kv=1, head_dim=64)
+    small = Plan(a=2, b=2, seq_total=4 * 512, batch=1, k_q=4, k_kv=1, order=1, **kw)
+    big = Plan(a=2, b=2, seq_total=4 * 512, batch=9000, k_q=4, k_kv=1, order=1, **kw)      # 36 004 lists before the fix
+    assert big.query(B.Q_FWD_ITEMS_PER_GPU) == 9000 * small.query(B.Q_FWD_ITEMS_PER_GPU)
+    assert big.query(B.Q_BWD_ITEMS_PER_GPU) == 9000 * small.query(B.Q_BWD_ITEMS_PER_GPU)
+    with pytest.raises(MeshAttnError):                      # per-pair partials: k_q * b lists
+        Plan(a=1, b=4096, seq_total=4096 * 2048, batch=1, k_q=16, k_kv=1, partial_mode=1, **kw)
+
+
+def test_plan_health_on_a_host_only_plan():
+    p = Plan(a=2, b=2, seq_total=4 * 128, batch=1, heads_q=1, heads_kv=1, head_dim=64)
+    p.health()                                              # no device, no fault: OK
 
 
 def test_goo_executor_volumes():
