@@ -151,6 +151,7 @@ int upload_plan(mesh_attn_plan* p)
     p->d_bwd_seglists = (const SegList*)put(p->bwd_seglists.data(), p->bwd_seglists.size() * sizeof(SegList), b5);
     p->d_goo_items = (const FwdItem*)put(p->goo_items.data(), p->goo_items.size() * sizeof(FwdItem), b6);
     p->d_goo_bwd_items = (const BwdItem*)put(p->goo_bwd_items.data(), p->goo_bwd_items.size() * sizeof(BwdItem), b7);
+    p->d_counter = (int*)d;                                 // the trailing 256 bytes of the blob
     if (e != cudaSuccess) { cudaFree(p->d_blob); p->d_blob = nullptr; return cuda_fail("cudaMemcpy(work lists)", (int)e); }
     // watchdog status words: pinned host memory the kernels write through its device mapping (no host sync needed to read it)
     e = cudaHostAlloc((void**)&p->h_status, 8 * sizeof(int), cudaHostAllocMapped);
@@ -220,6 +221,11 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
     fp.partial_O = partial_O;
     fp.partial_lse = partial_lse;
     fp.status = p->d_status;
+    fp.counter = p->d_counter + 1;                          // tile_fwd's own counter (a forward and a backward may be in flight on one stream)
+    {
+        const cudaError_t e0 = cudaMemsetAsync(fp.counter, 0, sizeof(int), (cudaStream_t)stream);
+        if (e0 != cudaSuccess) return cuda_fail("tile_fwd: work-item counter", (int)e0);
+    }
     ProfScope prof(MESH_ATTN_K_TILE_FWD, (cudaStream_t)stream);
     const int e = launch_tile_fwd(fp, tmQ, tmK, tmV, p->num_sms, (cudaStream_t)stream);
     if (e) return cuda_fail(who, e);
@@ -337,6 +343,11 @@ static int launch_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count,
     bp.split = p->desc.precision;
     bp.pair = pair;
     bp.status = p->d_status;
+    bp.counter = p->d_counter;
+    {   // the kernel's scheduler warps take work items from this counter
+        const cudaError_t e0 = cudaMemsetAsync(p->d_counter, 0, sizeof(int), (cudaStream_t)stream);
+        if (e0 != cudaSuccess) return cuda_fail("tile_bwd: work-item counter", (int)e0);
+    }
     bp.ws = bwd_ws + ln.hq0 * N;
     bp.ws_plane = (long long)p->geom.batch * p->desc.heads_q * N;
     bp.vec_stride_b = (long long)p->desc.heads_q * N;

@@ -137,6 +137,7 @@ struct mesh_attn_plan {
     // plan reported a fault (1: mbarrier wait timed out, 2: misaligned shared memory), [1..4] = block, thread, barrier, parity
     int* h_status = nullptr;
     int* d_status = nullptr;
+    int* d_counter = nullptr;    // tile_bwd's work-item counter (inside d_blob), zeroed on the launch stream before every launch
     const mesh_attn::FwdItem* d_fwd_items = nullptr;
     const mesh_attn::FwdItem* d_goo_items = nullptr;
     const mesh_attn::BwdItem* d_goo_bwd_items = nullptr;

@@ -88,8 +88,9 @@ template <int D, bool kSplit, bool kExch> struct BwdCfg {
     static constexpr int kOffRecv = kOffStg;                    // aliases the first half of the staging memory (kExch)
     static constexpr int kOffVec = kOffStg + kStgBytes;         // per Q stage: log2(scale)-lse*log2e [128], delta[128] fp32
     static constexpr int kOffBars = kOffVec + kStages * 1024;
-    static constexpr int kNumBars = 2 + 2 * kStages + 12;
-    static constexpr int kSmemBytes = kOffBars + kNumBars * 8 + 16 + kWatchdogBytes;   // + TMEM slot + watchdog state (last 16 bytes)
+    static constexpr int kSchedSlots = 2;                       // ring of work-item indices handed out by the scheduler warp
+    static constexpr int kNumBars = 2 + 2 * kStages + 12 + 3 * kSchedSlots;
+    static constexpr int kSmemBytes = kOffBars + kNumBars * 8 + 16 + 16 + kWatchdogBytes;   // + TMEM slot + item ring + watchdog state (last 16 bytes)
     static constexpr uint32_t kColS = 0, kColDP = 128, kColDK = 256, kColDV = 384;
 };
 
@@ -245,7 +246,11 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* do_empty = s_full + 9;
     uint64_t* send_ok = s_full + 10;                    // kExch: the peer's receive buffer is free for this step's half (remote arrive)
     uint64_t* recv_full = s_full + 11;                  // kExch: the peer's dQ^T half for this CTA's queries has landed in sRecv (transaction count)
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(s_full + 12);
+    uint64_t* sched_full = s_full + 12;                 // [kSchedSlots] the scheduler warp has put the next work-item index into slot k
+    uint64_t* sched_empty = sched_full + Cfg::kSchedSlots;   // [kSchedSlots] every role has read slot k
+    uint64_t* peer_free = sched_empty + Cfg::kSchedSlots;    // [kSchedSlots] kPair, rank 0: the peer's slot k is armed for the next index
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(peer_free + Cfg::kSchedSlots);
+    volatile int* sched_idx = reinterpret_cast<volatile int*>(tmem_slot + 4);
     uint8_t* sdO = smem + Cfg::kOffdO;
     float* sStg = reinterpret_cast<float*>(smem + Cfg::kOffStg);
     auto sQ = [&](int st) { return smem + Cfg::kOffQ + st * Cfg::kTileBytes; };
@@ -257,6 +262,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const int total_items = p.items_per_gpu * p.g_count;
     const long long N = gm.rows_q;
     constexpr int kCompute = 2 * kBlock;                // threads of the two compute groups
+    constexpr int kSchedReaders = 2 + kCompute + kBlock;   // threads that read every work-item index: producer, MMA issuer, compute groups, drain group
 
     if (smem_u32(smem) & 1023u) {                       // the 128-byte swizzle needs a 1024-byte aligned base: report, do not trap
         if (threadIdx.x == 0 && p.status != nullptr && atomicCAS_system(p.status, 0, 2) == 0) { p.status[1] = (int)blockIdx.x; __threadfence_system(); }
@@ -280,6 +286,11 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(do_empty, kPair ? 2 : 1);
         mbar_init(recv_full, 1);
         mbar_init(send_ok, 1);
+        for (int k = 0; k < Cfg::kSchedSlots; ++k) {
+            mbar_init(&sched_full[k], 1);
+            mbar_init(&sched_empty[k], kSchedReaders + ((kPair && cluster_ctarank() == 1) ? 1 : 0));   // rank 1's scheduler reads the ring too
+            mbar_init(&peer_free[k], 1);
+        }
         fence_mbar_init();
     }
     if (warp == 2) tmem_alloc<512>(tmem_slot);
@@ -290,13 +301,64 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     const uint32_t tmem = *tmem_slot;
     const uint32_t pair_rank = kPair ? cluster_ctarank() : 0;
 
+    // Work items are handed out DYNAMICALLY: the scheduler warp takes the next index (the next pair of indices, for a cluster)
+    // from a global counter and publishes it through a ring in shared memory, which every role reads in order.  With the static
+    // round-robin (item = blockIdx.x + k gridDim.x) the persistent CTAs, whose items differ in length under the causal mask, drift
+    // apart by hundreds of items, and the Q / dO / dQ rows they stream stop being shared in L2 (profiles/r02_v1_README.md:
+    // 55 % of the dQ reductions and 58 % of the tile loads of a BASELINE.json configs[4] launch miss L2); taking items in list
+    // order keeps every running CTA inside the same ~148 consecutive items.
+    uint32_t sc_slot = 0, sc_phase = 0;
+    auto next_item = [&]() -> int {
+        if constexpr (kPair) mbar_wait_cluster(&sched_full[sc_slot], sc_phase);   // rank 1's index arrives from the peer (st.async)
+        else mbar_wait(&sched_full[sc_slot], sc_phase);
+        const int v = sched_idx[sc_slot];
+        mbar_arrive(&sched_empty[sc_slot]);
+        if (++sc_slot == Cfg::kSchedSlots) { sc_slot = 0; sc_phase ^= 1; }
+        return v;
+    };
+
     if (warp < 4) reg_dealloc<kCtrlRegs>();
-    if (warp == 0) {
+    if (warp == 3) {
+        // =============================== work-item scheduler ===============================
+        if (elect_one()) {
+            if (!kPair || pair_rank == 0) {
+                const uint32_t peer_idx = kPair ? mapa(smem_u32(const_cast<int*>(sched_idx)), 1u) : 0u;
+                const uint32_t peer_full = kPair ? mapa(smem_u32(sched_full), 1u) : 0u;
+                uint32_t slot = 0, phase = 0;
+                while (true) {
+                    mbar_wait(&sched_empty[slot], phase ^ 1);                    // the slot's previous index has been read by every role
+                    if constexpr (kPair) mbar_wait(&peer_free[slot], phase);     // ... and the peer's slot is armed
+                    const int v = atomicAdd(p.counter, kPair ? 2 : 1);
+                    sched_idx[slot] = v;
+                    mbar_arrive(&sched_full[slot]);
+                    if constexpr (kPair)                                         // the peer takes the odd item of the pair
+                        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                                     ::"r"(peer_idx + slot * 4), "r"(v + 1), "r"(peer_full + slot * 8) : "memory");
+                    if (v >= total_items) break;
+                    if (++slot == Cfg::kSchedSlots) { slot = 0; phase ^= 1; }
+                }
+            } else {
+                // rank 1: arm a slot (expect the 4 bytes of the index), tell rank 0, and follow the ring like every other role to
+                // learn when it ends
+                const uint32_t r0_free = mapa(smem_u32(peer_free), 0u);
+                for (int k = 0; k < Cfg::kSchedSlots; ++k) { mbar_expect_tx(&sched_full[k], 4); mbar_arrive_remote(r0_free + k * 8); }
+                uint32_t slot = 0, phase = 0;
+                while (true) {
+                    const int v = next_item();
+                    if (v >= total_items) break;
+                    mbar_wait(&sched_empty[slot], phase);                        // every role has read it: arm the slot again
+                    mbar_expect_tx(&sched_full[slot], 4);
+                    mbar_arrive_remote(r0_free + slot * 8);
+                    if (++slot == Cfg::kSchedSlots) { slot = 0; phase ^= 1; }
+                }
+            }
+        }
+    } else if (warp == 0) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, kv_phase = 0, do_ph = 0;
             const float* nlse = p.ws + p.ws_plane;                            // ws[1] = log2(scale) - lse*log2e
-            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            for (int idx = next_item(); idx < total_items; idx = next_item()) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
                 QStep q;
@@ -374,7 +436,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
                 return st;
             };
-            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            for (int idx = next_item(); idx < total_items; idx = next_item()) {
                 const BwdItemCtx c = load_bwd_item(p, idx);
                 QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
                 const int nsteps = walk.count_steps();
@@ -582,7 +644,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             tc_fence_before();
             mbar_arrive(ds_full);
         };
-        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+        for (int idx = next_item(); idx < total_items; idx = next_item()) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
             QStep q;
@@ -637,7 +699,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const uint32_t peer_send_ok = kExch ? mapa(smem_u32(send_ok), pair_rank ^ 1u) : 0u;
         uint32_t rf_ph = 0, sok_ph = 0;
         PT_DECL;
-        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+        for (int idx = next_item(); idx < total_items; idx = next_item()) {
             const BwdItemCtx c = load_bwd_item(p, idx);
             QWalk walk(gm, c.segs, c.nseg, c.g, c.v, c.it.t0, c.it.head_kv);
             QStep q;

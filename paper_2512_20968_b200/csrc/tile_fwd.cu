@@ -37,7 +37,8 @@ using namespace sm100;
 namespace {
 
 constexpr int kThreads = 384;
-constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSoftmaxWarp0 = 4;
+constexpr int kLoaderWarp = 0, kMmaWarp = 1, kAllocWarp = 2, kSchedWarp = 3, kSoftmaxWarp0 = 4;
+constexpr int kSchedSlots = 2;           // ring of work-item indices handed out by the scheduler warp
 // register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kSoftmaxRegs <= 65536
 constexpr int kCtrlRegs = 88, kSoftmaxRegs = 208;
 constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
@@ -56,8 +57,8 @@ template <int D> struct FwdCfg {
     static constexpr int kStages = D == 128 ? 5 : 8;       // K/V ring slots (each one tile)
     static constexpr int kSmemQ = 2 * kTileBytes;
     static constexpr int kSmemRing = kStages * kTileBytes;
-    static constexpr int kNumBars = 2 + 2 * kStages + 8;
-    static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 1024 + kWatchdogBytes;   // + TMEM slot, alignment slack, watchdog state (last 16 bytes)
+    static constexpr int kNumBars = 2 + 2 * kStages + 8 + 2 * kSchedSlots;
+    static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 16 + 1024 + kWatchdogBytes;   // + TMEM slot, item ring, alignment slack, watchdog state (last 16 bytes)
     static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
 };
 
@@ -136,7 +137,10 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* s_full = kv_empty + Cfg::kStages;   // [2]
     uint64_t* p_half = s_full + 2;                // [2 sub-tiles][2 column halves]: P is handed to the PV MMA in two halves
     uint64_t* o_full = p_half + 4;                // [2]
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(o_full + 2);
+    uint64_t* sched_full = o_full + 2;            // [kSchedSlots] the scheduler warp has put the next work-item index into slot k
+    uint64_t* sched_empty = sched_full + kSchedSlots;   // [kSchedSlots] every role has read slot k
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sched_empty + kSchedSlots);
+    volatile int* sched_idx = reinterpret_cast<volatile int*>(tmem_slot + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const Geom& gm = p.gm;
@@ -150,6 +154,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
         for (int t = 0; t < 2; ++t) { mbar_init(&s_full[t], 1); mbar_init(&o_full[t], 1); }
         for (int t = 0; t < 4; ++t) mbar_init(&p_half[t], kBlock);
+        for (int k = 0; k < kSchedSlots; ++k) { mbar_init(&sched_full[k], 1); mbar_init(&sched_empty[k], 2 + 2 * kBlock); }   // readers: loader, MMA issuer, softmax groups
         fence_mbar_init();
     }
     if (warp == kAllocWarp) tmem_alloc<512>(tmem_slot);
@@ -158,12 +163,37 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
+    // Work items are handed out DYNAMICALLY (a global counter, published through a ring in shared memory that every role reads
+    // in order): with the static round-robin the persistent CTAs, whose items differ in length under the causal mask, drift
+    // apart by hundreds of items and the K / V blocks they stream stop being shared in L2 (see tile_bwd.cu).
+    uint32_t sc_slot = 0, sc_phase = 0;
+    auto next_item = [&]() -> int {
+        mbar_wait(&sched_full[sc_slot], sc_phase);
+        const int v = sched_idx[sc_slot];
+        mbar_arrive(&sched_empty[sc_slot]);
+        if (++sc_slot == kSchedSlots) { sc_slot = 0; sc_phase ^= 1; }
+        return v;
+    };
+
     if (warp < kSoftmaxWarp0) reg_dealloc<kCtrlRegs>();
-    if (warp == kLoaderWarp) {
+    if (warp == kSchedWarp) {
+        // =============================== work-item scheduler ===============================
+        if (elect_one()) {
+            uint32_t slot = 0, phase = 0;
+            while (true) {
+                mbar_wait(&sched_empty[slot], phase ^ 1);        // the slot's previous index has been read by every role
+                const int v = atomicAdd(p.counter, 1);
+                sched_idx[slot] = v;
+                mbar_arrive(&sched_full[slot]);
+                if (v >= total_items) break;
+                if (++slot == kSchedSlots) { slot = 0; phase ^= 1; }
+            }
+        }
+    } else if (warp == kLoaderWarp) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, q_phase = 0;
-            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            for (int idx = next_item(); idx < total_items; idx = next_item()) {
                 const ItemCtx c = load_item(p, idx);
                 bool first = true;
                 for_each_kv_block(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1, [&](int v, int t0, int) {
@@ -221,7 +251,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                                 umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || k4 > 0 || x > 0) ? 1u : 0u);
                     }
             };
-            for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+            for (int idx = next_item(); idx < total_items; idx = next_item()) {
                 const ItemCtx c = load_item(p, idx);
                 const int nb = count_kv_blocks(gm, c.segs, c.nseg, c.g, c.u, c.it.q0 + c.it.nrows - 1);
                 if (nb == 0) continue;
@@ -269,7 +299,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const float c2 = gm.scale_log2;
         uint32_t s_phase = 0, o_phase = 0;
         PT_DECL;
-        for (int idx = blockIdx.x; idx < total_items; idx += gridDim.x) {
+        for (int idx = next_item(); idx < total_items; idx = next_item()) {
             const ItemCtx c = load_item(p, idx);
             if (t >= c.nt) continue;
             const int srow = c.it.q0 + t * kBlock + row;            // local query row

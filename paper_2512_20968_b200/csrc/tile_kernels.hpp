@@ -34,6 +34,7 @@ struct FwdParams {
     float* partial_O;          // [g_count][slots][B][L][Hq][D]
     float* partial_lse;        // [g_count][slots][B][Hq][L]
     int* status;               // the plan's host-mapped status words (sm100.cuh watchdog); may be null
+    int* counter;              // work-item counter of the launch (device memory; zero when the kernel starts)
 };
 
 struct BwdParams {
@@ -46,8 +47,9 @@ struct BwdParams {
     int split;                 // precision: 1 = hi+lo bf16 operands for P and dS
     int pair;                  // 1: items 2k, 2k+1 walk the same Q blocks -> 2-CTA clusters with multicast Q/dO tiles (tmQ, tmdO: 64-row boxes);
                                // 2: the pair also exchanges dQ^T halves (bf16, distributed shared memory) and each CTA reduces 64 of the
-                               //    step's 128 query rows (tmdQ: 8-row boxes)
+                               //    step's 128 query rows (tmdQ: kBwdStgRowsExch-row boxes)
     int* status;               // the plan's host-mapped status words (sm100.cuh watchdog); may be null
+    int* counter;              // work-item counter of the launch (device memory; zero when the kernel starts)
     const float* ws;           // [2][B][Hq][N]: delta, log2(scale) - lse*log2e (written by bwd_preprocess); head 0 = first head of the lane
     long long ws_plane;        // elements between ws[0] and ws[1] (B * all heads * N)
     long long vec_stride_b;    // batch stride of the [B][Hq][N] vectors (all heads * N)

@@ -80,7 +80,10 @@ def _probe_keys(w, rng):
         loc = loc[p % 3:] + loc[:p % 3]                    # which of the three comes first rotates with the partition
         loc += [int(x) for x in rng.integers(0, w.L, max(0, per - 3))]
         keys += [p * w.L + s for s in loc[:per]]
-    return np.unique(np.asarray(keys, dtype=np.int64))
+    keys = np.unique(np.asarray(keys, dtype=np.int64))
+    while len(keys) < PROBE_KEYS:                          # duplicates collapsed: top up with random rows
+        keys = np.unique(np.concatenate([keys, rng.integers(0, w.seq_total, PROBE_KEYS - len(keys))]))
+    return keys
 
 
 @pytest.mark.parametrize("name", ["C2", "C3", "C4", "C5"])
