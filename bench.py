@@ -46,9 +46,13 @@ def load_traffic(workload: str, kernel: str):
     if not files:
         return None, {"reason": f"no profiles/*_traffic_{workload.lower()}_{kernel}.csv capture for this workload and kernel"}
     f = files[-1]
+    import io
+
     vals = {}
     with open(f, newline="") as fh:
-        for row in csv.DictReader(fh):
+        body = "".join(line for line in fh if line.startswith('"'))       # ncu prefixes the csv with ==PROF== / ==WARNING== lines
+    if True:
+        for row in csv.DictReader(io.StringIO(body)):
             try:
                 vals[row["Metric Name"]] = float(row["Metric Value"].replace(",", ""))
             except (KeyError, ValueError, TypeError):
