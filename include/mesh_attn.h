@@ -91,12 +91,13 @@ typedef struct {
                                  halves the dQ atomics; precision 1 pairs without the exchange), 1 never (single-CTA kernel),
                                  2 paired, shared tile loads only (no dQ exchange).  1 and 2 exist for A/B measurements
                                  and for callers that want the dQ sums free of the exchange's bf16 rounding */
-    int32_t bwd_piece_blocks; /* tile_bwd work items: > 0 cuts the Q sweep of a 128-key block (all Q partitions of the tile) into pieces of
+    int32_t bwd_piece_blocks; /* tile_bwd work items: the Q sweep of a 128-key block (all Q partitions of the tile) is cut into pieces of
                                  at most this many 128-row Q blocks (whole segments = Q chunks of one partition), one work item per
-                                 (key block, piece), the key blocks of a piece adjacent in the list; 0 (default) = one item per key
-                                 block.  Short sweeps keep the Q / dO / dQ rows the running CTAs share in L2, very short ones pay the
-                                 per-item K / V load and dK / dV epilogue more often (measured: DESIGN.md 6.3).  The results are
-                                 the same sums in another order.                                                       */
+                                 (key block, piece), the key blocks of a piece adjacent in the list.  0 = default: pieces whose Q, dO,
+                                 dQ rows (x the query heads of a GQA group) amount to 32 MiB, at least 64 blocks; a large value
+                                 (>= a*L/128) = one item per key block.  Short sweeps keep the rows the running CTAs share in
+                                 L2, very short ones pay the per-item K / V load and dK / dV epilogue more often (measured:
+                                 DESIGN.md 6.3).  The results are the same sums in another order.                       */
     int32_t reserved[2];      /* must be 0                                                             */
 } mesh_attn_plan_desc;
 

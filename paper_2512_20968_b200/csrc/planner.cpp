@@ -221,14 +221,16 @@ void build_worklists(mesh_attn_plan* p)
 
     // ---------- backward: item = (batch, kv_local, kv head, 128-key block) ----------
     // The Q sweep of a key block (every Q chunk of every Q partition of the tile, in the order the C-i-j tasks of KV chunk j
-    // execute) can be cut into PIECES of at most bwd_piece_blocks 128-row blocks, a piece being a run of consecutive segments; a
-    // work item is (key block, piece), and all key blocks of a (KV chunk, head, piece) are adjacent in the list, so that the
-    // CTAs running at the same time sweep the same few MB of Q / dO / dQ rows.  dK / dV of a key block are then accumulated per
-    // piece and added atomically like every other partial sum (Alg.3 l.7).  Default: one piece (the whole sweep).
-    // Measured (profiles/r02_v1_README.md): on a 131 072-token probe 128-block pieces beat 512-block sweeps by 18 %, at
-    // BASELINE.json configs[4] they do not (864 vs 874 TFLOP/s): there the persistent CTAs, which take items round-robin, drift
-    // apart by many pieces, so the shorter sweep does not make them share L2 lines.
-    const int piece_blocks = p->desc.bwd_piece_blocks > 0 ? p->desc.bwd_piece_blocks : (1 << 30);
+    // execute) is cut into PIECES of at most piece_blocks 128-row blocks, a piece being a run of consecutive segments; a work
+    // item is (key block, piece), and all key blocks of a (KV chunk, head, piece) are adjacent in the list, so that the CTAs
+    // running at the same time (the kernels take items in list order) sweep the same Q / dO / dQ rows and find them in L2.
+    // dK / dV of a key block are accumulated per piece and added atomically like every other partial sum (Alg.3 l.7, PAPER.md
+    // L255).  Default: pieces whose working set -- rows x (query heads of a GQA group) x head_dim x (2 + 2 + 4) bytes of Q, dO,
+    // dQ -- is 32 MiB, but not shorter than 64 blocks (every item pays a K / V load and a dK / dV epilogue).  Measured
+    // (profiles/r02_v1_README.md): BASELINE.json configs[3] (GQA 4:1, 128 MiB per sweep) 908 (one piece) / 957 (64 MiB) /
+    // 990 (32 MiB) / 979 (16 MiB) TFLOP/s; configs[4] (64 MiB per sweep) 990 / 990 (32 MiB) / 980 (8 MiB).
+    const long long auto_blocks = (32ll << 20) / ((long long)kBlock * gm.group * gm.head_dim * 8);
+    const int piece_blocks = p->desc.bwd_piece_blocks > 0 ? p->desc.bwd_piece_blocks : (int)std::max<long long>(64, auto_blocks);
     const std::vector<int> kv_chunks_b = first_appearance<int>(p->order_bwd, false);
     struct Piece { int list_id, max_end; };
     std::vector<std::vector<Piece>> bwd_pieces(p->k_kv);   // seg lists per KV chunk, shared by every batch index
