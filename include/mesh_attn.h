@@ -20,7 +20,9 @@
  *     The library owns only the plan object and its small device-resident work lists.
  *   - Hot calls (tile_fwd, merge, bwd_preprocess, tile_bwd, forward, backward) never
  *     allocate, never synchronise the host, never touch the default stream implicitly:
- *     everything is enqueued on `stream`.
+ *     everything is enqueued on `stream` (a tile_fwd / tile_bwd call enqueues a 4-byte memset of
+ *     the plan's work-item counter in front of its kernel: the persistent CTAs take their work
+ *     items from that counter in list order).
  *   - Every function returns a mesh_attn_status (0 = OK, negative = error) and never
  *     throws or aborts; mesh_attn_last_error() gives a thread-local detail string.
  *   - There is no CPU fallback: on a machine without an sm_100 CUDA device (none at all, or another

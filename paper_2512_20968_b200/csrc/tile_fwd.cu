@@ -20,8 +20,8 @@
 // Softmax details, each from a measurement (profiles/): the whole 128-column score row of a thread
 // is held in registers (one TMEM read per block); the reference max only follows the running max
 // when it moved by more than 2^8, so the accumulator rescale is rare; the arithmetic is packed
-// fp32x2; 2 of 8 exponentials run on the FMA pipe (degree-3 polynomial) because the MUFU's 16
-// ex2/clk/SM would otherwise take exactly as long as the MMAs; P is handed over in two 64-key
+// fp32x2; a compile-time fraction of the exponentials can run on the FMA pipe (degree-3 polynomial;
+// MESH_ATTN_POLY_OF_8, default 0: under the power cap the MUFU is the cheaper place); P is handed over in two 64-key
 // halves so the PV MMA starts while the second half is still being exponentiated; single-thread
 // roles are entered through elect.sync so TMA / MMA issue runs on the uniform datapath.
 // kSplit (plan precision = 1): P as hi + lo bf16, two PV MMAs.
@@ -43,8 +43,11 @@ constexpr int kSchedSlots = 2;           // ring of work-item indices handed out
 constexpr int kCtrlRegs = 88, kSoftmaxRegs = 208;
 constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is rescaled only when the row max moved by > 2^8
 #ifndef MESH_ATTN_POLY_OF_8
-#define MESH_ATTN_POLY_OF_8 2            // exponentials per 8 evaluated on the FMA pipe (packed fp32x2 polynomial) instead of the
-                                         // MUFU: measured 0 / 2 / 4 of 8 -> 6.08 / 5.89 / 6.19 ms per C2 launch (profiles/r01_v3_README.md)
+#define MESH_ATTN_POLY_OF_8 0            // exponentials per 8 evaluated on the FMA pipe (packed fp32x2 polynomial) instead of the MUFU.
+                                         // Round 1 (static item order, C2 at burst clocks): 0 / 2 / 4 of 8 -> 6.08 / 5.89 / 6.19 ms per launch.
+                                         // Round 2 (dynamic item order; C5 and C4 run under the power cap, where the polynomial's extra
+                                         // instructions cost clock): C5 tile_fwd 1057 / 1037 / 1040 / 999 / 997 TFLOP/s for 0 / 1 / 2 / 3 / 4 of 8,
+                                         // C4 1056 / 1036 (0 / 1), C2 1124 / 1126: all on the MUFU (profiles/r02_v1_README.md)
 #endif
 
 template <int N> struct IntTag { static constexpr int value = N; };

@@ -163,3 +163,19 @@ def test_mesh_groups_follow_the_assignment_matrix():
     w = W.Workload("m", 7, False, 2, 2, 1, 512, 2, 2, 64, kvr=False)
     with pytest.raises(ValueError):
         mesh_groups(plan_for(w), 4)
+
+
+def test_bench_reads_roofline_traffic_from_profiles():
+    """roofline.traffic comes from an ncu capture under profiles/ (never from a constant in bench.py), with the commit and the
+    kernel-source hash it was taken at; a workload without a capture gets null and a reason."""
+    sys.path.insert(0, str(ROOT))
+    import bench
+    from paper_2512_20968_b200.build import kernel_source_hash
+
+    traffic, src = bench.load_traffic("C5", "tile_bwd")
+    assert traffic and traffic == src["dram_read_bytes"] + src["dram_write_bytes"]
+    assert src["file"].startswith("profiles/") and (ROOT / src["file"]).exists()
+    assert src["kernel_sha16_now"] == kernel_source_hash("tile_bwd") and len(src["kernel_sha16_now"]) == 16
+    assert isinstance(src["matches_current_kernel"], bool) and src["commit"]
+    none, why = bench.load_traffic("C3", "tile_bwd")
+    assert none is None and "reason" in why
