@@ -241,6 +241,30 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_co
 int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
                       float* O, float* lse, float* partial_O, float* partial_lse, void* stream);
 
+/* mesh_attn_forward for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same tile_fwd -> merge waves (Alg.2 l.3-6), with the partial (O, lse)
+ * scratch in a device array BUILT INTO the library -- MESH_ATTN_FORWARD_STATIC_SCRATCH_BYTES per GPU that loads the
+ * library, held until the process exits -- instead of caller-owned partial_O / partial_lse.  The call allocates nothing
+ * (no cudaMalloc / cudaFree, no allocating library routine); Q, K, V, O, lse are the caller's device buffers as in
+ * mesh_attn_forward, and the result is bit-identical to mesh_attn_forward's.
+ *   - Limit: a * (PARTIAL_O_BYTES + PARTIAL_LSE_BYTES) of the plan (mesh_attn_forward_static_limits gives the exact
+ *     figure) must fit the array; a larger plan returns MESH_ATTN_EUNSUPPORTED with both numbers in
+ *     mesh_attn_last_error() and launches nothing.
+ *   - The plan's device must be the current device (EINVAL otherwise): the array's address is looked up per device.
+ *   - Every call, from every plan and thread of the process, shares the ONE array and finds the last call's contents in
+ *     it.  Nothing has to start at zero (tile_fwd writes every partial the merge reads before it is read), but two calls
+ *     that overlap on the GPU (different streams, or different processes' threads on one device without ordering) RACE on
+ *     it: order them on one stream or with events. */
+#define MESH_ATTN_FORWARD_STATIC_SCRATCH_BYTES 33554432 /* 32 MiB */
+int mesh_attn_forward_static(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
+                             float* O, float* lse, void* stream);
+/* need_bytes (may be NULL; needs a plan): scratch bytes a mesh_attn_forward_static call of this plan uses;
+ * capacity_bytes (may be NULL): MESH_ATTN_FORWARD_STATIC_SCRATCH_BYTES.  Host-only, works without a device. */
+int mesh_attn_forward_static_limits(const mesh_attn_plan* plan, int64_t* need_bytes, int64_t* capacity_bytes);
+/* Test hook: fills the whole built-in scratch array with the 32-bit `word` on `stream` (e.g. 0x7FC00000, a NaN), so
+ * that a test can show that a following mesh_attn_forward_static reads nothing it has not written itself. */
+int mesh_attn_forward_static_poison(const mesh_attn_plan* plan, uint32_t word, void* stream);
+
 /* GOO executor for the `a` simulated GPUs of Q group q_group: runs the plan's forward STEP
  * LIST (mesh_attn_plan_steps) step by step.  A step's compute tasks C-i-j (Q chunk i of every Q partition of the group
  * against KV chunk j of every KV partition of each GPU's footprint) are chunk-granular tile_fwd launches on `stream`

@@ -75,6 +75,9 @@ lib.mesh_attn_rank_sum_peers.argtypes = [_P, C.POINTER(_P), C.c_int32, C.c_int64
 lib.mesh_attn_rank_bwd.argtypes = [_P, C.c_int32] + [_P] * 9
 lib.mesh_attn_step_host.argtypes = [_P, C.POINTER(HostIO), _P]
 lib.mesh_attn_plan_health.argtypes = [_P]
+lib.mesh_attn_forward_static.argtypes = [_P] * 7
+lib.mesh_attn_forward_static_limits.argtypes = [_P, C.POINTER(C.c_int64), C.POINTER(C.c_int64)]
+lib.mesh_attn_forward_static_poison.argtypes = [_P, C.c_uint32, _P]
 lib.mesh_attn_launch_count.restype = C.c_int64
 lib.mesh_attn_profile_enable.argtypes = [C.c_int32, C.c_int32]
 lib.mesh_attn_profile_read.argtypes = [C.c_int32, C.POINTER(C.c_double), C.POINTER(C.c_int64)]
@@ -88,6 +91,7 @@ EXPORTED = [
     "mesh_attn_tile_bwd", "mesh_attn_forward", "mesh_attn_forward_goo", "mesh_attn_backward_goo", "mesh_attn_backward", "mesh_attn_step_host", "mesh_attn_launch_count", "mesh_attn_plan_health",
     "mesh_attn_profile_enable", "mesh_attn_profile_read", "mesh_attn_strerror", "mesh_attn_last_error",
     "mesh_attn_rank_fwd", "mesh_attn_rank_merge", "mesh_attn_rank_merge_peers", "mesh_attn_rank_sum_peers", "mesh_attn_rank_bwd_preprocess", "mesh_attn_rank_bwd",
+    "mesh_attn_forward_static", "mesh_attn_forward_static_limits", "mesh_attn_forward_static_poison",
 ]
 K_TILE_FWD, K_MERGE, K_BWD_PREPROCESS, K_TILE_BWD = range(4)
 
@@ -212,6 +216,21 @@ class Plan:
 
     def forward(self, Q, K, V, O, lse, partial_O, partial_lse, stream=None):
         _check(lib.mesh_attn_forward(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _ptr(partial_O), _ptr(partial_lse), _stream(stream)))
+
+    def forward_static(self, Q, K, V, O, lse, stream=None):
+        """forward() with the partial (O, lse) scratch in the library's built-in device array: allocates nothing; plans beyond
+        forward_static_limits()[1] bytes raise MeshAttnError(EUNSUPPORTED); calls that overlap on the GPU race on the array"""
+        _check(lib.mesh_attn_forward_static(self._h, _ptr(Q), _ptr(K), _ptr(V), _ptr(O), _ptr(lse), _stream(stream)))
+
+    def forward_static_limits(self):
+        """(scratch bytes a forward_static of this plan uses, bytes the built-in array holds)"""
+        need, cap = C.c_int64(), C.c_int64()
+        _check(lib.mesh_attn_forward_static_limits(self._h, C.byref(need), C.byref(cap)))
+        return need.value, cap.value
+
+    def forward_static_poison(self, word=0x7FC00000, stream=None):
+        """test hook: fill the built-in scratch array with `word` (default: a NaN)"""
+        _check(lib.mesh_attn_forward_static_poison(self._h, word, _stream(stream)))
 
     def forward_goo(self, q_group, Q, K, V, O, lse, partial_O, partial_lse, comm_ws=None, comm_repeat=0, overlap=True, stream=None):
         nbytes = 0 if comm_ws is None else comm_ws.numel() * comm_ws.element_size()

@@ -17,7 +17,7 @@ CSRC = PKG / "csrc"
 INCLUDE = PKG.parent / "include"
 LIB = PKG / "libmesh_attn.so"
 OBJ = PKG / "build"
-SOURCES = ["planner.cpp", "capi.cu", "tile_fwd.cu", "tile_bwd.cu", "aux_kernels.cu"]
+SOURCES = ["planner.cpp", "capi.cu", "tile_fwd.cu", "tile_bwd.cu", "aux_kernels.cu", "no_alloc.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC", "-Xptxas", "-v", f"-I{INCLUDE}", f"-I{CSRC}",
