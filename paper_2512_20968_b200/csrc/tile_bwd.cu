@@ -57,6 +57,13 @@ constexpr int kBwdThreads = 512;
 #define MESH_ATTN_BWD_POLY_OF_4 0        // exponentials per 4 evaluated on the FMA pipe instead of the MUFU
 #endif
 constexpr int kBwdPolyOf4 = MESH_ATTN_BWD_POLY_OF_4;
+// Ablation builds (tuning only, results are WRONG): bit 0 = the compute groups skip P^T / dS^T (they only pass the barriers on),
+// bit 1 = the dQ drain group skips the TMEM load, the exchange, the staging and the reduces.  What is left of the step time
+// tells which role bounds the kernel (profiles/r02_v4_README.md).
+#ifndef MESH_ATTN_BWD_ABLATE
+#define MESH_ATTN_BWD_ABLATE 0
+#endif
+constexpr int kAblate = MESH_ATTN_BWD_ABLATE;
 // register budget per thread (setmaxnreg): 128 x kCtrlRegs + 256 x kComputeRegs + 128 x kDrainRegs <= 65536
 constexpr int kCtrlRegs = 80, kComputeRegs = 136, kDrainRegs = 160;
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
@@ -551,6 +558,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             s_ph ^= 1;
             tc_fence_after();
             PT_MARK(3);
+            if (kAblate & 1) { tc_fence_before(); mbar_arrive(p_full); return; }
             uint32_t(&pu)[64] = reinterpret_cast<uint32_t(&)[64]>(pr);      // S^T lands in the registers P^T is computed in
             tmem_ld_x32(tS, *reinterpret_cast<uint32_t(*)[32]>(&pu[0]));
             tmem_ld_x32(tS + 32, *reinterpret_cast<uint32_t(*)[32]>(&pu[32]));
@@ -602,6 +610,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             dp_ph ^= 1;
             tc_fence_after();
             PT_MARK(1);
+            if (kAblate & 1) { tc_fence_before(); mbar_arrive(ds_full); return; }
             uint32_t ra[16], rb[16];             // 16-column chunks: chunk c+1 is in flight while chunk c is processed
             auto ds_chunk = [&](int c16, const uint32_t (&r)[16]) {
 #pragma unroll
@@ -705,6 +714,14 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             QStep q;
             while (q.next(walk)) {
                 PT_MARK(0);
+                if (kAblate & 2) {
+                    mbar_wait(dq_full, dq_ph);
+                    dq_ph ^= 1;
+                    tc_fence_after();
+                    tc_fence_before();
+                    mbar_arrive(dq_empty);
+                    continue;
+                }
                 if constexpr (kExch) {
                     // One step of the exchange (see the kernel's header comment).  The staging memory is used twice per step: its
                     // first half receives the peer's bf16 half, then all of it holds this CTA's 64 fp32 rows, reduced as kSlices
