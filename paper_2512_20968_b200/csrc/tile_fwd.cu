@@ -50,6 +50,13 @@ constexpr float kRescaleStep = 8.f;      // log2 domain: the accumulator is resc
                                          // C4 1056 / 1036 (0 / 1), C2 1124 / 1126: all on the MUFU (profiles/r02_v1_README.md)
 #endif
 
+// Ablation build (tuning only, results are WRONG): 1 = the softmax groups skip the TMEM load, the max, the exponentials and the P
+// store (they only pass the barriers on): what is left is the time of the MMAs and the TMA loads (profiles/r02_v4_README.md).
+#ifndef MESH_ATTN_FWD_ABLATE
+#define MESH_ATTN_FWD_ABLATE 0
+#endif
+constexpr int kFwdAblate = MESH_ATTN_FWD_ABLATE;
+
 template <int N> struct IntTag { static constexpr int value = N; };
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
@@ -319,6 +326,13 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mbar_wait(&s_full[t], s_phase);
                 s_phase ^= 1;
                 tc_fence_after();
+                if (kFwdAblate & 1) {
+                    tc_fence_before();
+                    mbar_arrive(&p_half[2 * t]);
+                    mbar_arrive(&p_half[2 * t + 1]);
+                    ++j;
+                    return;
+                }
                 uint32_t s[kBlock];                                 // the whole score row of this thread
 #pragma unroll
                 for (int ch = 0; ch < kBlock / 32; ++ch) tmem_ld_x32(tS + ch * 32, *reinterpret_cast<uint32_t(*)[32]>(&s[ch * 32]));
