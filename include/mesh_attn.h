@@ -32,7 +32,7 @@
  * L = seq_total / n):
  *   Q, dO      bf16  [B, N, Hq,  D]   (tensor_layout 0)  or [B, Hq,  N, D] (tensor_layout 1)
  *   K, V       bf16  [B, N, Hkv, D]                      or [B, Hkv, N, D]
- *   O, dQ      fp32  same shape as Q;   dK, dV fp32 same shape as K
+ *   O, dQ      fp32  same shape as Q;   dK, dV fp32 same shape as K   (bf16 with plan out_dtype = 1, see the field)
  *   lse        fp32  [B, Hq, N]   natural log of the sum of exp of the SCALED scores
  *   partial_O  fp32  [g_count][slots][B][L][Hq][D]   slots = a (partial_mode 0) or a*b (1)
  *   partial_lse fp32 [g_count][slots][B][Hq][L]
@@ -100,7 +100,16 @@ typedef struct {
                                  (>= a*L/128) = one item per key block.  Short sweeps keep the rows the running CTAs share in
                                  L2, very short ones pay the per-item K / V load and dK / dV epilogue more often (measured:
                                  DESIGN.md 6.3).  The results are the same sums in another order.                       */
-    int32_t reserved[2];      /* must be 0                                                             */
+    int32_t out_dtype;        /* 0: O, dQ, dK, dV are fp32 (default); 1: bf16 (round to nearest even, same shapes).  Applies to the O of
+                                 merge / forward / forward_static / forward_goo / step_host, to the O that bwd_preprocess / backward read,
+                                 and to the dQ, dK, dV of backward / step_host, whose sums are then accumulated in fp32 behind the two
+                                 planes of bwd_ws (MESH_ATTN_Q_BWD_WS_BYTES grows by the three fp32 tensors) and rounded once at the end.
+                                 lse, the partials and the per-kernel call mesh_attn_tile_bwd (which ACCUMULATES into caller buffers)
+                                 stay fp32; backward_goo and the per-rank calls return EUNSUPPORTED.  The backward then sees the ROUNDED O:
+                                 delta = rowsum(dO o O) carries up to 2^-9 sum|dO O| of rounding, which reaches dQ, dK (measured
+                                 1.6e-2 max against the fp32 path on a causal case; dV is unaffected).  An option beyond the paper's
+                                 (unpinned: tests compare against the fp32 path and the oracle at that resolution).              */
+    int32_t reserved[1];      /* must be 0                                                             */
 } mesh_attn_plan_desc;
 
 /* what = ... for mesh_attn_plan_query */
@@ -117,7 +126,7 @@ enum {
     MESH_ATTN_Q_BLOCKS_FWD = 9,        /* 128x128 score blocks the forward computes (all GPUs, heads)     */
     MESH_ATTN_Q_COMM_UNITS = 10,       /* paper's aggregate communication units of this AM   */
     MESH_ATTN_Q_HAS_DEVICE = 11,       /* 1 if the plan's work lists are resident on a CUDA device        */
-    MESH_ATTN_Q_BWD_WS_BYTES = 12,     /* bytes of the backward workspace bwd_ws: 2*B*Hq*N*4               */
+    MESH_ATTN_Q_BWD_WS_BYTES = 12,     /* bytes of the backward workspace bwd_ws: 2*B*Hq*N*4 (+ B*N*(Hq+2Hkv)*D*4 with out_dtype 1) */
     /* planner analytics (what the paper's cluster would move; nothing here is executed): */
     MESH_ATTN_Q_MESH_COMM_BYTES_FWD = 13,  /* per-GPU forward volume of this a x b tiling, closed form
                                               2(a+b-2) N d / n elements x 2 bytes (bf16), d = Hq*head_dim */
@@ -212,7 +221,7 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_co
  * g_count = a.  Writes rows of partitions u of O [B,N,Hq,D] and lse [B,Hq,N]. */
 int mesh_attn_merge(const mesh_attn_plan* plan, int32_t q_group,
                     const float* partial_O, const float* partial_lse,
-                    float* O, float* lse, void* stream);
+                    void* O /* fp32; bf16 with out_dtype 1 */, float* lse, void* stream);
 
 /* Backward workspace bwd_ws, fp32 [2][B][Hq][N] (MESH_ATTN_Q_BWD_WS_BYTES), all rows:
  *   bwd_ws[0][b,h,row] = delta = sum_d dO * O  (needed by every pair touching the row; the
@@ -220,7 +229,7 @@ int mesh_attn_merge(const mesh_attn_plan* plan, int32_t q_group,
  *   bwd_ws[1][b,h,row] = log2(softmax_scale) - lse * log2(e)  (exponent offset, in base 2, of
  *                        scale * P = scale * exp(S - lse); lse is the FINAL merged LSE,
  *                        DESIGN.md reading R8) */
-int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const float* O, const void* dO,
+int mesh_attn_bwd_preprocess(const mesh_attn_plan* plan, const void* O /* fp32; bf16 with out_dtype 1 */, const void* dO,
                              const float* lse, float* bwd_ws, void* stream);
 
 /* Alg.3 l.3-5 for simulated GPUs g_first..: for each pair of the tile
@@ -239,7 +248,7 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* plan, int32_t g_first, int32_t g_co
  * merge(lane*b + r). partial_O / partial_lse must hold `a` simulated GPUs (query PARTIAL_*_BYTES * a).
  * tile_fwd / tile_bwd ranges [g_first, g_first+g_count) must stay inside one lane (EINVAL). */
 int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
-                      float* O, float* lse, float* partial_O, float* partial_lse, void* stream);
+                      void* O /* fp32; bf16 with out_dtype 1 */, float* lse, float* partial_O, float* partial_lse, void* stream);
 
 /* mesh_attn_forward for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
  * harnesses that forbid cudaMalloc): the same tile_fwd -> merge waves (Alg.2 l.3-6), with the partial (O, lse)
@@ -257,7 +266,7 @@ int mesh_attn_forward(const mesh_attn_plan* plan, const void* Q, const void* K, 
  *     it: order them on one stream or with events. */
 #define MESH_ATTN_FORWARD_STATIC_SCRATCH_BYTES 33554432 /* 32 MiB */
 int mesh_attn_forward_static(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
-                             float* O, float* lse, void* stream);
+                             void* O /* fp32; bf16 with out_dtype 1 */, float* lse, void* stream);
 /* need_bytes (may be NULL; needs a plan): scratch bytes a mesh_attn_forward_static call of this plan uses;
  * capacity_bytes (may be NULL): MESH_ATTN_FORWARD_STATIC_SCRATCH_BYTES.  Host-only, works without a device. */
 int mesh_attn_forward_static_limits(const mesh_attn_plan* plan, int64_t* need_bytes, int64_t* capacity_bytes);
@@ -276,7 +285,7 @@ int mesh_attn_forward_static_poison(const mesh_attn_plan* plan, uint32_t word, v
  * the schedule's timing, the result is the attention of mesh_attn_forward.  partial_O / partial_lse: `a` x
  * MESH_ATTN_Q_GOO_PARTIAL_*_BYTES.  Time it with events on `stream`. */
 int mesh_attn_forward_goo(const mesh_attn_plan* plan, int32_t q_group, const void* Q, const void* K, const void* V,
-                          float* O, float* lse, float* partial_O, float* partial_lse,
+                          void* O /* fp32; bf16 with out_dtype 1 */, float* lse, float* partial_O, float* partial_lse,
                           void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap, void* stream);
 
 /* ---- per-rank calls (Alg.2, Alg.3) ----------------------
@@ -334,10 +343,11 @@ int mesh_attn_backward_goo(const mesh_attn_plan* plan, int32_t q_group, const vo
                            const float* bwd_ws, float* dQ, float* dK, float* dV,
                            void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap, void* stream);
 
-/* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs. */
+/* Zero dQ,dK,dV; bwd_preprocess; tile_bwd over all n simulated GPUs.  O, dQ, dK, dV: fp32, or bf16 with out_dtype 1 (the sums
+ * are then accumulated in fp32 inside bwd_ws and rounded once, by three cast launches at the end). */
 int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K, const void* V,
-                       const float* O, const void* dO, const float* lse, float* bwd_ws,
-                       float* dQ, float* dK, float* dV, void* stream);
+                       const void* O, const void* dO, const float* lse, float* bwd_ws,
+                       void* dQ, void* dK, void* dV, void* stream);
 
 /* End-to-end step with HOST buffers (pinned or pageable): copies Q,K,V(,dO) host->device
  * into the caller's device staging buffers, runs forward (and backward if dO_host != NULL),
@@ -351,9 +361,10 @@ int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K,
  * shapes above. */
 typedef struct {
     const void *Q_host, *K_host, *V_host, *dO_host;      /* bf16 host inputs (dO_host may be NULL) */
-    float *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* fp32 host outputs (any may be NULL = not copied back) */
+    void *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* host outputs (any may be NULL = not copied back): lse fp32; O, dQ, dK, dV
+                                                              fp32, or bf16 with out_dtype 1 (half the bytes down) */
     void *d_Q, *d_K, *d_V, *d_dO;                          /* device staging                         */
-    float *d_O, *d_lse, *d_bwd_ws, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;
+    void *d_O, *d_lse, *d_bwd_ws, *d_dQ, *d_dK, *d_dV, *d_partial_O, *d_partial_lse;   /* d_O, d_dQ, d_dK, d_dV: dtype as the host outputs */
 } mesh_attn_host_io;
 int mesh_attn_step_host(const mesh_attn_plan* plan, const mesh_attn_host_io* io, void* stream);
 

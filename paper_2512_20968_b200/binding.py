@@ -37,7 +37,7 @@ class PlanDesc(C.Structure):
         ("gamma", C.c_float), ("t_ag_q", C.c_float), ("t_ag_kv", C.c_float), ("t_rs_q", C.c_float), ("t_c", C.c_float),
         ("softmax_scale", C.c_float),
         ("tensor_layout", C.c_int32), ("partial_mode", C.c_int32), ("precision", C.c_int32),
-        ("usp_lanes", C.c_int32), ("bwd_pairing", C.c_int32), ("bwd_piece_blocks", C.c_int32), ("reserved", C.c_int32 * 2),
+        ("usp_lanes", C.c_int32), ("bwd_pairing", C.c_int32), ("bwd_piece_blocks", C.c_int32), ("out_dtype", C.c_int32), ("reserved", C.c_int32 * 1),
     ]
 
 

@@ -2,6 +2,7 @@
 //   merge_kernel   LSE-weighted merge of the partial outputs of a Q group (online-softmax
 //                  reducer of PAPER.md L77, Alg.2 l.6 L174; reading R4)
 //   delta_kernel   backward preprocess Delta = rowsum(dO o O), plus -lse*log2e
+//   cast_kernel    plan out_dtype = 1: the fp32 gradient accumulators -> the caller's bf16 dQ, dK, dV
 // Both are streaming kernels: 16-byte vector loads, many independent loads in flight per
 // thread, streaming cache hints, no shared-memory reuse of the bulk data.
 #include <algorithm>
@@ -22,6 +23,17 @@ __device__ __forceinline__ float4 ld_stream(const float4* p)
 __device__ __forceinline__ void st_stream(float4* p, const float4& v)
 {
     asm volatile("st.global.cs.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(p), "f"(v.x), "f"(v.y), "f"(v.z), "f"(v.w) : "memory");
+}
+
+__device__ __forceinline__ uint2 pack4_bf16(const float4& v)
+{
+    const __nv_bfloat162 lo = __floats2bfloat162_rn(v.x, v.y), hi = __floats2bfloat162_rn(v.z, v.w);
+    return make_uint2(*reinterpret_cast<const uint32_t*>(&lo), *reinterpret_cast<const uint32_t*>(&hi));
+}
+__device__ __forceinline__ void st_stream_bf16x4(void* p, const float4& v)
+{
+    const uint2 w = pack4_bf16(v);
+    asm volatile("st.global.cs.v2.b32 [%0], {%1, %2};" ::"l"(p), "r"(w.x), "r"(w.y) : "memory");
 }
 
 constexpr int kMergeThreads = 256;
@@ -95,8 +107,9 @@ __global__ void __launch_bounds__(kMergeThreads) merge_kernel(const MergeParams 
             }
         }
         const int r = rh / Hq, h = rh - r * Hq;
-        float* dst = p.O + (size_t)bt * p.o_stride_b + ((size_t)u * gm.L + s0 + r) * p.o_stride_row + (size_t)h * p.o_stride_h + d4 * 4;
-        st_stream(reinterpret_cast<float4*>(dst), acc);
+        const size_t at = (size_t)bt * p.o_stride_b + ((size_t)u * gm.L + s0 + r) * p.o_stride_row + (size_t)h * p.o_stride_h + d4 * 4;
+        if (p.out_bf16) st_stream_bf16x4(reinterpret_cast<__nv_bfloat16*>(p.O) + at, acc);
+        else st_stream(reinterpret_cast<float4*>(reinterpret_cast<float*>(p.O) + at), acc);
     }
 }
 
@@ -114,14 +127,24 @@ __global__ void __launch_bounds__(256) delta_kernel(const DeltaParams p)
     const int bt = (int)(wid / ((long long)gm.heads_q * N));
     const size_t base = (size_t)bt * p.stride_b + (size_t)row * p.stride_row + (size_t)h * p.stride_h;
     const __nv_bfloat16* dO = reinterpret_cast<const __nv_bfloat16*>(p.dO) + base;
-    const float* O = p.O + base;
     float acc = 0.f;
-    if (D == 128) {
+    if (p.o_bf16) {                              // the forward wrote O as bf16 (plan out_dtype = 1)
+        const __nv_bfloat16* O = reinterpret_cast<const __nv_bfloat16*>(p.O) + base;
+        constexpr int kPer = D / 32;             // elements per lane
+#pragma unroll
+        for (int i = 0; i < kPer; i += 2) {
+            const __nv_bfloat162 o = *reinterpret_cast<const __nv_bfloat162*>(O + lane * kPer + i);
+            const __nv_bfloat162 g = *reinterpret_cast<const __nv_bfloat162*>(dO + lane * kPer + i);
+            acc += __low2float(o) * __low2float(g) + __high2float(o) * __high2float(g);
+        }
+    } else if (D == 128) {
+        const float* O = reinterpret_cast<const float*>(p.O) + base;
         const float4 o = *reinterpret_cast<const float4*>(O + lane * 4);
         const uint2 g = *reinterpret_cast<const uint2*>(dO + lane * 4);
         const __nv_bfloat162 g0 = *reinterpret_cast<const __nv_bfloat162*>(&g.x), g1 = *reinterpret_cast<const __nv_bfloat162*>(&g.y);
         acc = o.x * __low2float(g0) + o.y * __high2float(g0) + o.z * __low2float(g1) + o.w * __high2float(g1);
     } else {
+        const float* O = reinterpret_cast<const float*>(p.O) + base;
         const float2 o = *reinterpret_cast<const float2*>(O + lane * 2);
         const __nv_bfloat162 g = *reinterpret_cast<const __nv_bfloat162*>(dO + lane * 2);
         acc = o.x * __low2float(g) + o.y * __high2float(g);
@@ -157,7 +180,24 @@ __global__ void __launch_bounds__(256) sum_peers_kernel(const SumParams p)
     }
 }
 
+// dst (bf16) = src (fp32), float4 granularity, grid-stride
+__global__ void __launch_bounds__(256) cast_kernel(const float* __restrict__ src, void* dst, long long count4)
+{
+    const long long stride = (long long)gridDim.x * blockDim.x;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < count4; i += stride)
+        st_stream_bf16x4(reinterpret_cast<uint2*>(dst) + i, ld_stream(reinterpret_cast<const float4*>(src) + i));
+}
+
 }  // namespace
+
+int launch_cast_bf16(const float* src, void* dst, long long count, int num_sms, cudaStream_t stream)
+{
+    const long long count4 = count / 4, blocks = (count4 + 255) / 256;
+    const unsigned grid = (unsigned)std::min<long long>(blocks, (long long)num_sms * 16);
+    if (grid == 0) return 0;
+    cast_kernel<<<grid, 256, 0, stream>>>(src, dst, count4);
+    return (int)cudaGetLastError();
+}
 
 int launch_sum_peers(const SumParams& p, int num_sms, cudaStream_t stream)
 {

@@ -55,6 +55,22 @@ template <class T> T* head_slice(T* base, long long h0, const Strides& s, int el
     return (T*)((char*)base + h0 * s.h * elem_bytes);
 }
 
+// plan out_dtype: bytes per element of O (and of dQ, dK, dV in the composite calls)
+int out_bytes(const mesh_attn_plan* p) { return p->desc.out_dtype == 1 ? 2 : 4; }
+// fp32 accumulators of dQ, dK, dV behind the two planes of bwd_ws (out_dtype = 1 only)
+struct GradAcc { float *dQ, *dK, *dV; size_t nq, nk; };
+GradAcc grad_acc(const mesh_attn_plan* p, float* bwd_ws)
+{
+    const size_t N = (size_t)p->geom.n * p->geom.L, B = p->geom.batch, D = p->geom.head_dim;
+    GradAcc a;
+    a.nq = B * N * p->desc.heads_q * D;
+    a.nk = B * N * p->desc.heads_kv * D;
+    a.dQ = bwd_ws + 2 * B * p->desc.heads_q * N;
+    a.dK = a.dQ + a.nq;
+    a.dV = a.dK + a.nk;
+    return a;
+}
+
 // bf16 tensor map of the lane's head slice: H_lane heads starting at h0 of a tensor with H_all heads
 bool make_map(const mesh_attn_plan* p, CUtensorMap* m, const void* base, int H_lane, int H_all, long long h0, int box_rows = kBlock,
               long long rows = 0)
@@ -234,7 +250,7 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
 }
 
 static int launch_merge_slots(const mesh_attn_plan* p, int32_t q_group, int per, int slots_per_gpu, const float* partial_O, const float* partial_lse,
-                              float* O, float* lse, void* stream)
+                              void* O, float* lse, void* stream)
 {
     if (int rc = check_device(p, "merge")) return rc;
     if (!partial_O || !partial_lse || !O || !lse) return fail(MESH_ATTN_EINVAL, "merge: null pointer");
@@ -259,7 +275,8 @@ static int launch_merge_slots(const mesh_attn_plan* p, int32_t q_group, int per,
     mp.partial_O = partial_O;
     mp.partial_lse = partial_lse;
     const Strides s = strides_of(p, p->desc.heads_q);
-    mp.O = head_slice(O, ln.hq0, s, 4);
+    mp.O = head_slice((char*)O, ln.hq0, s, out_bytes(p));
+    mp.out_bf16 = p->desc.out_dtype == 1;
     mp.lse = lse + ln.hq0 * N;
     mp.lse_stride_b = (long long)p->desc.heads_q * N;
     mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
@@ -278,14 +295,14 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
                            "tile_fwd");
 }
 
-int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, float* O, float* lse,
+int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, void* O, float* lse,
                     void* stream)
 {
     if (int rc = check_device(p, "merge")) return rc;
     return launch_merge_slots(p, q_group, p->desc.partial_mode == 1 ? p->geom.b : 1, p->geom.slots_per_gpu, partial_O, partial_lse, O, lse, stream);
 }
 
-int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void* dO, const float* lse, float* bwd_ws, void* stream)
+int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const void* O, const void* dO, const float* lse, float* bwd_ws, void* stream)
 {
     if (int rc = check_device(p, "bwd_preprocess")) return rc;
     if (!O || !dO || !lse || !bwd_ws) return fail(MESH_ATTN_EINVAL, "bwd_preprocess: null pointer");
@@ -294,6 +311,7 @@ int mesh_attn_bwd_preprocess(const mesh_attn_plan* p, const float* O, const void
     dp.gm.heads_q = p->desc.heads_q;      // all lanes in one launch
     dp.gm.heads_kv = p->desc.heads_kv;
     dp.O = O; dp.dO = dO; dp.lse = lse; dp.ws = bwd_ws;
+    dp.o_bf16 = p->desc.out_dtype == 1;
     const Strides s = strides_of(p, p->desc.heads_q);
     dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
@@ -372,8 +390,8 @@ int mesh_attn_tile_bwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
 static int check_rank(const mesh_attn_plan* p, int32_t g, const char* who)
 {
     if (int rc = check_device(p, who)) return rc;
-    if (lanes_of(p) != 1 || p->desc.partial_mode != 0)
-        return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": per-rank calls need usp_lanes == 1 and partial_mode == 0");
+    if (lanes_of(p) != 1 || p->desc.partial_mode != 0 || p->desc.out_dtype != 0)
+        return fail(MESH_ATTN_EUNSUPPORTED, std::string(who) + ": per-rank calls need usp_lanes == 1, partial_mode == 0 and out_dtype == 0");
     if (g < 0 || g >= p->geom.n) return fail(MESH_ATTN_EINVAL, std::string(who) + ": rank g out of range");
     return MESH_ATTN_OK;
 }
@@ -418,6 +436,7 @@ static int launch_rank_merge(const mesh_attn_plan* p, const float* partial_O_rec
     mp.partial_lse = partial_lse_recv;
     const Strides s = strides_of(p, g0.heads_q, g0.L);
     mp.O = O_own;
+    mp.out_bf16 = 0;
     mp.lse = lse_own;
     mp.lse_stride_b = (long long)g0.heads_q * g0.L;
     mp.o_stride_b = s.b; mp.o_stride_row = s.row; mp.o_stride_h = s.h;
@@ -470,6 +489,7 @@ int mesh_attn_rank_bwd_preprocess(const mesh_attn_plan* p, const float* O_own, c
     dp.gm = p->geom;
     dp.gm.rows_q = p->geom.L;
     dp.O = O_own; dp.dO = dO_own; dp.lse = lse_own; dp.ws = ws_own;
+    dp.o_bf16 = 0;
     const Strides s = strides_of(p, p->geom.heads_q, p->geom.L);
     dp.stride_b = s.b; dp.stride_row = s.row; dp.stride_h = s.h;
     ProfScope prof(MESH_ATTN_K_BWD_PREPROCESS, (cudaStream_t)stream);
@@ -486,7 +506,7 @@ int mesh_attn_rank_bwd(const mesh_attn_plan* p, int32_t g, const void* Q_loc, co
     return launch_bwd(p, g, 1, Q_loc, K_loc, V_loc, dO_loc, ws_loc, dQ_loc, dK_loc, dV_loc, stream, true);
 }
 
-int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, float* O, float* lse, float* partial_O,
+int mesh_attn_forward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, void* O, float* lse, float* partial_O,
                       float* partial_lse, void* stream)
 {
     if (int rc = check_device(p, "forward")) return rc;
@@ -511,7 +531,7 @@ static long long goo_task_bytes(const mesh_attn_plan* p, int kind)
     }
 }
 
-int mesh_attn_forward_goo(const mesh_attn_plan* p, int32_t q_group, const void* Q, const void* K, const void* V, float* O, float* lse,
+int mesh_attn_forward_goo(const mesh_attn_plan* p, int32_t q_group, const void* Q, const void* K, const void* V, void* O, float* lse,
                           float* partial_O, float* partial_lse, void* comm_ws, int64_t comm_ws_bytes, int32_t comm_repeat, int32_t overlap,
                           void* stream)
 {
@@ -581,6 +601,7 @@ int mesh_attn_backward_goo(const mesh_attn_plan* p, int32_t q_group, const void*
                            int32_t overlap, void* stream)
 {
     if (int rc = check_device(p, "backward_goo")) return rc;
+    if (p->desc.out_dtype != 0) return fail(MESH_ATTN_EUNSUPPORTED, "backward_goo: accumulates into fp32 dQ, dK, dV (plan out_dtype must be 0)");
     if (!Q || !K || !V || !dO || !bwd_ws || !dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward_goo: null pointer");
     if (comm_repeat < 0 || (comm_repeat > 0 && (!comm_ws || comm_ws_bytes < 4096))) return fail(MESH_ATTN_EINVAL, "backward_goo: comm_ws too small");
     const Geom& gm = p->geom;
@@ -642,23 +663,35 @@ int mesh_attn_backward_goo(const mesh_attn_plan* p, int32_t q_group, const void*
     return MESH_ATTN_OK;
 }
 
-int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const float* O, const void* dO,
-                       const float* lse, float* bwd_ws, float* dQ, float* dK, float* dV, void* stream)
+int mesh_attn_backward(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, const void* O, const void* dO,
+                       const float* lse, float* bwd_ws, void* dQ, void* dK, void* dV, void* stream)
 {
     if (int rc = check_device(p, "backward")) return rc;
-    if (!dQ || !dK || !dV) return fail(MESH_ATTN_EINVAL, "backward: null pointer");
+    if (!dQ || !dK || !dV || !bwd_ws) return fail(MESH_ATTN_EINVAL, "backward: null pointer");
     const Geom& gm = p->geom;
-    const size_t N = (size_t)gm.n * gm.L;
     cudaStream_t st = (cudaStream_t)stream;
-    cudaError_t e = cudaMemsetAsync(dQ, 0, (size_t)gm.batch * N * p->desc.heads_q * gm.head_dim * 4, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(dK, 0, (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim * 4, st);
-    if (e == cudaSuccess) e = cudaMemsetAsync(dV, 0, (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim * 4, st);
+    // out_dtype = 1: the atomics accumulate in fp32 behind the two planes of bwd_ws; dQ, dK, dV receive the rounded sums
+    const bool bf16_out = p->desc.out_dtype == 1;
+    const GradAcc acc = grad_acc(p, bwd_ws);
+    float* aQ = bf16_out ? acc.dQ : (float*)dQ;
+    float* aK = bf16_out ? acc.dK : (float*)dK;
+    float* aV = bf16_out ? acc.dV : (float*)dV;
+    cudaError_t e = cudaMemsetAsync(aQ, 0, acc.nq * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(aK, 0, acc.nk * 4, st);
+    if (e == cudaSuccess) e = cudaMemsetAsync(aV, 0, acc.nk * 4, st);
     if (e != cudaSuccess) return cuda_fail("backward memset", (int)e);
     if (int rc = mesh_attn_bwd_preprocess(p, O, dO, lse, bwd_ws, stream)) return rc;
     // keep each launch's work-item count below 2^31: one call per Q group
     for (int lane = 0; lane < lanes_of(p); ++lane)
         for (int r = 0; r < gm.b; ++r)
-            if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, Q, K, V, dO, bwd_ws, dQ, dK, dV, stream)) return rc;
+            if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, Q, K, V, dO, bwd_ws, aQ, aK, aV, stream)) return rc;
+    if (bf16_out) {
+        int err = launch_cast_bf16(aQ, dQ, (long long)acc.nq, p->num_sms, st);
+        if (!err) err = launch_cast_bf16(aK, dK, (long long)acc.nk, p->num_sms, st);
+        if (!err) err = launch_cast_bf16(aV, dV, (long long)acc.nk, p->num_sms, st);
+        if (err) return cuda_fail("backward cast launch", err);
+        g_launches.fetch_add(3);
+    }
     return MESH_ATTN_OK;
 }
 
@@ -675,6 +708,13 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
     const size_t N = (size_t)gm.n * gm.L;
     const size_t nq = (size_t)gm.batch * N * p->desc.heads_q * gm.head_dim, nk = (size_t)gm.batch * N * p->desc.heads_kv * gm.head_dim;
     const size_t nl = (size_t)gm.batch * N * p->desc.heads_q;
+    // out_dtype = 1: O, dQ, dK, dV (device and host) are bf16; the gradients accumulate in fp32 behind the planes of d_bwd_ws
+    const bool bf16_out = p->desc.out_dtype == 1;
+    const size_t ob = (size_t)out_bytes(p);
+    const GradAcc acc = grad_acc(p, (float*)io->d_bwd_ws);
+    float* aQ = bf16_out ? acc.dQ : (float*)io->d_dQ;
+    float* aK = bf16_out ? acc.dK : (float*)io->d_dK;
+    float* aV = bf16_out ? acc.dV : (float*)io->d_dV;
     cudaStream_t st = (cudaStream_t)stream, up = (cudaStream_t)p->s_h2d, down = (cudaStream_t)p->s_d2h;
     auto ev = [&](int i) { return (cudaEvent_t)p->copy_events[i]; };
     // events: 0 start, 1 K,V on the device, 2 dO on the device, 3 forward done, 4 backward done, 5 copies back done,
@@ -707,39 +747,53 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
         for (int r = 0; r < nb; ++r) {
             if (lane == 0 && ok()) e = cudaStreamWaitEvent(st, ev(6 + r), 0);
             if (!ok()) return cuda_fail("step_host forward", (int)e);
-            if (int rc = mesh_attn_tile_fwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_partial_O, io->d_partial_lse, stream)) return rc;
-            if (int rc = mesh_attn_merge(p, lane * nb + r, io->d_partial_O, io->d_partial_lse, io->d_O, io->d_lse, stream)) return rc;
+            if (int rc = mesh_attn_tile_fwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, (float*)io->d_partial_O, (float*)io->d_partial_lse, stream)) return rc;
+            if (int rc = mesh_attn_merge(p, lane * nb + r, (const float*)io->d_partial_O, (const float*)io->d_partial_lse, io->d_O, (float*)io->d_lse, stream)) return rc;
         }
     e = cudaEventRecord(ev(3), st);
     if (ok()) e = cudaStreamWaitEvent(down, ev(3), 0);
-    if (ok() && io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * 4, cudaMemcpyDeviceToHost, down);   // during the backward
+    if (ok() && io->O_host) e = cudaMemcpyAsync(io->O_host, io->d_O, nq * ob, cudaMemcpyDeviceToHost, down);   // during the backward
     if (ok() && io->lse_host) e = cudaMemcpyAsync(io->lse_host, io->d_lse, nl * 4, cudaMemcpyDeviceToHost, down);
     if (bwd) {
         // ---- backward: the simulated GPUs of Q group r hold exactly the Q partitions of group r, so dQ of those rows is
         // final once the last lane's call for r has run (Alg.3 l.6)
         if (ok()) e = cudaStreamWaitEvent(st, ev(2), 0);
-        if (ok()) e = cudaMemsetAsync(io->d_dQ, 0, nq * 4, st);
-        if (ok()) e = cudaMemsetAsync(io->d_dK, 0, nk * 4, st);
-        if (ok()) e = cudaMemsetAsync(io->d_dV, 0, nk * 4, st);
+        if (ok()) e = cudaMemsetAsync(aQ, 0, nq * 4, st);
+        if (ok()) e = cudaMemsetAsync(aK, 0, nk * 4, st);
+        if (ok()) e = cudaMemsetAsync(aV, 0, nk * 4, st);
         if (!ok()) return cuda_fail("step_host backward setup", (int)e);
-        if (int rc = mesh_attn_bwd_preprocess(p, io->d_O, io->d_dO, io->d_lse, io->d_bwd_ws, stream)) return rc;
+        if (int rc = mesh_attn_bwd_preprocess(p, io->d_O, io->d_dO, (const float*)io->d_lse, (float*)io->d_bwd_ws, stream)) return rc;
         for (int lane = 0; lane < U; ++lane)
             for (int r = 0; r < nb; ++r) {
-                if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_dO, io->d_bwd_ws, io->d_dQ, io->d_dK,
-                                                io->d_dV, stream))
+                if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_dO, (const float*)io->d_bwd_ws, aQ, aK,
+                                                aV, stream))
                     return rc;
-                if (lane == U - 1 && by_group && io->dQ_host) {
-                    e = cudaEventRecord(ev(6 + nb + r), st);
-                    if (ok()) e = cudaStreamWaitEvent(down, ev(6 + nb + r), 0);
-                    if (ok()) e = cudaMemcpyAsync(io->dQ_host + r * q_chunk, io->d_dQ + r * q_chunk, q_chunk * 4, cudaMemcpyDeviceToHost, down);
-                    if (!ok()) return cuda_fail("step_host dQ D2H", (int)e);
+                if (lane == U - 1 && by_group) {
+                    if (bf16_out) {                  // the rows of Q group r are final: round them into the caller's dQ
+                        if (int err = launch_cast_bf16(aQ + r * q_chunk, (char*)io->d_dQ + r * q_chunk * 2, (long long)q_chunk, p->num_sms, st))
+                            return cuda_fail("step_host cast launch", err);
+                        g_launches.fetch_add(1);
+                    }
+                    if (io->dQ_host) {
+                        e = cudaEventRecord(ev(6 + nb + r), st);
+                        if (ok()) e = cudaStreamWaitEvent(down, ev(6 + nb + r), 0);
+                        if (ok()) e = cudaMemcpyAsync((char*)io->dQ_host + r * q_chunk * ob, (const char*)io->d_dQ + r * q_chunk * ob, q_chunk * ob, cudaMemcpyDeviceToHost, down);
+                        if (!ok()) return cuda_fail("step_host dQ D2H", (int)e);
+                    }
                 }
             }
+        if (bf16_out) {
+            int err = by_group ? 0 : launch_cast_bf16(aQ, io->d_dQ, (long long)nq, p->num_sms, st);
+            if (!err) err = launch_cast_bf16(aK, io->d_dK, (long long)nk, p->num_sms, st);
+            if (!err) err = launch_cast_bf16(aV, io->d_dV, (long long)nk, p->num_sms, st);
+            if (err) return cuda_fail("step_host cast launch", err);
+            g_launches.fetch_add(by_group ? 2 : 3);
+        }
         e = cudaEventRecord(ev(4), st);
         if (ok()) e = cudaStreamWaitEvent(down, ev(4), 0);
-        if (ok() && io->dQ_host && !by_group) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * 4, cudaMemcpyDeviceToHost, down);
-        if (ok() && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * 4, cudaMemcpyDeviceToHost, down);
-        if (ok() && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * 4, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dQ_host && !by_group) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * ob, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * ob, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * ob, cudaMemcpyDeviceToHost, down);
     }
     if (ok()) e = cudaEventRecord(ev(5), down);
     if (ok()) e = cudaStreamWaitEvent(st, ev(5), 0);

@@ -90,7 +90,7 @@ extern "C" int mesh_attn_forward_static_limits(const mesh_attn_plan* p, int64_t*
     return MESH_ATTN_OK;
 }
 
-extern "C" int mesh_attn_forward_static(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, float* O, float* lse, void* stream)
+extern "C" int mesh_attn_forward_static(const mesh_attn_plan* p, const void* Q, const void* K, const void* V, void* O, float* lse, void* stream)
 {
     int dev = -1;
     if (int rc = current_device_of(p, "forward_static", &dev)) return rc;

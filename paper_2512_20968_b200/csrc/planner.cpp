@@ -374,6 +374,7 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
         if (v != 0 && v != 1) return fail(MESH_ATTN_EINVAL, "plan_create: flag fields must be 0 or 1");
     if (d->bwd_piece_blocks < 0) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_piece_blocks must be >= 0 (0 = default)");
     if (d->bwd_pairing < 0 || d->bwd_pairing > 2) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_pairing must be 0 (auto), 1 (never) or 2 (shared tile loads only)");
+    if (d->out_dtype < 0 || d->out_dtype > 1) return fail(MESH_ATTN_EINVAL, "plan_create: out_dtype must be 0 (fp32) or 1 (bf16)");
     for (int v : d->reserved) if (v != 0) return fail(MESH_ATTN_EINVAL, "plan_create: reserved fields must be 0");
     const int k_q = d->k_q <= 0 ? 1 : d->k_q, k_kv = d->k_kv <= 0 ? 1 : d->k_kv;
     if (k_q * k_kv > 16) return fail(MESH_ATTN_EINVAL, "plan_create: k_q*k_kv must be <= 16 (PAPER.md L206)");
@@ -618,7 +619,11 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             *value = (int64_t)((2.0L - 2.0L / gm.n) * Nd);
             break;
         }
-        case MESH_ATTN_Q_BWD_WS_BYTES: *value = 2ll * gm.batch * Hq * (int64_t)gm.n * gm.L * 4; break;
+        case MESH_ATTN_Q_BWD_WS_BYTES:
+            *value = 2ll * gm.batch * Hq * (int64_t)gm.n * gm.L * 4;
+            if (p->desc.out_dtype == 1)         // + the fp32 accumulators of dQ, dK, dV
+                *value += (int64_t)gm.batch * gm.n * gm.L * ((int64_t)p->desc.heads_q + 2ll * p->desc.heads_kv) * gm.head_dim * 4;
+            break;
         case MESH_ATTN_Q_USP_LANES: *value = U; break;
         case MESH_ATTN_Q_GOO_PARTIAL_O_BYTES: *value = (int64_t)gm.a * p->k_kv * unit * gm.head_dim * 4; break;
         case MESH_ATTN_Q_GOO_PARTIAL_LSE_BYTES: *value = (int64_t)gm.a * p->k_kv * unit * 4; break;

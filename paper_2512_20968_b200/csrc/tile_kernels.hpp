@@ -72,7 +72,8 @@ struct MergeParams {
     int peers;
     const float* peer_O[kMaxPeers];
     const float* peer_lse[kMaxPeers];
-    float* O;
+    void* O;                   // fp32, or bf16 when out_bf16 (plan out_dtype = 1)
+    int out_bf16;
     float* lse;
     long long lse_stride_b;    // batch stride of lse [B][Hq][N] (all heads * N)
     long long o_stride_b, o_stride_row, o_stride_h;   // element strides of O
@@ -87,7 +88,8 @@ struct SumParams {               // out[i] = sum_k src[k][i]: the reduce-scatter
 
 struct DeltaParams {
     Geom gm;
-    const float* O;
+    const void* O;             // fp32, or bf16 when o_bf16 (plan out_dtype = 1)
+    int o_bf16;
     const void* dO;            // bf16
     const float* lse;          // [B][Hq][N] final merged LSE (natural log)
     float* ws;                 // [2][B][Hq][N]: delta, log2(scale) - lse*log2e
@@ -102,5 +104,6 @@ int launch_tile_bwd(const BwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
 int launch_merge(const MergeParams& p, cudaStream_t stream);
 int launch_delta(const DeltaParams& p, cudaStream_t stream);
 int launch_sum_peers(const SumParams& p, int num_sms, cudaStream_t stream);
+int launch_cast_bf16(const float* src, void* dst, long long count, int num_sms, cudaStream_t stream);   // dst (bf16)[i] = src[i], count % 4 == 0
 
 }  // namespace mesh_attn

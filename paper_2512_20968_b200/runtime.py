@@ -4,7 +4,7 @@ from __future__ import annotations
 
 import torch
 
-from .binding import Plan, Q_PARTIAL_LSE_BYTES, Q_PARTIAL_O_BYTES
+from .binding import Plan, Q_BWD_WS_BYTES, Q_PARTIAL_LSE_BYTES, Q_PARTIAL_O_BYTES
 from .workloads import Workload
 
 
@@ -28,11 +28,13 @@ class Buffers:
         f32 = dict(dtype=torch.float32, device=device)
         self.partial_O = torch.empty(plan.query(Q_PARTIAL_O_BYTES) * g_count // 4, **f32)
         self.partial_lse = torch.empty(plan.query(Q_PARTIAL_LSE_BYTES) * g_count // 4, **f32)
-        self.O = torch.empty((B, N, Hq, D), **f32)
+        out = dict(dtype=torch.bfloat16 if plan.desc.out_dtype == 1 else torch.float32, device=device)   # plan desc field out_dtype
+        self.O = torch.empty((B, N, Hq, D), **out)
         self.lse = torch.empty((B, Hq, N), **f32)
         if backward:
-            self.bwd_ws = torch.empty((2, B, Hq, N), **f32)      # [0] = delta, [1] = log2(scale) - lse*log2(e)  (Q_BWD_WS_BYTES)
-            self.delta = self.bwd_ws[0]
-            self.dQ = torch.empty((B, N, Hq, D), **f32)
-            self.dK = torch.empty((B, N, Hkv, D), **f32)
-            self.dV = torch.empty((B, N, Hkv, D), **f32)
+            # [0] = delta, [1] = log2(scale) - lse*log2(e); out_dtype 1: the fp32 accumulators of dQ, dK, dV follow (Q_BWD_WS_BYTES)
+            self.bwd_ws = torch.empty(plan.query(Q_BWD_WS_BYTES) // 4, **f32)
+            self.delta = self.bwd_ws[:B * Hq * N].view(B, Hq, N)
+            self.dQ = torch.empty((B, N, Hq, D), **out)
+            self.dK = torch.empty((B, N, Hkv, D), **out)
+            self.dV = torch.empty((B, N, Hkv, D), **out)

@@ -292,3 +292,19 @@ def test_goo_executor_volumes():
         assert p.query(B.Q_GOO_COMM_BYTES) == 4 * p.query(B.Q_MESH_COMM_BYTES_FWD)
         assert p.query(B.Q_GOO_PARTIAL_O_BYTES) == k_kv * p.query(B.Q_PARTIAL_O_BYTES)
         assert p.query(B.Q_GOO_PARTIAL_LSE_BYTES) == k_kv * p.query(B.Q_PARTIAL_LSE_BYTES)
+
+
+def test_out_dtype_field_is_validated_and_sizes_the_backward_workspace():
+    """plan desc field out_dtype (include/mesh_attn.h): 0 fp32, 1 bf16 outputs; with 1 the backward workspace also holds the fp32
+    accumulators of dQ, dK, dV (host-only plans answer the query too)."""
+    kw = dict(a=2, b=2, n=4, batch=2, seq_total=2048, heads_q=8, heads_kv=2, head_dim=128, causal=1, seq_layout=1)
+    p0, p1 = Plan(**kw), Plan(out_dtype=1, **kw)
+    planes = 2 * 2 * 8 * 2048 * 4
+    assert p0.query(B.Q_BWD_WS_BYTES) == planes
+    assert p1.query(B.Q_BWD_WS_BYTES) == planes + 2 * 2048 * (8 + 2 * 2) * 128 * 4
+    for what in (B.Q_PARTIAL_O_BYTES, B.Q_PARTIAL_LSE_BYTES, B.Q_FLOPS_FWD, B.Q_FLOPS_BWD, B.Q_BWD_ITEMS_PER_GPU):
+        assert p0.query(what) == p1.query(what)
+    for bad in (-1, 2):
+        with pytest.raises(MeshAttnError) as e:
+            Plan(out_dtype=bad, **kw)
+        assert e.value.status == B.EINVAL
