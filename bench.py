@@ -84,6 +84,8 @@ def parse_args():
     ap.add_argument("--goo-executor", type=int, default=-1, metavar="R",
                     help="separate mode (not the driver's bench line): time the GOO executor (mesh_attn_forward_goo) on --workload with every "
                          "communication stand-in copied R times, overlapped vs serialised, against the fused forward")
+    ap.add_argument("--fwd-pairing", type=int, default=0, choices=[0, 1],
+                    help="plan desc field fwd_pairing (A/B runs): 0 auto (tile_fwd as CTA pairs with cta_group::2 MMAs where the plan allows), 1 single CTAs")
     ap.add_argument("--bwd-pairing", type=int, default=0, choices=[0, 1, 2],
                     help="plan desc field bwd_pairing (A/B runs): 0 auto (2-CTA clusters + dQ exchange), 1 single CTAs, 2 clusters without the exchange")
     ap.add_argument("--bwd-piece-blocks", type=int, default=0, help="plan desc field bwd_piece_blocks (A/B runs): Q blocks per tile_bwd work item, 0 = default")
@@ -429,7 +431,7 @@ def run_ours(args):
     w = W.CONFIGS[args.workload]
     peaks, peak_src = load_peaks()
     inp = W.make_inputs(w, "cuda", ("q", "k", "v", "do") if w.backward else ("q", "k", "v"))
-    plan = plan_for(w, usp_lanes=args.usp_lanes, bwd_pairing=args.bwd_pairing, bwd_piece_blocks=args.bwd_piece_blocks)
+    plan = plan_for(w, usp_lanes=args.usp_lanes, bwd_pairing=args.bwd_pairing, bwd_piece_blocks=args.bwd_piece_blocks, fwd_pairing=args.fwd_pairing)
     buf = Buffers(plan, w, backward=w.backward)
 
     def step():
@@ -537,6 +539,7 @@ def run_ours(args):
     }
     if args.usp_lanes > 1:
         line["config"]["usp_lanes"] = args.usp_lanes
+    line["config"]["tile_fwd_kernel"] = {0: "single CTAs", 1: "2-CTA clusters, tcgen05 cta_group::2 MMAs (K / V halves per CTA)"}[plan.query(B.Q_FWD_PAIRED)]
     line["config"]["tile_bwd_kernel"] = {0: "single CTAs", 1: "2-CTA clusters, shared Q/dO tile loads", 2: "2-CTA clusters, shared tile loads + dQ exchange"}[plan.query(B.Q_BWD_PAIRED)]
     print(json.dumps(line), flush=True)
     if dist is not None:

@@ -109,7 +109,11 @@ typedef struct {
                                  delta = rowsum(dO o O) carries up to 2^-9 sum|dO O| of rounding, which reaches dQ, dK (measured
                                  1.6e-2 max against the fp32 path on a causal case; dV is unaffected).  An option beyond the paper's
                                  (unpinned: tests compare against the fp32 path and the oracle at that resolution).              */
-    int32_t reserved[1];      /* must be 0                                                             */
+    int32_t fwd_pairing;      /* tile_fwd as 2-CTA clusters over work items 2k, 2k+1 with tcgen05 cta_group::2 MMAs (each CTA holds half of
+                                 every K / V block: half the shared-memory operand traffic per SM; MESH_ATTN_Q_FWD_PAIRED): 0 auto
+                                 (paired when the planner finds that the two items stream the same K / V blocks on every simulated GPU
+                                 -- non-causal and striped-causal plans with an even item count -- and head_dim = 128, precision = 0),
+                                 1 never (single-CTA kernel; for A/B measurements).  Results are bit-identical either way.            */
 } mesh_attn_plan_desc;
 
 /* what = ... for mesh_attn_plan_query */
@@ -142,6 +146,7 @@ enum {
     MESH_ATTN_Q_GOO_COMM_BYTES = 21,       /* bytes the forward step list's collectives move for the a GPUs of one Q group:
                                               k_q (AG-Q + RS-Q) of (a-1) Q chunks + k_kv AG-KV of (b-1) K and V chunks, each x a
                                               (= a x MESH_ATTN_Q_MESH_COMM_BYTES_FWD, the per-GPU volume of P:L290-292) */
+    MESH_ATTN_Q_FWD_PAIRED = 22,           /* 1 if tile_fwd runs as 2-CTA clusters with cta_group::2 MMAs (desc.fwd_pairing) */
     MESH_ATTN_Q_USP_A2A_BYTES_FWD = 17     /* per-GPU forward volume of the Ulysses all-to-alls around the lanes (Q, K, V in,
                                               O out): (U-1)/U of the GPU's N/(n*U) tokens x (2 Hq + 2 Hkv) head_dim x 2 bytes;
                                               with n = 1 and Hq = Hkv this is Table 1's Ulysses entry 4(U-1)/U^2 N d */

@@ -24,7 +24,7 @@ lib = C.CDLL(str(_LIB_PATH))
 OK, EINVAL, EUNSUPPORTED, EWORKSPACE, ECUDA, ENOMEM = 0, -1, -2, -3, -4, -5
 (Q_PARTIAL_O_BYTES, Q_PARTIAL_LSE_BYTES, Q_SLOTS_PER_GPU, Q_FLOPS_FWD, Q_FLOPS_BWD, Q_WAVES, Q_MERGE_BYTES,
  Q_FWD_ITEMS_PER_GPU, Q_BWD_ITEMS_PER_GPU, Q_BLOCKS_FWD, Q_COMM_UNITS, Q_HAS_DEVICE, Q_BWD_WS_BYTES,
- Q_MESH_COMM_BYTES_FWD, Q_MESH_COMM_BYTES_BWD, Q_RING_COMM_BYTES_FWD, Q_USP_LANES, Q_USP_A2A_BYTES_FWD, Q_BWD_PAIRED, Q_GOO_PARTIAL_O_BYTES, Q_GOO_PARTIAL_LSE_BYTES, Q_GOO_COMM_BYTES) = range(22)
+ Q_MESH_COMM_BYTES_FWD, Q_MESH_COMM_BYTES_BWD, Q_RING_COMM_BYTES_FWD, Q_USP_LANES, Q_USP_A2A_BYTES_FWD, Q_BWD_PAIRED, Q_GOO_PARTIAL_O_BYTES, Q_GOO_PARTIAL_LSE_BYTES, Q_GOO_COMM_BYTES, Q_FWD_PAIRED) = range(23)
 TASK_AG_KV, TASK_AG_Q, TASK_RS_Q, TASK_C, TASK_RS_KV = range(5)
 
 
@@ -37,7 +37,7 @@ class PlanDesc(C.Structure):
         ("gamma", C.c_float), ("t_ag_q", C.c_float), ("t_ag_kv", C.c_float), ("t_rs_q", C.c_float), ("t_c", C.c_float),
         ("softmax_scale", C.c_float),
         ("tensor_layout", C.c_int32), ("partial_mode", C.c_int32), ("precision", C.c_int32),
-        ("usp_lanes", C.c_int32), ("bwd_pairing", C.c_int32), ("bwd_piece_blocks", C.c_int32), ("out_dtype", C.c_int32), ("reserved", C.c_int32 * 1),
+        ("usp_lanes", C.c_int32), ("bwd_pairing", C.c_int32), ("bwd_piece_blocks", C.c_int32), ("out_dtype", C.c_int32), ("fwd_pairing", C.c_int32),
     ]
 
 

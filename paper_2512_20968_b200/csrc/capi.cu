@@ -209,7 +209,7 @@ extern "C" {
 // tile_fwd over an item list (the plan's fused list, or one compute task of the GOO executor)
 static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int items_per_gpu, int slots_per_gpu, int32_t g_first, int32_t g_count,
                            const void* Q, const void* K, const void* V, float* partial_O, float* partial_lse, void* stream, const char* who,
-                           bool local = false)
+                           bool local = false, bool pair = false)
 {
     const long long rq = local ? (long long)p->geom.a * p->geom.L : 0, rk = local ? (long long)p->geom.b * p->geom.L : 0;
     if (int rc = check_device(p, who)) return rc;
@@ -220,7 +220,7 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
     if (items_per_gpu == 0) return MESH_ATTN_OK;
     CUtensorMap tmQ, tmK, tmV;
     if (!make_map(p, &tmQ, Q, p->geom.heads_q, p->desc.heads_q, ln.hq0, kBlock, rq) ||
-        !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, rk) ||
+        !make_map(p, &tmK, K, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, pair ? kBlock / 2 : kBlock, rk) ||   // pair: each CTA loads 64 key rows
         !make_map(p, &tmV, V, p->geom.heads_kv, p->desc.heads_kv, ln.hk0, kBlock, rk))
         return fail(MESH_ATTN_ECUDA, std::string(who) + ": cuTensorMapEncodeTiled failed (pointers must be 16-byte aligned device memory)");
     FwdParams fp;
@@ -234,6 +234,7 @@ static int launch_fwd_list(const mesh_attn_plan* p, const FwdItem* items, int it
     fp.g_first = g_first % p->geom.n;
     fp.g_count = g_count;
     fp.split = p->desc.precision;
+    fp.pair = pair ? 1 : 0;
     fp.partial_O = partial_O;
     fp.partial_lse = partial_lse;
     fp.status = p->d_status;
@@ -292,7 +293,7 @@ int mesh_attn_tile_fwd(const mesh_attn_plan* p, int32_t g_first, int32_t g_count
 {
     if (int rc = check_device(p, "tile_fwd")) return rc;
     return launch_fwd_list(p, p->d_fwd_items, (int)p->fwd_items.size(), p->geom.slots_per_gpu, g_first, g_count, Q, K, V, partial_O, partial_lse, stream,
-                           "tile_fwd");
+                           "tile_fwd", false, p->fwd_pair());
 }
 
 int mesh_attn_merge(const mesh_attn_plan* p, int32_t q_group, const float* partial_O, const float* partial_lse, void* O, float* lse,

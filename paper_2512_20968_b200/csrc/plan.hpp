@@ -120,6 +120,10 @@ struct mesh_attn_plan {
     // KV partition, each walking Q chunk i of every Q partition (their seg lists are appended to bwd_segs / bwd_seglists)
     std::vector<mesh_attn::BwdItem> goo_bwd_items;
     std::vector<mesh_attn::SegList> goo_bwd_task;
+    // forward items 2k, 2k+1 stream the same K / V blocks on every simulated GPU (planner.cpp): tile_fwd then runs as CTA pairs
+    // with tcgen05 cta_group::2 MMAs (head_dim 128, single-operand mode); desc.fwd_pairing = 1 forces the single-CTA kernel
+    bool fwd_pairable = false;
+    bool fwd_pair() const { return fwd_pairable && desc.fwd_pairing != 1 && desc.precision == 0 && geom.head_dim == 128; }
     // backward items 2k and 2k+1 visit the same Q blocks on every simulated GPU (tile_bwd then runs 2-CTA clusters that
     // share the Q / dO tile loads); desc.bwd_pairing selects never / shared loads only / shared loads + dQ exchange
     bool bwd_pairable = false;

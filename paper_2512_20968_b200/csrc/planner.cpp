@@ -332,6 +332,34 @@ bool bwd_items_pairable(const mesh_attn_plan* p)
     return true;
 }
 
+// Do forward items 2k and 2k+1 stream the same K / V blocks (same batch, KV head, partitions and key rows) on every simulated GPU?
+// (tile_fwd.cu kv_range, restated: the visible key rows of a segment are clipped at the item's last query row.)
+bool fwd_items_pairable(const mesh_attn_plan* p)
+{
+    const Geom& gm = p->geom;
+    const size_t cnt = p->fwd_items.size();
+    if (cnt < 2 || cnt % 2) return false;
+    for (size_t k = 0; k < cnt; k += 2) {
+        const FwdItem &x = p->fwd_items[k], &y = p->fwd_items[k + 1];
+        if (x.batch != y.batch || x.head / gm.group != y.head / gm.group || x.seglist != y.seglist || x.nrows != y.nrows) return false;
+        if (!gm.causal) continue;
+        const SegList sl = p->fwd_seglists[x.seglist];
+        for (int g = 0; g < gm.n; ++g) {
+            const int ux = (g / gm.a) * gm.a + x.u_local, uy = (g / gm.a) * gm.a + y.u_local;
+            for (int i = 0; i < sl.count; ++i) {
+                const Seg& sg = p->fwd_segs[sl.offset + i];
+                const int v = kv_partition(gm, g, sg.part_local);
+                auto t_hi = [&](const FwdItem& it, int u) {
+                    const int lim = it.q0 + it.nrows - 1 + causal_off(gm, u, v);
+                    return lim < sg.begin ? sg.begin : std::min<int>(sg.end, (lim / kBlock + 1) * kBlock);
+                };
+                if (t_hi(x, ux) != t_hi(y, uy)) return false;
+            }
+        }
+    }
+    return true;
+}
+
 // number of 128x128 score blocks the forward computes for one simulated GPU g and one head
 int64_t fwd_blocks_of_gpu(const mesh_attn_plan* p, int g)
 {
@@ -375,7 +403,7 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     if (d->bwd_piece_blocks < 0) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_piece_blocks must be >= 0 (0 = default)");
     if (d->bwd_pairing < 0 || d->bwd_pairing > 2) return fail(MESH_ATTN_EINVAL, "plan_create: bwd_pairing must be 0 (auto), 1 (never) or 2 (shared tile loads only)");
     if (d->out_dtype < 0 || d->out_dtype > 1) return fail(MESH_ATTN_EINVAL, "plan_create: out_dtype must be 0 (fp32) or 1 (bf16)");
-    for (int v : d->reserved) if (v != 0) return fail(MESH_ATTN_EINVAL, "plan_create: reserved fields must be 0");
+    if (d->fwd_pairing < 0 || d->fwd_pairing > 1) return fail(MESH_ATTN_EINVAL, "plan_create: fwd_pairing must be 0 (auto) or 1 (never)");
     const int k_q = d->k_q <= 0 ? 1 : d->k_q, k_kv = d->k_kv <= 0 ? 1 : d->k_kv;
     if (k_q * k_kv > 16) return fail(MESH_ATTN_EINVAL, "plan_create: k_q*k_kv must be <= 16 (PAPER.md L206)");
     if (L % k_q || (L / k_q) % kBlock || L % k_kv || (L / k_kv) % kBlock)
@@ -432,6 +460,7 @@ extern "C" int mesh_attn_plan_create(const mesh_attn_plan_desc* d, mesh_attn_pla
     }
     build_worklists(p);
     p->bwd_pairable = bwd_items_pairable(p);
+    p->fwd_pairable = fwd_items_pairable(p);
     if (p->fwd_seglists.size() > 32767 || p->bwd_seglists.size() > 32767) {     // FwdItem / BwdItem::seglist are 16 bits
         delete p;
         return fail(MESH_ATTN_EINVAL, "plan_create: too many segment lists (k_q, k_kv, b too large for partial_mode 1)");
@@ -635,6 +664,7 @@ extern "C" int mesh_attn_plan_query(const mesh_attn_plan* p, int32_t what, int64
             break;
         }
         case MESH_ATTN_Q_BWD_PAIRED: *value = p->bwd_pair_mode(); break;
+        case MESH_ATTN_Q_FWD_PAIRED: *value = p->fwd_pair() ? 1 : 0; break;
         case MESH_ATTN_Q_USP_A2A_BYTES_FWD: {
             // the GPU holds N/(n U) tokens of all heads before the all-to-all and keeps 1/U of them
             const long double tokens = (long double)gm.batch * gm.n * gm.L / ((long double)gm.n * U);

@@ -223,6 +223,12 @@ __device__ __forceinline__ void mbar_arrive_remote(uint32_t remote_bar)
 {
     asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(remote_bar) : "memory");
 }
+// the same with release semantics at cluster scope: what this thread (and the threads it synchronised with) wrote is visible to
+// the peer's thread that acquires the barrier at cluster scope
+__device__ __forceinline__ void mbar_arrive_remote_release(uint32_t remote_bar)
+{
+    asm volatile("mbarrier.arrive.release.cluster.shared::cluster.b64 _, [%0];" ::"r"(remote_bar) : "memory");
+}
 // wait that acquires at cluster scope: the data the peer's st.async delivered is visible afterwards
 __device__ __forceinline__ bool mbar_try_wait_cluster(uint64_t* bar, uint32_t parity)
 {
@@ -254,6 +260,52 @@ __device__ __forceinline__ void tma_load_4d_mc(void* smem_dst, const CUtensorMap
         " [%0], [%1, {%4, %5, %6, %7}], [%2], %3, %8;"
         ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(bar)), "h"(cta_mask), "r"(c0), "r"(c1), "r"(c2), "r"(c3),
           "l"(policy)
+        : "memory");
+}
+
+// ---------------------------------------------------------------------------------- CTA pairs (tcgen05 cta_group::2)
+// Two CTAs of a cluster (ranks 0 and 1, the same TPC) run ONE MMA of M = 256: each CTA supplies 128 rows of A (its own shared
+// memory or tensor memory, at the same offsets) and HALF of B (N / 2 rows of a K-major B, N / 2 columns of an MN-major B), and
+// receives its 128 rows of D in its own tensor memory.  Only rank 0 issues; the tensor core of each SM reads half as many B
+// bytes from shared memory.  Every tcgen05 alloc / mma / commit of such a kernel carries cta_group::2.
+template <uint32_t kCols> __device__ __forceinline__ void tmem_alloc_2cta(uint32_t* smem_slot)   // one warp of EACH CTA, same warp index
+{
+    asm volatile("tcgen05.alloc.cta_group::2.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(smem_slot)), "n"(kCols) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::2.sync.aligned;" ::: "memory");
+}
+template <uint32_t kCols> __device__ __forceinline__ void tmem_dealloc_2cta(uint32_t addr)
+{
+    asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;" ::"r"(addr), "n"(kCols) : "memory");
+}
+__device__ __forceinline__ void umma_ss_2cta(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::2.kind::f16 [%0], %1, %2, %3, p;\n}"
+        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+__device__ __forceinline__ void umma_ts_2cta(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accumulate)
+{
+    asm volatile(
+        "{\n.reg .pred p;\nsetp.ne.b32 p, %4, 0;\ntcgen05.mma.cta_group::2.kind::f16 [%0], [%1], %2, %3, p;\n}"
+        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accumulate)
+        : "memory");
+}
+// arrives (once the pair's MMAs issued so far have completed) on the barrier at this CTA-relative address in both CTAs
+__device__ __forceinline__ void umma_commit_2cta(uint64_t* bar)
+{
+    asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;"
+                 ::"r"(smem_u32(bar)), "h"((uint16_t)3) : "memory");
+}
+// 4-D tiled load into THIS CTA's shared memory whose bytes complete on the barrier at `bar_cluster_addr` (a shared::cluster
+// address: rank 0's copy of the barrier, mapa(smem_u32(bar), 0)), so that the issuing CTA of the pair sees both halves land
+__device__ __forceinline__ void tma_load_4d_2cta(void* smem_dst, const CUtensorMap* m, uint32_t bar_cluster_addr, int c0, int c1, int c2,
+                                                 int c3, uint64_t policy)
+{
+    asm volatile(
+        "cp.async.bulk.tensor.4d.cta_group::2.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+        " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;"
+        ::"r"(smem_u32(smem_dst)), "l"(reinterpret_cast<uint64_t>(m)), "r"(bar_cluster_addr), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
         : "memory");
 }
 

@@ -27,6 +27,8 @@
 // kSplit (plan precision = 1): P as hi + lo bf16, two PV MMAs.
 #include <cuda_bf16.h>
 
+#include <atomic>
+
 #include "plan.hpp"
 #include "sm100.cuh"
 #include "tile_kernels.hpp"
@@ -61,13 +63,21 @@ template <int N> struct IntTag { static constexpr int value = N; };
 template <int kRegs> __device__ __forceinline__ void reg_alloc() { asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 template <int kRegs> __device__ __forceinline__ void reg_dealloc() { asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(kRegs)); }
 
-template <int D> struct FwdCfg {
+// kPair: the kernel runs as clusters of two CTAs that take work items 2k and 2k+1, which the planner has checked to stream the
+// SAME K / V blocks (FwdParams::pair), and every MMA is a tcgen05 cta_group::2 MMA of M = 256 issued by rank 0: 128 query rows
+// of each CTA against one K / V block of which each CTA's shared memory holds HALF -- K rows 64r..64r+63 (B of S = Q K^T is
+// K-major, split along N = keys), V columns 64r..64r+63 (B of O += P V is MN-major, split along N = head_dim).  Per block a
+// CTA's tensor core then reads 128 KB of operands instead of 192 KB and the TMA writes 32 KB instead of 64 KB: shared-memory
+// bandwidth (128 B/clk), which bounds the single-CTA kernel (profiles/r02_v4_README.md), is no longer the limit.
+template <int D, bool kPair> struct FwdCfg {
+    static_assert(!kPair || D == 128, "the CTA-pair kernel is built for head_dim 128");
     static constexpr int kBoxes = D / 64;                  // 64-element (128-byte) TMA boxes per row
     static constexpr int kTileBytes = kBlock * D * 2;      // one [128 x D] bf16 tile
-    static constexpr int kStages = D == 128 ? 5 : 8;       // K/V ring slots (each one tile)
+    static constexpr int kSlotBytes = kPair ? kTileBytes / 2 : kTileBytes;   // a ring slot: a K or V tile, or this CTA's half of one
+    static constexpr int kStages = (D == 128 ? 5 : 8) * (kPair ? 2 : 1);     // K/V ring slots
     static constexpr int kSmemQ = 2 * kTileBytes;
-    static constexpr int kSmemRing = kStages * kTileBytes;
-    static constexpr int kNumBars = 2 + 2 * kStages + 8 + 2 * kSchedSlots;
+    static constexpr int kSmemRing = kStages * kSlotBytes;
+    static constexpr int kNumBars = 2 + 2 * kStages + 8 + 3 * kSchedSlots;
     static constexpr int kSmemBytes = kSmemQ + kSmemRing + kNumBars * 8 + 16 + 16 + 1024 + kWatchdogBytes;   // + TMEM slot, item ring, alignment slack, watchdog state (last 16 bytes)
     static constexpr uint32_t kColS = 0, kColO = 256;      // TMEM columns
 };
@@ -129,12 +139,13 @@ __device__ __forceinline__ ItemCtx load_item(const FwdParams& p, int idx)
     return c;
 }
 
-template <int D, bool kSplit>
+template <int D, bool kSplit, bool kPair>
 __global__ void __launch_bounds__(kThreads, 1)
 tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__ CUtensorMap tmK,
-                const __grid_constant__ CUtensorMap tmV, const FwdParams p)
+                const __grid_constant__ CUtensorMap tmV, const FwdParams p)      // kPair: tmK has 64-row boxes
 {
-    using Cfg = FwdCfg<D>;
+    static_assert(!(kPair && kSplit), "the CTA-pair kernel is built for the single-operand mode");
+    using Cfg = FwdCfg<D, kPair>;
     extern __shared__ uint8_t smem_raw[];
     uint8_t* smem = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
     uint8_t* sQ = smem;
@@ -149,12 +160,15 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     uint64_t* o_full = p_half + 4;                // [2]
     uint64_t* sched_full = o_full + 2;            // [kSchedSlots] the scheduler warp has put the next work-item index into slot k
     uint64_t* sched_empty = sched_full + kSchedSlots;   // [kSchedSlots] every role has read slot k
-    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(sched_empty + kSchedSlots);
+    uint64_t* peer_free = sched_empty + kSchedSlots;    // [kSchedSlots] kPair, rank 0: the peer's slot k is armed for the next index
+    uint32_t* tmem_slot = reinterpret_cast<uint32_t*>(peer_free + kSchedSlots);
     volatile int* sched_idx = reinterpret_cast<volatile int*>(tmem_slot + 4);
 
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const Geom& gm = p.gm;
     const int total_items = p.items_per_gpu * p.g_count;
+    const uint32_t pair_rank = kPair ? cluster_ctarank() : 0;
+    const bool leader = pair_rank == 0;                 // issues the pair's MMAs, owns the barriers the operands land on
 
     if (warp == kLoaderWarp && lane == 0) {
         prefetch_tmap(&tmQ); prefetch_tmap(&tmK); prefetch_tmap(&tmV);
@@ -163,13 +177,22 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         mbar_init(q_empty, 1);
         for (int s = 0; s < Cfg::kStages; ++s) { mbar_init(&kv_full[s], 1); mbar_init(&kv_empty[s], 1); }
         for (int t = 0; t < 2; ++t) { mbar_init(&s_full[t], 1); mbar_init(&o_full[t], 1); }
-        for (int t = 0; t < 4; ++t) mbar_init(&p_half[t], kBlock);
-        for (int k = 0; k < kSchedSlots; ++k) { mbar_init(&sched_full[k], 1); mbar_init(&sched_empty[k], 2 + 2 * kBlock); }   // readers: loader, MMA issuer, softmax groups
+        for (int t = 0; t < 4; ++t) mbar_init(&p_half[t], kPair ? kBlock + kBlock / 32 : kBlock);   // + one arrival per softmax warp of the peer
+        for (int k = 0; k < kSchedSlots; ++k) {
+            mbar_init(&sched_full[k], 1);
+            // readers: loader, MMA issuer (rank 0), softmax groups; the peer's scheduler thread follows its ring too
+            mbar_init(&sched_empty[k], 1 + (leader ? 1 : 0) + 2 * kBlock + ((kPair && !leader) ? 1 : 0));
+            mbar_init(&peer_free[k], 1);
+        }
         fence_mbar_init();
     }
-    if (warp == kAllocWarp) tmem_alloc<512>(tmem_slot);
+    if (warp == kAllocWarp) {
+        if constexpr (kPair) tmem_alloc_2cta<512>(tmem_slot);
+        else tmem_alloc<512>(tmem_slot);
+    }
     tc_fence_before();
     __syncthreads();
+    if constexpr (kPair) cluster_sync();                // the peer's barriers are initialised before anything is sent to them
     tc_fence_after();
     const uint32_t tmem = *tmem_slot;
 
@@ -178,7 +201,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     // apart by hundreds of items and the K / V blocks they stream stop being shared in L2 (see tile_bwd.cu).
     uint32_t sc_slot = 0, sc_phase = 0;
     auto next_item = [&]() -> int {
-        mbar_wait(&sched_full[sc_slot], sc_phase);
+        if constexpr (kPair) mbar_wait_cluster(&sched_full[sc_slot], sc_phase);   // rank 1's index arrives from the peer (st.async)
+        else mbar_wait(&sched_full[sc_slot], sc_phase);
         const int v = sched_idx[sc_slot];
         mbar_arrive(&sched_empty[sc_slot]);
         if (++sc_slot == kSchedSlots) { sc_slot = 0; sc_phase ^= 1; }
@@ -189,20 +213,44 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
     if (warp == kSchedWarp) {
         // =============================== work-item scheduler ===============================
         if (elect_one()) {
-            uint32_t slot = 0, phase = 0;
-            while (true) {
-                mbar_wait(&sched_empty[slot], phase ^ 1);        // the slot's previous index has been read by every role
-                const int v = atomicAdd(p.counter, 1);
-                sched_idx[slot] = v;
-                mbar_arrive(&sched_full[slot]);
-                if (v >= total_items) break;
-                if (++slot == kSchedSlots) { slot = 0; phase ^= 1; }
+            if (leader) {
+                const uint32_t peer_idx = kPair ? mapa(smem_u32(const_cast<int*>(sched_idx)), 1u) : 0u;
+                const uint32_t peer_full = kPair ? mapa(smem_u32(sched_full), 1u) : 0u;
+                uint32_t slot = 0, phase = 0;
+                while (true) {
+                    mbar_wait(&sched_empty[slot], phase ^ 1);                    // the slot's previous index has been read by every role
+                    if constexpr (kPair) mbar_wait(&peer_free[slot], phase);     // ... and the peer's slot is armed
+                    const int v = atomicAdd(p.counter, kPair ? 2 : 1);
+                    sched_idx[slot] = v;
+                    mbar_arrive(&sched_full[slot]);
+                    if constexpr (kPair)                                         // the peer takes the odd item of the pair
+                        asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.b32 [%0], %1, [%2];"
+                                     ::"r"(peer_idx + slot * 4), "r"(v + 1), "r"(peer_full + slot * 8) : "memory");
+                    if (v >= total_items) break;
+                    if (++slot == kSchedSlots) { slot = 0; phase ^= 1; }
+                }
+            } else {
+                // rank 1: arm a slot (expect the 4 bytes of the index), tell rank 0, and follow the ring like every other role
+                const uint32_t r0_free = mapa(smem_u32(peer_free), 0u);
+                for (int k = 0; k < kSchedSlots; ++k) { mbar_expect_tx(&sched_full[k], 4); mbar_arrive_remote(r0_free + k * 8); }
+                uint32_t slot = 0, phase = 0;
+                while (true) {
+                    const int v = next_item();
+                    if (v >= total_items) break;
+                    mbar_wait(&sched_empty[slot], phase);                        // every role has read it: arm the slot again
+                    mbar_expect_tx(&sched_full[slot], 4);
+                    mbar_arrive_remote(r0_free + slot * 8);
+                    if (++slot == kSchedSlots) { slot = 0; phase ^= 1; }
+                }
             }
         }
     } else if (warp == kLoaderWarp) {
         // =============================== TMA producer ===============================
         if (elect_one()) {
             uint32_t stage = 0, ring_phase = 0, q_phase = 0;
+            // kPair: every load lands in this CTA's shared memory and completes its bytes on RANK 0's barrier (the MMA issuer waits
+            // there for both CTAs' operands); rank 0 alone arms the barrier, with the bytes of both CTAs
+            const uint32_t q_full_r0 = kPair ? mapa(smem_u32(q_full), 0u) : 0u, kv_full_r0 = kPair ? mapa(smem_u32(kv_full), 0u) : 0u;
             for (int idx = next_item(); idx < total_items; idx = next_item()) {
                 const ItemCtx c = load_item(p, idx);
                 bool first = true;
@@ -211,29 +259,49 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         first = false;
                         mbar_wait(q_empty, q_phase ^ 1);
                         q_phase ^= 1;
-                        mbar_expect_tx(q_full, c.nt * Cfg::kTileBytes);
+                        if (leader) mbar_expect_tx(q_full, (kPair ? 2 : 1) * c.nt * Cfg::kTileBytes);
                         for (int t = 0; t < c.nt; ++t)
-                            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
-                                tma_load_4d(sQ + t * Cfg::kTileBytes + bx * (kBlock * 128), &tmQ, q_full, bx * 64, c.it.head,
-                                            q_row_part(gm, c.u, c.it.u_local) * gm.L + c.it.q0 + t * kBlock, c.it.batch, kEvictFirst);
+                            for (int bx = 0; bx < Cfg::kBoxes; ++bx) {
+                                const int row = q_row_part(gm, c.u, c.it.u_local) * gm.L + c.it.q0 + t * kBlock;
+                                if constexpr (kPair)
+                                    tma_load_4d_2cta(sQ + t * Cfg::kTileBytes + bx * (kBlock * 128), &tmQ, q_full_r0, bx * 64, c.it.head, row, c.it.batch, kEvictFirst);
+                                else
+                                    tma_load_4d(sQ + t * Cfg::kTileBytes + bx * (kBlock * 128), &tmQ, q_full, bx * 64, c.it.head, row, c.it.batch, kEvictFirst);
+                            }
                     }
                     const int hk = c.it.head / gm.group;
                     for (int kv = 0; kv < 2; ++kv) {       // K block then V block through the ring
                         mbar_wait(&kv_empty[stage], ring_phase ^ 1);
-                        mbar_expect_tx(&kv_full[stage], Cfg::kTileBytes);
-                        for (int bx = 0; bx < Cfg::kBoxes; ++bx)
-                            tma_load_4d(sRing + stage * Cfg::kTileBytes + bx * (kBlock * 128), kv == 0 ? &tmK : &tmV, &kv_full[stage],
-                                        bx * 64, hk, v * gm.L + t0, c.it.batch, kEvictLast);
+                        if constexpr (kPair) {
+                            if (leader) mbar_expect_tx(&kv_full[stage], Cfg::kTileBytes);      // both CTAs' halves
+                            uint8_t* dst = sRing + stage * Cfg::kSlotBytes;
+                            if (kv == 0)                                                       // K rows 64r .. 64r+63: two [64 x 64] boxes
+                                for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+                                    tma_load_4d_2cta(dst + bx * (kBlock / 2 * 128), &tmK, kv_full_r0 + stage * 8, bx * 64, hk,
+                                                     v * gm.L + t0 + (int)pair_rank * (kBlock / 2), c.it.batch, kEvictLast);
+                            else                                                               // V columns 64r .. 64r+63: one [128 x 64] box
+                                tma_load_4d_2cta(dst, &tmV, kv_full_r0 + stage * 8, (int)pair_rank * 64, hk, v * gm.L + t0, c.it.batch, kEvictLast);
+                        } else {
+                            mbar_expect_tx(&kv_full[stage], Cfg::kTileBytes);
+                            for (int bx = 0; bx < Cfg::kBoxes; ++bx)
+                                tma_load_4d(sRing + stage * Cfg::kTileBytes + bx * (kBlock * 128), kv == 0 ? &tmK : &tmV, &kv_full[stage],
+                                            bx * 64, hk, v * gm.L + t0, c.it.batch, kEvictLast);
+                        }
                         if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
                     }
                 });
             }
         }
     } else if (warp == kMmaWarp) {
-        // =============================== MMA issuer ===============================
-        if (elect_one()) {
-            constexpr uint32_t idesc_qk = umma_idesc(kBlock, kBlock, false, false);
-            constexpr uint32_t idesc_pv = umma_idesc(kBlock, D, false, true);
+        // =============================== MMA issuer (kPair: rank 0 issues for both CTAs) ===============================
+        if (leader && elect_one()) {
+            constexpr int kM = kPair ? 2 * kBlock : kBlock;
+            constexpr uint32_t idesc_qk = umma_idesc(kM, kBlock, false, false);
+            constexpr uint32_t idesc_pv = umma_idesc(kM, D, false, true);
+            auto commit = [&](uint64_t* bar) {               // kPair: the same barrier of both CTAs
+                if constexpr (kPair) umma_commit_2cta(bar);
+                else umma_commit(bar);
+            };
             uint32_t stage = 0, ring_phase = 0, q_phase = 0, p_phase[2] = {0, 0};
             PT_DECL;
             auto ring_wait = [&](uint32_t& slot) {
@@ -242,23 +310,32 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 if (++stage == Cfg::kStages) { stage = 0; ring_phase ^= 1; }
             };
             auto issue_qk = [&](int t, uint32_t kslot) {
-                const uint32_t qa = smem_u32(sQ + t * Cfg::kTileBytes), ka = smem_u32(sRing + kslot * Cfg::kTileBytes);
+                const uint32_t qa = smem_u32(sQ + t * Cfg::kTileBytes), ka = smem_u32(sRing + kslot * Cfg::kSlotBytes);
 #pragma unroll
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t o = (kk / 4) * (kBlock * 128) + (kk % 4) * 32;
-                    umma_ss(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc_qk, kk > 0);
+                    if constexpr (kPair) {                   // this CTA's K half: 64 rows per 64-column box
+                        const uint32_t ob = (kk / 4) * (kBlock / 2 * 128) + (kk % 4) * 32;
+                        umma_ss_2cta(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + ob, 16, 1024), idesc_qk, kk > 0);
+                    } else {
+                        umma_ss(tmem + Cfg::kColS + t * kBlock, umma_desc(qa + o, 16, 1024), umma_desc(ka + o, 16, 1024), idesc_qk, kk > 0);
+                    }
                 }
             };
             // P (bf16) in TMEM over S: hi at columns 0..63, lo at 64..127; `half` = keys 0..63 or 64..127 of the block
             auto issue_pv = [&](int t, uint32_t vslot, int half, bool acc) {
-                const uint32_t va = smem_u32(sRing + vslot * Cfg::kTileBytes);
+                const uint32_t va = smem_u32(sRing + vslot * Cfg::kSlotBytes);
 #pragma unroll
                 for (int x = 0; x < (kSplit ? 2 : 1); ++x)
 #pragma unroll
                     for (int k4 = 0; k4 < kBlock / 32; ++k4) {
                         const int kk = half * (kBlock / 32) + k4;
-                        umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + x * 64 + kk * 8,
-                                umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || k4 > 0 || x > 0) ? 1u : 0u);
+                        if constexpr (kPair)                 // this CTA's V half: the 64 head_dim columns of one box, all 128 keys
+                            umma_ts_2cta(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + kk * 8,
+                                         umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || k4 > 0) ? 1u : 0u);
+                        else
+                            umma_ts(tmem + Cfg::kColO + t * D, tmem + Cfg::kColS + t * kBlock + x * 64 + kk * 8,
+                                    umma_desc(va + kk * 2048, kBlock * 128, 1024), idesc_pv, (acc || k4 > 0 || x > 0) ? 1u : 0u);
                     }
             };
             for (int idx = next_item(); idx < total_items; idx = next_item()) {
@@ -270,8 +347,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 uint32_t kslot, vslot;
                 ring_wait(kslot);
                 tc_fence_after();
-                for (int t = 0; t < c.nt; ++t) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
-                umma_commit(&kv_empty[kslot]);
+                for (int t = 0; t < c.nt; ++t) { issue_qk(t, kslot); commit(&s_full[t]); }
+                commit(&kv_empty[kslot]);
                 for (int j = 0; j < nb; ++j) {
                     const bool more = j + 1 < nb;
                     PT_MARK(0);
@@ -279,6 +356,8 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     if (more) ring_wait(kslot);
                     PT_MARK(1);
                     for (int t = 0; t < c.nt; ++t) {
+                        // (kPair: P lives in tensor memory, ordered by the tcgen05 fences on both sides of the barrier: the wait needs no
+                        // cluster-scope acquire, which would cost a cache invalidation per wait)
                         mbar_wait(&p_half[2 * t], p_phase[t]);       // the PV MMA starts on the first 64 keys while the softmax
                         tc_fence_after();                             // group is still exponentiating the other 64
                         PT_MARK(2 + 2 * t);
@@ -287,14 +366,14 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         p_phase[t] ^= 1;
                         tc_fence_after();
                         issue_pv(t, vslot, 1, true);
-                        if (more) { issue_qk(t, kslot); umma_commit(&s_full[t]); }
-                        else umma_commit(&o_full[t]);
+                        if (more) { issue_qk(t, kslot); commit(&s_full[t]); }
+                        else commit(&o_full[t]);
                         PT_MARK(3 + 2 * t);
                     }
-                    umma_commit(&kv_empty[vslot]);
-                    if (more) umma_commit(&kv_empty[kslot]);
+                    commit(&kv_empty[vslot]);
+                    if (more) commit(&kv_empty[kslot]);
                 }
-                umma_commit(q_empty);
+                commit(q_empty);
             }
             PT_REPORT("fwd MMA thread clocks per block: ring_wait, wait_p0, issue0, wait_p1, issue1");
         }
@@ -307,6 +386,7 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
         const uint32_t tS = tmem + lane_base + Cfg::kColS + t * kBlock;
         const uint32_t tO = tmem + lane_base + Cfg::kColO + t * D;
         const float c2 = gm.scale_log2;
+        const uint32_t p_half_r0 = kPair ? mapa(smem_u32(p_half), 0u) : 0u;
         uint32_t s_phase = 0, o_phase = 0;
         PT_DECL;
         for (int idx = next_item(); idx < total_items; idx = next_item()) {
@@ -328,8 +408,13 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 tc_fence_after();
                 if (kFwdAblate & 1) {
                     tc_fence_before();
-                    mbar_arrive(&p_half[2 * t]);
-                    mbar_arrive(&p_half[2 * t + 1]);
+                    if (kPair && !leader) {
+                        __syncwarp();
+                        if (lane == 0) { mbar_arrive_remote(p_half_r0 + (2 * t) * 8); mbar_arrive_remote(p_half_r0 + (2 * t + 1) * 8); }
+                    } else {
+                        mbar_arrive(&p_half[2 * t]);
+                        mbar_arrive(&p_half[2 * t + 1]);
+                    }
                     ++j;
                     return;
                 }
@@ -410,7 +495,12 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                         if (ch & 1) {                                 // half of the keys done: hand it to the PV MMA
                             tmem_st_wait();
                             tc_fence_before();
-                            mbar_arrive(&p_half[2 * t + (ch >> 1)]);
+                            if (kPair && !leader) {                   // the issuer is in the peer CTA: one arrival per warp on ITS barrier
+                                __syncwarp();
+                                if (lane == 0) mbar_arrive_remote(p_half_r0 + (2 * t + (ch >> 1)) * 8);
+                            } else {
+                                mbar_arrive(&p_half[2 * t + (ch >> 1)]);
+                            }
                         }
                     }
                 };
@@ -451,16 +541,50 @@ tile_fwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
 
     tc_fence_before();
     __syncthreads();
-    if (warp == kAllocWarp) tmem_dealloc<512>(tmem);
+    if constexpr (kPair) cluster_sync();                // no CTA leaves while its peer may still read its operands or arrive on its barriers
+    if (warp == kAllocWarp) {
+        if constexpr (kPair) tmem_dealloc_2cta<512>(tmem);
+        else tmem_dealloc<512>(tmem);
+    }
 }
 
-template <int D, bool kSplit>
+template <int D, bool kSplit, bool kPair>
 int launch_fwd_one(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMap& tmK, const CUtensorMap& tmV, int grid, cudaStream_t stream)
 {
-    cudaError_t e = cudaFuncSetAttribute(tile_fwd_kernel<D, kSplit>, cudaFuncAttributeMaxDynamicSharedMemorySize, FwdCfg<D>::kSmemBytes);
+    using Cfg = FwdCfg<D, kPair>;
+    static_assert(Cfg::kSmemBytes <= 227 * 1024, "tile_fwd shared memory over the 227 KB CTA limit");
+    auto kernel = tile_fwd_kernel<D, kSplit, kPair>;
+    cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes);
     if (e != cudaSuccess) return (int)e;
-    tile_fwd_kernel<D, kSplit><<<grid, kThreads, FwdCfg<D>::kSmemBytes, stream>>>(tmQ, tmK, tmV, p);
-    return (int)cudaGetLastError();
+    cudaLaunchConfig_t cfg{};
+    cfg.blockDim = dim3(kThreads);
+    cfg.dynamicSmemBytes = Cfg::kSmemBytes;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    if (kPair) {
+        attr[0].id = cudaLaunchAttributeClusterDimension;
+        attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+        cfg.attrs = attr;
+        cfg.numAttrs = 1;
+        // co-resident 2-CTA clusters of this kernel (GPCs with an odd SM count leave one SM out), cached per device
+        constexpr int kMaxDevices = 64;
+        static std::atomic<int> max_clusters[kMaxDevices];      // 0 = not queried yet, else count + 1
+        int dev = 0;
+        e = cudaGetDevice(&dev);
+        if (e != cudaSuccess) return (int)e;
+        int n = (dev >= 0 && dev < kMaxDevices) ? max_clusters[dev].load(std::memory_order_relaxed) - 1 : -1;
+        if (n < 0) {
+            cfg.gridDim = dim3(2);
+            e = cudaOccupancyMaxActiveClusters(&n, kernel, &cfg);
+            if (e != cudaSuccess) return (int)e;
+            if (dev >= 0 && dev < kMaxDevices) max_clusters[dev].store(n + 1, std::memory_order_relaxed);
+        }
+        if (n <= 0) return (int)cudaErrorLaunchOutOfResources;
+        grid = (grid / 2 < n ? grid / 2 : n) * 2;
+    }
+    cfg.gridDim = dim3(grid);
+    e = cudaLaunchKernelEx(&cfg, kernel, tmQ, tmK, tmV, p);
+    return e != cudaSuccess ? (int)e : (int)cudaGetLastError();
 }
 
 }  // namespace
@@ -471,9 +595,13 @@ int launch_tile_fwd(const FwdParams& p, const CUtensorMap& tmQ, const CUtensorMa
     const int total = p.items_per_gpu * p.g_count;
     if (total <= 0) return 0;
     const int grid = total < num_sms ? total : num_sms;
+    if (p.pair) {                                       // checked by the caller: head_dim 128, single-operand mode, an even item count
+        if (p.gm.head_dim != 128 || p.split || (total & 1)) return (int)cudaErrorInvalidValue;
+        return launch_fwd_one<128, false, true>(p, tmQ, tmK, tmV, grid, stream);
+    }
     if (p.gm.head_dim == 128)
-        return p.split ? launch_fwd_one<128, true>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<128, false>(p, tmQ, tmK, tmV, grid, stream);
-    return p.split ? launch_fwd_one<64, true>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<64, false>(p, tmQ, tmK, tmV, grid, stream);
+        return p.split ? launch_fwd_one<128, true, false>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<128, false, false>(p, tmQ, tmK, tmV, grid, stream);
+    return p.split ? launch_fwd_one<64, true, false>(p, tmQ, tmK, tmV, grid, stream) : launch_fwd_one<64, false, false>(p, tmQ, tmK, tmV, grid, stream);
 }
 
 }  // namespace mesh_attn

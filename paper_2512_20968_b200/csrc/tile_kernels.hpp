@@ -31,6 +31,7 @@ struct FwdParams {
     int items_per_gpu;
     int g_first, g_count;
     int split;                 // precision: 1 = P fed to the PV MMA as hi + lo bf16
+    int pair;                  // 1: items 2k, 2k+1 stream the same K / V blocks -> 2-CTA clusters, cta_group::2 MMAs (tmK: 64-row boxes)
     float* partial_O;          // [g_count][slots][B][L][Hq][D]
     float* partial_lse;        // [g_count][slots][B][Hq][L]
     int* status;               // the plan's host-mapped status words (sm100.cuh watchdog); may be null

@@ -184,7 +184,7 @@ int main()
         d = desc(2, 2, 256, 4, 3, 64, 0, 1, 0, 0, 1, 1); CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
         d = desc(2, 2, 256, 4, 4, 96, 0, 1, 0, 0, 1, 1); CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EUNSUPPORTED);
         d = desc(2, 2, 256, 4, 4, 64, 0, 1, 0, 0, 5, 4); CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
-        d = desc(2, 2, 256, 4, 4, 64, 0, 1, 0, 0, 1, 1); d.reserved[0] = 1; CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
+        d = desc(2, 2, 256, 4, 4, 64, 0, 1, 0, 0, 1, 1); d.fwd_pairing = 2; CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
         d = desc(2, 2, 256, 4, 4, 64, 0, 1, 0, 0, 1, 1); d.out_dtype = 2; CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
         d = desc(2, 2, 256, 4, 4, 64, 0, 1, 0, 0, 1, 1); d.bwd_pairing = 7; CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);
         d = desc(1, 4096, 2048, 1, 1, 64, 0, 1, 0, 0, 16, 1); d.partial_mode = 1; CHECK(mesh_attn_plan_create(&d, &p) == MESH_ATTN_EINVAL);

@@ -186,3 +186,70 @@ def test_merge_kernel_alone(oracle):
         assert np.abs(O[row, h] - O_ref).max() <= 1e-5
         assert (l_ref == -np.inf and lse[h, row] == -np.inf) or abs(lse[h, row] - l_ref) <= 1e-5
     assert torch.all(buf.O[0, : w.a * w.L] == 0)              # other Q groups untouched
+
+
+@pytest.mark.parametrize("case", ["noncausal_odd_mesh", "striped_gqa", "striped_greedy_chunks", "batch2_bhnd", "per_pair", "usp_lanes"])
+def test_cta_pair_kernel_matches_single_cta_kernel(oracle, case):
+    """tile_fwd as 2-CTA clusters with tcgen05 cta_group::2 MMAs (plan desc field fwd_pairing, MESH_ATTN_Q_FWD_PAIRED): each CTA of
+    a pair holds half of every K / V block.  The arithmetic per output element is the same sequence of MMAs and softmax steps, so
+    O, lse and the partials are BIT-IDENTICAL to the single-CTA kernel's; the oracle is checked on the paired result.  Cases: an odd
+    mesh height (pairs straddle Q tiles and Q partitions), GQA (pairs inside a head group), the greedy order with chunked Q / KV
+    (several seg lists), batch 2 in the [B,H,N,D] layout, per-pair partials, Mesh-USP lanes."""
+    from dataclasses import replace
+
+    import paper_2512_20968_b200.binding as B
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    kw, layout = {}, 0
+    if case == "noncausal_odd_mesh":
+        w = W.Workload("pair_a", 41, False, 3, 3, 1, 9 * 512, 4, 4, 128)
+    elif case == "striped_gqa":
+        w = W.Workload("pair_b", 42, True, 2, 4, 1, 8 * 512, 8, 2, 128, seq_layout="striped")
+    elif case == "striped_greedy_chunks":
+        w = W.Workload("pair_c", 43, True, 4, 4, 1, 16 * 512, 2, 2, 128, seq_layout="striped", order="greedy", k_q=2, k_kv=2)
+    elif case == "batch2_bhnd":
+        w = W.Workload("pair_d", 44, True, 2, 2, 2, 4 * 256, 4, 4, 128, seq_layout="striped")
+        layout = 1
+    elif case == "per_pair":
+        w = W.Workload("pair_e", 45, False, 2, 3, 1, 6 * 256, 2, 2, 128)
+        kw = dict(partial_mode=1)
+    else:
+        w = W.Workload("pair_f", 46, True, 2, 2, 1, 4 * 512, 8, 4, 128, seq_layout="striped")
+        kw = dict(usp_lanes=2)
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    if layout == 1:
+        inp = {k_: v_.permute(0, 2, 1, 3).contiguous() for k_, v_ in inp.items()}
+    res = {}
+    for pairing in (0, 1):
+        plan = plan_for(w, fwd_pairing=pairing, tensor_layout=layout, **kw)
+        assert plan.query(B.Q_FWD_PAIRED) == 1 - pairing, (case, pairing)
+        buf = Buffers(plan, w, backward=False)
+        if layout == 1:
+            buf.O = buf.O.permute(0, 2, 1, 3).contiguous()
+        for t in (buf.O, buf.lse, buf.partial_O, buf.partial_lse):
+            t.fill_(float("nan"))
+        plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+        torch.cuda.synchronize()
+        plan.health()
+        res[pairing] = buf
+    a, b = res[0], res[1]
+    assert torch.equal(a.O, b.O) and torch.equal(a.lse, b.lse)
+    assert torch.equal(a.partial_lse, b.partial_lse) and torch.equal(a.partial_O.nan_to_num(7.0), b.partial_O.nan_to_num(7.0))
+    O = a.O[0].permute(1, 0, 2) if layout == 1 else a.O[0]
+    q_in = {k_: (v_.permute(0, 2, 1, 3).contiguous() if layout == 1 else v_) for k_, v_ in inp.items()}
+    rows = sample_rows(w, 3, np.random.default_rng(41))
+    check_against_oracle(oracle, w, q_in, O.cpu().numpy(), a.lse[0].cpu().numpy(), rows=rows)
+
+
+def test_cta_pair_kernel_is_not_used_where_the_streams_differ():
+    """contiguous causal layout with a > 1: the Q partitions of a pair see different KV partitions -> single-CTA kernel; likewise
+    head_dim 64 and precision = 1 (the pair kernel is built for head_dim 128, one bf16 operand)."""
+    import paper_2512_20968_b200.binding as B
+    from paper_2512_20968_b200 import plan_for
+
+    base = dict(a=2, b=2, n=4, batch=1, seq_total=4 * 512, heads_q=4, heads_kv=4, head_dim=128)
+    assert B.Plan(causal=1, seq_layout=0, **base).query(B.Q_FWD_PAIRED) == 0
+    assert B.Plan(causal=1, seq_layout=1, **base).query(B.Q_FWD_PAIRED) == 1
+    assert B.Plan(causal=1, seq_layout=1, precision=1, **base).query(B.Q_FWD_PAIRED) == 0
+    assert B.Plan(causal=1, seq_layout=1, fwd_pairing=1, **base).query(B.Q_FWD_PAIRED) == 0
+    assert B.Plan(causal=0, **dict(base, head_dim=64)).query(B.Q_FWD_PAIRED) == 0

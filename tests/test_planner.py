@@ -308,3 +308,25 @@ def test_out_dtype_field_is_validated_and_sizes_the_backward_workspace():
         with pytest.raises(MeshAttnError) as e:
             Plan(out_dtype=bad, **kw)
         assert e.value.status == B.EINVAL
+
+
+def test_forward_item_pairing_rule():
+    """MESH_ATTN_Q_FWD_PAIRED (tile_fwd as CTA pairs, tcgen05 cta_group::2): items 2k, 2k+1 must stream the same K / V blocks on
+    every simulated GPU -- true for non-causal and striped-causal plans with an even item count, false for the contiguous causal
+    layout with a > 1 (the pair's Q partitions see different KV partitions); head_dim 128 and precision 0 only; fwd_pairing = 1
+    turns it off.  BASELINE.json's configs: C2, C4, C5 pair, C3 (contiguous, precision 1) and C1 (head_dim 64) do not."""
+    base = dict(a=2, b=2, n=4, batch=1, seq_total=4 * 512, heads_q=4, heads_kv=4, head_dim=128)
+    assert Plan(causal=0, **base).query(B.Q_FWD_PAIRED) == 1
+    assert Plan(causal=1, seq_layout=1, **base).query(B.Q_FWD_PAIRED) == 1
+    assert Plan(causal=1, seq_layout=0, **base).query(B.Q_FWD_PAIRED) == 0
+    assert Plan(causal=1, seq_layout=0, **dict(base, a=1, b=4, heads_q=8, heads_kv=2)).query(B.Q_FWD_PAIRED) == 1   # a = 1: pairs inside a GQA group
+    assert Plan(causal=1, seq_layout=1, precision=1, **base).query(B.Q_FWD_PAIRED) == 0
+    assert Plan(causal=1, seq_layout=1, fwd_pairing=1, **base).query(B.Q_FWD_PAIRED) == 0
+    assert Plan(causal=0, **dict(base, head_dim=64)).query(B.Q_FWD_PAIRED) == 0
+    for bad in (-1, 2):
+        with pytest.raises(MeshAttnError):
+            Plan(fwd_pairing=bad, **base)
+    from paper_2512_20968_b200 import plan_for, workloads as W
+    got = {name: plan_for(W.scaled_down(w, 512)).query(B.Q_FWD_PAIRED) for name, w in W.CONFIGS.items() if name != "C1"}
+    assert got == {"C2": 1, "C3": 0, "C4": 1, "C5": 1}, got
+    assert plan_for(W.scaled_down(W.C2, 256)).query(B.Q_FWD_PAIRED) == 0     # 3 items per KV head: a pair would straddle two heads
