@@ -488,21 +488,32 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     ds_ph ^= 1;
                     tc_fence_after();
                     PT_MARK(3);
+                    auto issue_dq = [&]() {
 #pragma unroll
-                    for (int x = 0; x < Cfg::kNumDs; ++x)
+                        for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
-                        for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
-                                    umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
-                    umma_commit(dq_full);
+                            for (int kk = 0; kk < kBlock / 16; ++kk)
+                                umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
+                                        umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
+                        umma_commit(dq_full);
+                    };
+                    auto issue_dk = [&]() {
 #pragma unroll
-                    for (int x = 0; x < Cfg::kNumDs; ++x)
+                        for (int x = 0; x < Cfg::kNumDs; ++x)
 #pragma unroll
-                        for (int kk = 0; kk < kBlock / 16; ++kk)
-                            umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
-                                    umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
-                    if constexpr (kPair) umma_commit_mc(&qd_empty[st_cur], 3);
-                    else umma_commit(&qd_empty[st_cur]);
+                            for (int kk = 0; kk < kBlock / 16; ++kk)
+                                umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
+                                        umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
+                        if constexpr (kPair) umma_commit_mc(&qd_empty[st_cur], 3);
+                        else umma_commit(&qd_empty[st_cur]);
+                    };
+                    if constexpr (Cfg::kStages == 1) {   // single Q stage (hi+lo operands): dK first, it is what releases the stage, so that
+                        issue_dk();                      // Q(i+1) is loaded under the two dQ^T MMAs instead of after them
+                        issue_dq();
+                    } else {
+                        issue_dq();
+                        issue_dk();
+                    }
                     if (Cfg::kStages == 1 && more) {     // single stage: Q(i+1) can only land once dK(i) released the stage
                         st_next = next_stage();
                         mma_kmajor(Cfg::kColS, aK, smem_u32(sQ(st_next)));
