@@ -8,7 +8,8 @@ memory -- its partial (O, lse) scratch is a 32 MiB device array built into the l
 
 Each result is compared with the existing path's on the same inputs, within BASELINE.json's forward tolerances (the two run the
 same kernels, so the difference printed is 0), and call 1 with the fp64 oracle on sampled rows.  Also: a plan beyond the limit is
-refused with both byte counts in the error and launches nothing; the calls leave the device's free memory unchanged.
+refused with both byte counts in the error and launches nothing; the calls leave the device's free memory unchanged; the call
+is captured into a CUDA graph and replayed (the use it exists for).
 
 The file sorts last on purpose (pytest -x at the round's end: a failure here hides no other test); it passes alone in a fresh
 process and after the other tests (the array is shared with nothing else)."""
@@ -94,3 +95,37 @@ def test_forward_static_refuses_plans_beyond_the_array():
     assert str(need) in str(e.value) and str(cap) in str(e.value), str(e.value)
     torch.cuda.synchronize()
     assert launch_count() == n0 and not O.any() and not lse.any()          # nothing was launched, nothing written
+
+
+def test_forward_static_under_cuda_graph_capture():
+    """The use the entry point is for: it is captured into a CUDA graph (no allocation, no host synchronisation, nothing on the
+    default stream; the per-launch 4-byte memset of the work-item counter and the cluster launches are capturable) and the
+    replays give the eager result bit for bit, also after the inputs were changed in place."""
+    from paper_2512_20968_b200 import plan_for
+
+    w = W.Workload("static_graph", 25, True, 2, 2, 1, 2048, 4, 4, 128, seq_layout="striped")
+    plan = plan_for(w)
+    inp = W.make_inputs(w, "cuda", which=("q", "k", "v"))
+    O_ref, lse_ref = _existing_path(plan, w, inp)
+    O, lse = torch.full_like(O_ref, float("nan")), torch.full_like(lse_ref, float("nan"))
+    side = torch.cuda.Stream()
+    with torch.cuda.stream(side):
+        plan.forward_static(inp["q"], inp["k"], inp["v"], O, lse, stream=side)      # warm-up: attributes, occupancy query, scratch address
+    side.synchronize()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph, stream=side):
+        plan.forward_static(inp["q"], inp["k"], inp["v"], O, lse, stream=torch.cuda.current_stream())
+    for rep in range(2):
+        O.fill_(float("nan"))
+        lse.fill_(float("nan"))
+        graph.replay()
+        torch.cuda.synchronize()
+        assert torch.equal(O, O_ref) and torch.equal(lse, lse_ref), rep
+    other = W.make_inputs(W.Workload("static_graph2", 26, True, 2, 2, 1, 2048, 4, 4, 128, seq_layout="striped"), "cuda", which=("q", "k", "v"))
+    O2_ref, lse2_ref = _existing_path(plan, w, other)
+    for name in ("q", "k", "v"):
+        inp[name].copy_(other[name])                       # same buffers, new contents
+    graph.replay()
+    torch.cuda.synchronize()
+    plan.health()
+    assert torch.equal(O, O2_ref) and torch.equal(lse, lse2_ref)
