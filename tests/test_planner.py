@@ -330,3 +330,16 @@ def test_forward_item_pairing_rule():
     got = {name: plan_for(W.scaled_down(w, 512)).query(B.Q_FWD_PAIRED) for name, w in W.CONFIGS.items() if name != "C1"}
     assert got == {"C2": 1, "C3": 0, "C4": 1, "C5": 1}, got
     assert plan_for(W.scaled_down(W.C2, 256)).query(B.Q_FWD_PAIRED) == 0     # 3 items per KV head: a pair would straddle two heads
+
+
+def test_kernel_variants_chosen_for_the_baseline_configs_at_full_size():
+    """Which tile kernels BASELINE.json's configs run at FULL size (host-only plans, no GPU needed): the CTA-pair forward
+    (MESH_ATTN_Q_FWD_PAIRED) and the paired backward with the dQ exchange (MESH_ATTN_Q_BWD_PAIRED = 2) on C2, C4, C5; on C3
+    (contiguous causal layout, precision 1) the single-CTA forward and the paired backward without the exchange (1); C1 (head_dim 64)
+    does not pair the forward and runs no backward."""
+    from paper_2512_20968_b200 import plan_for, workloads as W
+
+    fwd = {name: plan_for(w).query(B.Q_FWD_PAIRED) for name, w in W.CONFIGS.items()}
+    assert fwd == {"C1": 0, "C2": 1, "C3": 0, "C4": 1, "C5": 1}, fwd
+    bwd = {name: plan_for(w).query(B.Q_BWD_PAIRED) for name, w in W.CONFIGS.items() if name != "C1"}
+    assert bwd == {"C2": 2, "C3": 1, "C4": 2, "C5": 2}, bwd
