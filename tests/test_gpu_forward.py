@@ -253,3 +253,36 @@ def test_cta_pair_kernel_is_not_used_where_the_streams_differ():
     assert B.Plan(causal=1, seq_layout=1, precision=1, **base).query(B.Q_FWD_PAIRED) == 0
     assert B.Plan(causal=1, seq_layout=1, fwd_pairing=1, **base).query(B.Q_FWD_PAIRED) == 0
     assert B.Plan(causal=0, **dict(base, head_dim=64)).query(B.Q_FWD_PAIRED) == 0
+
+
+def test_cta_pair_kernel_rescale_path_on_outlier_scores(oracle):
+    """Outlier scores (4 of 128 channels x 8: BASELINE.json configs[2]'s value distribution) with precision = 0: the running row
+    maximum jumps by more than 2^8 again and again, so the accumulator rescale in tensor memory (rare on N(0,1) data) runs in
+    both CTAs of a pair between the pair's MMAs.  Pair kernel and single-CTA kernel must agree bit for bit; the oracle is met at the
+    accuracy one bf16 P operand allows on such data (the tolerance BASELINE.json asks for needs precision = 1 here)."""
+    import paper_2512_20968_b200.binding as B
+    from paper_2512_20968_b200 import Buffers, plan_for
+
+    w = W.Workload("pair_outlier", 47, True, 2, 2, 1, 4 * 1024, 4, 4, 128, outlier=True, seq_layout="striped")
+    inp = W.make_inputs(w, "cuda", ("q", "k", "v"))
+    res = {}
+    for pairing in (0, 1):
+        plan = plan_for(w, fwd_pairing=pairing, precision=0)
+        assert plan.query(B.Q_FWD_PAIRED) == 1 - pairing
+        buf = Buffers(plan, w, backward=False)
+        buf.O.fill_(float("nan"))
+        buf.lse.fill_(float("nan"))
+        plan.forward(inp["q"], inp["k"], inp["v"], buf.O, buf.lse, buf.partial_O, buf.partial_lse)
+        torch.cuda.synchronize()
+        plan.health()
+        res[pairing] = buf
+    assert torch.equal(res[0].O, res[1].O) and torch.equal(res[0].lse, res[1].lse)
+    q, k, v = (torch_bits(inp[x][0]) for x in ("q", "k", "v"))
+    pos = oracle.positions(w.n, w.L, w.seq_layout)
+    rows = sample_rows(w, 6, np.random.default_rng(47))
+    rr, hh = np.tile(rows, w.heads_q), np.repeat(np.arange(w.heads_q, dtype=np.int32), len(rows))
+    O_ref, lse_ref = oracle.fwd_rows(q, k, v, w.scale, w.causal, pos, rr, hh)
+    eO = np.abs(res[0].O[0].cpu().numpy()[rr, hh].astype(np.float64) - O_ref).max()
+    el = np.abs(res[0].lse[0].cpu().numpy()[hh, rr].astype(np.float64) - lse_ref).max()
+    print(f"\npair kernel on outlier scores, precision 0: max|dO| {eO:.2e} max|dLSE| {el:.2e} (score range +-{np.abs(lse_ref).max():.0f})")
+    assert eO <= 3e-2 and el <= 1e-2
