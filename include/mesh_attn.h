@@ -358,12 +358,16 @@ int mesh_attn_backward(const mesh_attn_plan* plan, const void* Q, const void* K,
  * into the caller's device staging buffers, runs forward (and backward if dO_host != NULL),
  * copies O, lse (and dQ,dK,dV) device->host, and synchronises `stream` before returning.
  * The kernels run on `stream`; the copies run on two plan-owned streams (one per direction) ordered
- * against it by events, so that transfers overlap the kernels that do not need them: K, V and the
- * Q rows of the first Q group go up first, the other Q groups and dO follow behind the forward
- * waves; O and lse come down during the backward, the dQ rows of Q group r as soon as the
- * simulated GPUs of group r are done (batch 1, tensor_layout 0; whole tensors otherwise), dK and
- * dV at the end.  One step_host per plan at a time.  d_* are caller-owned DEVICE buffers of the
- * shapes above. */
+ * against it by events, so that transfers overlap the kernels that do not need them.  With batch 1
+ * and tensor_layout 0 (the rows of a partition are one byte range): the Q rows of the first Q
+ * group go up first, then K and V one KV column at a time (the b partitions of I^KV of the
+ * simulated GPUs g with g mod a = c); the first forward wave runs one launch per
+ * simulated GPU, each behind its own column; the other Q groups and dO follow behind the forward
+ * waves.  O and lse come down during the backward, the dQ rows of Q group r as soon as the
+ * simulated GPUs of group r are done; the LAST backward group runs one launch per simulated GPU
+ * again, and dK, dV of KV column c come down behind the launch that completes them (Alg.3 l.7,
+ * P:L255).  Otherwise whole tensors move: K, V, Q before the forward, dQ, dK, dV after the backward.
+ * One step_host per plan at a time.  d_* are caller-owned DEVICE buffers of the shapes above. */
 typedef struct {
     const void *Q_host, *K_host, *V_host, *dO_host;      /* bf16 host inputs (dO_host may be NULL) */
     void *O_host, *lse_host, *dQ_host, *dK_host, *dV_host; /* host outputs (any may be NULL = not copied back): lse fp32; O, dQ, dK, dV

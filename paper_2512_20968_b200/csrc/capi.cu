@@ -176,12 +176,13 @@ int upload_plan(mesh_attn_plan* p)
         e = cudaHostGetDevicePointer((void**)&p->d_status, p->h_status, 0);
     }
     if (e != cudaSuccess) { free_plan_device(p); return cuda_fail("plan_create: status words", (int)e); }
-    // step_host's copy engines: one stream per direction, events for the chunk hand-offs
+    // step_host's copy engines: one stream per direction, events for the chunk hand-offs (2b + 8, then a per copy direction for
+    // the KV columns: the list in mesh_attn_step_host)
     cudaStream_t s0 = nullptr, s1 = nullptr;
     e = cudaStreamCreateWithFlags(&s0, cudaStreamNonBlocking);
     if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&s1, cudaStreamNonBlocking);
     p->s_h2d = s0; p->s_d2h = s1;
-    for (int i = 0; e == cudaSuccess && i < 2 * p->geom.b + 8; ++i) {
+    for (int i = 0; e == cudaSuccess && i < 2 * p->geom.b + 8 + 2 * p->geom.a; ++i) {
         cudaEvent_t ev = nullptr;
         e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming);
         if (e == cudaSuccess) p->copy_events.push_back(ev);
@@ -719,36 +720,67 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
     cudaStream_t st = (cudaStream_t)stream, up = (cudaStream_t)p->s_h2d, down = (cudaStream_t)p->s_d2h;
     auto ev = [&](int i) { return (cudaEvent_t)p->copy_events[i]; };
     // events: 0 start, 1 K,V on the device, 2 dO on the device, 3 forward done, 4 backward done, 5 copies back done,
-    //         6+r Q rows of Q group r on the device, 6+b+r dQ rows of Q group r final
-    // Rows of Q group r are one contiguous byte range when batch == 1 in the [B,N,H,D] layout: then Q goes up and dQ comes
-    // down group by group, behind / ahead of the waves that need them; otherwise whole tensors move.
-    const bool by_group = gm.batch == 1 && p->desc.tensor_layout == 0 && nb > 1;
+    //         6+r Q rows of Q group r on the device, 6+b+r dQ rows of Q group r final, 2b+8+c K,V partitions of KV column c on
+    //         the device, 2b+8+a+c dK,dV partitions of KV column c final
+    // Rows of one partition are one contiguous byte range when batch == 1 in the [B,N,H,D] layout: then Q goes up and dQ comes
+    // down Q group by Q group, behind / ahead of the waves that need them, and K, V go up / dK, dV come down KV column by KV
+    // column (the b partitions of I^KV of the simulated GPUs g with g mod a = c) around the FIRST forward wave
+    // and the LAST backward group, which run one launch per simulated GPU; otherwise whole tensors move.
+    const bool rows_contig = gm.batch == 1 && p->desc.tensor_layout == 0;
+    const bool by_group = rows_contig && nb > 1;
+    const bool by_col = rows_contig && gm.a > 1;
     const size_t q_chunk = nq / nb;                   // elements of one Q group's rows
+    const size_t kv_part = nk / gm.n;                 // elements of one KV partition's rows
+    const size_t po_gpu = (size_t)gm.slots_per_gpu * gm.batch * gm.L * gm.heads_q * gm.head_dim;     // partial_O floats of one simulated GPU
+    const size_t pl_gpu = (size_t)gm.slots_per_gpu * gm.batch * gm.L * gm.heads_q;
+    auto ev_col_up = [&](int c) { return ev(2 * nb + 8 + c); };
+    auto ev_col_down = [&](int c) { return ev(2 * nb + 8 + gm.a + c); };
     cudaError_t e = cudaEventRecord(ev(0), st);
     auto ok = [&]() { return e == cudaSuccess; };
     if (ok()) e = cudaStreamWaitEvent(up, ev(0), 0);
     if (ok()) e = cudaStreamWaitEvent(down, ev(0), 0);
     // ---- host -> device, in the order the kernels need the data
-    if (ok()) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, up);
-    if (ok()) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, up);
-    if (ok()) e = cudaEventRecord(ev(1), up);
-    for (int r = 0; r < nb && ok(); ++r) {
+    auto upload_q = [&](int r) {
         if (by_group) e = cudaMemcpyAsync((char*)io->d_Q + r * q_chunk * 2, (const char*)io->Q_host + r * q_chunk * 2, q_chunk * 2, cudaMemcpyHostToDevice, up);
         else if (r == 0) e = cudaMemcpyAsync(io->d_Q, io->Q_host, nq * 2, cudaMemcpyHostToDevice, up);
         if (ok()) e = cudaEventRecord(ev(6 + r), up);
+    };
+    if (by_col) {
+        upload_q(0);                                   // the first wave starts behind 1 Q group + 1 KV column
+        for (int c = 0; c < gm.a && ok(); ++c) {
+            for (int t = 0; t < gm.b && ok(); ++t) {
+                const size_t at = (size_t)kv_partition(gm, c, t) * kv_part * 2;
+                e = cudaMemcpyAsync((char*)io->d_K + at, (const char*)io->K_host + at, kv_part * 2, cudaMemcpyHostToDevice, up);
+                if (ok()) e = cudaMemcpyAsync((char*)io->d_V + at, (const char*)io->V_host + at, kv_part * 2, cudaMemcpyHostToDevice, up);
+            }
+            if (ok()) e = cudaEventRecord(ev_col_up(c), up);
+        }
+    } else {
+        if (ok()) e = cudaMemcpyAsync(io->d_K, io->K_host, nk * 2, cudaMemcpyHostToDevice, up);
+        if (ok()) e = cudaMemcpyAsync(io->d_V, io->V_host, nk * 2, cudaMemcpyHostToDevice, up);
     }
+    if (ok()) e = cudaEventRecord(ev(1), up);
+    for (int r = by_col ? 1 : 0; r < nb && ok(); ++r) upload_q(r);
     if (bwd) {
         if (ok()) e = cudaMemcpyAsync(io->d_dO, io->dO_host, nq * 2, cudaMemcpyHostToDevice, up);      // lands during the forward
         if (ok()) e = cudaEventRecord(ev(2), up);
     }
     if (!ok()) return cuda_fail("step_host H2D", (int)e);
-    // ---- forward: wave r of every lane needs K, V and the Q rows of group r
-    e = cudaStreamWaitEvent(st, ev(1), 0);
+    // ---- forward: wave r of every lane needs K, V and the Q rows of group r; the first wave takes its simulated GPUs one by one,
+    // each behind the upload of its own KV column
+    if (!by_col) e = cudaStreamWaitEvent(st, ev(1), 0);
     for (int lane = 0; lane < U; ++lane)
         for (int r = 0; r < nb; ++r) {
             if (lane == 0 && ok()) e = cudaStreamWaitEvent(st, ev(6 + r), 0);
             if (!ok()) return cuda_fail("step_host forward", (int)e);
-            if (int rc = mesh_attn_tile_fwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, (float*)io->d_partial_O, (float*)io->d_partial_lse, stream)) return rc;
+            if (by_col && lane == 0 && r == 0) {
+                for (int c = 0; c < gm.a; ++c) {
+                    e = cudaStreamWaitEvent(st, ev_col_up(c), 0);
+                    if (!ok()) return cuda_fail("step_host forward", (int)e);
+                    if (int rc = mesh_attn_tile_fwd(p, c, 1, io->d_Q, io->d_K, io->d_V, (float*)io->d_partial_O + c * po_gpu, (float*)io->d_partial_lse + c * pl_gpu, stream)) return rc;
+                }
+            } else if (int rc = mesh_attn_tile_fwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, (float*)io->d_partial_O, (float*)io->d_partial_lse, stream))
+                return rc;
             if (int rc = mesh_attn_merge(p, lane * nb + r, (const float*)io->d_partial_O, (const float*)io->d_partial_lse, io->d_O, (float*)io->d_lse, stream)) return rc;
         }
     e = cudaEventRecord(ev(3), st);
@@ -764,10 +796,34 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
         if (ok()) e = cudaMemsetAsync(aV, 0, nk * 4, st);
         if (!ok()) return cuda_fail("step_host backward setup", (int)e);
         if (int rc = mesh_attn_bwd_preprocess(p, io->d_O, io->d_dO, (const float*)io->d_lse, (float*)io->d_bwd_ws, stream)) return rc;
+        // the last group runs one launch per simulated GPU: dK, dV of KV column c are final once every simulated GPU of the column
+        // has run (Alg.3 l.7), and come down behind that launch instead of behind the whole backward
+        const bool cols_down = by_col && (io->dK_host || io->dV_host);
         for (int lane = 0; lane < U; ++lane)
             for (int r = 0; r < nb; ++r) {
-                if (int rc = mesh_attn_tile_bwd(p, lane * gm.n + r * gm.a, gm.a, io->d_Q, io->d_K, io->d_V, io->d_dO, (const float*)io->d_bwd_ws, aQ, aK,
-                                                aV, stream))
+                const int g_first = lane * gm.n + r * gm.a;
+                if (cols_down && lane == U - 1 && r == nb - 1) {
+                    for (int c = 0; c < gm.a; ++c) {
+                        if (int rc = mesh_attn_tile_bwd(p, g_first + c, 1, io->d_Q, io->d_K, io->d_V, io->d_dO, (const float*)io->d_bwd_ws, aQ, aK, aV, stream)) return rc;
+                        if (bf16_out) {
+                            for (int t = 0; t < gm.b; ++t) {
+                                const size_t at = (size_t)kv_partition(gm, c, t) * kv_part;
+                                int err = launch_cast_bf16(aK + at, (char*)io->d_dK + at * 2, (long long)kv_part, p->num_sms, st);
+                                if (!err) err = launch_cast_bf16(aV + at, (char*)io->d_dV + at * 2, (long long)kv_part, p->num_sms, st);
+                                if (err) return cuda_fail("step_host cast launch", err);
+                                g_launches.fetch_add(2);
+                            }
+                        }
+                        e = cudaEventRecord(ev_col_down(c), st);
+                        if (ok()) e = cudaStreamWaitEvent(down, ev_col_down(c), 0);
+                        for (int t = 0; t < gm.b && ok(); ++t) {
+                            const size_t at = (size_t)kv_partition(gm, c, t) * kv_part * ob;
+                            if (io->dK_host) e = cudaMemcpyAsync((char*)io->dK_host + at, (const char*)io->d_dK + at, kv_part * ob, cudaMemcpyDeviceToHost, down);
+                            if (ok() && io->dV_host) e = cudaMemcpyAsync((char*)io->dV_host + at, (const char*)io->d_dV + at, kv_part * ob, cudaMemcpyDeviceToHost, down);
+                        }
+                        if (!ok()) return cuda_fail("step_host dK, dV D2H", (int)e);
+                    }
+                } else if (int rc = mesh_attn_tile_bwd(p, g_first, gm.a, io->d_Q, io->d_K, io->d_V, io->d_dO, (const float*)io->d_bwd_ws, aQ, aK, aV, stream))
                     return rc;
                 if (lane == U - 1 && by_group) {
                     if (bf16_out) {                  // the rows of Q group r are final: round them into the caller's dQ
@@ -785,16 +841,16 @@ int mesh_attn_step_host(const mesh_attn_plan* p, const mesh_attn_host_io* io, vo
             }
         if (bf16_out) {
             int err = by_group ? 0 : launch_cast_bf16(aQ, io->d_dQ, (long long)nq, p->num_sms, st);
-            if (!err) err = launch_cast_bf16(aK, io->d_dK, (long long)nk, p->num_sms, st);
-            if (!err) err = launch_cast_bf16(aV, io->d_dV, (long long)nk, p->num_sms, st);
+            if (!err && !cols_down) err = launch_cast_bf16(aK, io->d_dK, (long long)nk, p->num_sms, st);
+            if (!err && !cols_down) err = launch_cast_bf16(aV, io->d_dV, (long long)nk, p->num_sms, st);
             if (err) return cuda_fail("step_host cast launch", err);
-            g_launches.fetch_add(by_group ? 2 : 3);
+            g_launches.fetch_add((by_group ? 0 : 1) + (cols_down ? 0 : 2));
         }
         e = cudaEventRecord(ev(4), st);
         if (ok()) e = cudaStreamWaitEvent(down, ev(4), 0);
         if (ok() && io->dQ_host && !by_group) e = cudaMemcpyAsync(io->dQ_host, io->d_dQ, nq * ob, cudaMemcpyDeviceToHost, down);
-        if (ok() && io->dK_host) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * ob, cudaMemcpyDeviceToHost, down);
-        if (ok() && io->dV_host) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * ob, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dK_host && !cols_down) e = cudaMemcpyAsync(io->dK_host, io->d_dK, nk * ob, cudaMemcpyDeviceToHost, down);
+        if (ok() && io->dV_host && !cols_down) e = cudaMemcpyAsync(io->dV_host, io->d_dV, nk * ob, cudaMemcpyDeviceToHost, down);
     }
     if (ok()) e = cudaEventRecord(ev(5), down);
     if (ok()) e = cudaStreamWaitEvent(st, ev(5), 0);

@@ -259,8 +259,9 @@ def test_split_precision_iid(oracle):
 
 @pytest.mark.parametrize("batch,lanes", [(1, 1), (1, 2), (2, 1)])
 def test_step_host_matches_device_calls_and_profile_counters(batch, lanes):
-    """mesh_attn_step_host (host buffers; H2D, forward, backward and D2H overlapped on its copy streams: Q up and dQ down
-    per Q group when batch == 1, whole tensors otherwise) gives what the device-pointer calls give, twice in a row;
+    """mesh_attn_step_host (host buffers; H2D, forward, backward and D2H overlapped on its copy streams: when batch == 1, Q up
+    and dQ down per Q group, K, V up and dK, dV down per KV column around the first forward wave / last backward group, which
+    then run one launch per simulated GPU; whole tensors otherwise) gives what the device-pointer calls give, twice in a row;
     the per-kernel event profile counts one record per launch."""
     from paper_2512_20968_b200 import Buffers
     from paper_2512_20968_b200 import binding as B
@@ -287,7 +288,8 @@ def test_step_host_matches_device_calls_and_profile_counters(batch, lanes):
         counts = {k: B.profile_read(k)[1] for k in (B.K_TILE_FWD, B.K_MERGE, B.K_BWD_PREPROCESS, B.K_TILE_BWD)}
         B.profile_enable(False)
         waves = w.b * lanes
-        assert counts == {B.K_TILE_FWD: waves, B.K_MERGE: waves, B.K_BWD_PREPROCESS: 1, B.K_TILE_BWD: waves}
+        tiles = waves + (w.a - 1 if batch == 1 else 0)      # one wave / group split into its a simulated GPUs
+        assert counts == {B.K_TILE_FWD: tiles, B.K_MERGE: waves, B.K_BWD_PREPROCESS: 1, B.K_TILE_BWD: tiles}
         assert torch.equal(out["O"], ref.O.cpu()) and torch.equal(out["lse"], ref.lse.cpu())   # forward is deterministic
         for name, t in (("dQ", ref.dQ), ("dK", ref.dK), ("dV", ref.dV)):                      # atomics: order-dependent last bits
             assert (out[name] - t.cpu()).abs().max().item() <= 1e-3
