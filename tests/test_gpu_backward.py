@@ -295,6 +295,39 @@ def test_step_host_matches_device_calls_and_profile_counters(batch, lanes):
             assert (out[name] - t.cpu()).abs().max().item() <= 1e-3
 
 
+@pytest.mark.parametrize("kvr,a,b", [(False, 3, 2), (True, 4, 1), (False, 1, 4)])
+def test_step_host_kv_columns_of_other_footprints(kvr, a, b):
+    """The per-column copies of mesh_attn_step_host follow I^KV: contiguous footprints (no rotation), a mesh with
+    a > b, one Q group only (b = 1: the first wave is also the last group), and a = 1 (no columns: whole K, V, dK, dV).
+    Staging and host outputs start as NaN, so a partition that was not copied, or copied before it was final, shows."""
+    from paper_2512_20968_b200 import Buffers
+
+    w = replace(W.scaled_down(W.C4, 256, heads_q=4), a=a, b=b, seq_total=a * b * 256, heads_kv=2, kvr=kvr)
+    inp = W.make_inputs(w, "cuda")
+    plan, ref = run_fwd_bwd(w, inp)
+    host_in = {k: v.cpu().pin_memory() for k, v in inp.items()}
+    buf = Buffers(plan, w, backward=True)
+    dev = {k: torch.empty_like(v) for k, v in inp.items()}
+    for t in dev.values():
+        t.view(torch.int16).fill_(0x7FC0)
+    for t in (buf.O, buf.lse, buf.dQ, buf.dK, buf.dV):
+        t.fill_(float("nan"))
+    out = {k: torch.full(t.shape, float("nan"), dtype=t.dtype).pin_memory() for k, t in
+           dict(O=buf.O, lse=buf.lse, dQ=buf.dQ, dK=buf.dK, dV=buf.dV).items()}
+    plan.step_host(Q_host=host_in["q"], K_host=host_in["k"], V_host=host_in["v"], dO_host=host_in["do"],
+                   O_host=out["O"], lse_host=out["lse"], dQ_host=out["dQ"], dK_host=out["dK"], dV_host=out["dV"],
+                   d_Q=dev["q"], d_K=dev["k"], d_V=dev["v"], d_dO=dev["do"], d_O=buf.O, d_lse=buf.lse, d_bwd_ws=buf.bwd_ws,
+                   d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV, d_partial_O=buf.partial_O, d_partial_lse=buf.partial_lse)
+    plan.health()
+    for k in ("q", "k", "v", "do"):
+        assert torch.equal(dev[k].view(torch.int16), inp[k].view(torch.int16)), k
+    assert torch.equal(out["O"], ref.O.cpu()) and torch.equal(out["lse"], ref.lse.cpu())
+    for name, t in (("dQ", ref.dQ), ("dK", ref.dK), ("dV", ref.dV)):
+        assert torch.isfinite(out[name]).all(), name
+        assert (out[name] - t.cpu()).abs().max().item() <= 1e-3, name
+        assert torch.equal(out[name], getattr(buf, name).cpu()), name        # what came down is what the device holds at the end
+
+
 @pytest.mark.parametrize("causal", [False, True])
 def test_head_dim_64(oracle, causal):
     """head_dim 64 (BASELINE.json configs[0]'s heads) through the backward: the head_dim-128 kernel on tiles whose upper
