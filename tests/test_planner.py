@@ -343,3 +343,24 @@ def test_kernel_variants_chosen_for_the_baseline_configs_at_full_size():
     assert fwd == {"C1": 0, "C2": 1, "C3": 0, "C4": 1, "C5": 1}, fwd
     bwd = {name: plan_for(w).query(B.Q_BWD_PAIRED) for name, w in W.CONFIGS.items() if name != "C1"}
     assert bwd == {"C2": 2, "C3": 1, "C4": 2, "C5": 2}, bwd
+
+
+def test_random_geometry_draws_make_valid_plans_and_reach_every_kernel_variant():
+    """The seeded draws of tests/test_gpu_random_geometries.py (host arithmetic only) are all accepted by the planner, agree with the
+    plan oracle's assignment matrix, and between them reach both forward kernels, the single-CTA and the exchanging backward,
+    head_dim 64, GQA, both causal layouts, both footprints, both orders with chunks, batch 2 and two USP lanes."""
+    from paper_2512_20968_b200 import plan_for
+    from tests.test_gpu_random_geometries import SEEDS, geometry
+
+    seen = set()
+    for seed in SEEDS:
+        w, overrides = geometry(seed)
+        plan = plan_for(w, **overrides)
+        assert np.array_equal(plan.am(), np.asarray(po.assignment_matrix(w.n, w.a, w.b, w.kvr))), seed
+        seen |= {("fwd_pair", plan.query(B.Q_FWD_PAIRED)), ("bwd_pair", plan.query(B.Q_BWD_PAIRED)), ("D", w.head_dim), ("gqa", w.heads_q > w.heads_kv),
+                 ("layout", w.seq_layout if w.causal else "nc"), ("kvr", w.kvr), ("order", w.order), ("chunks", w.k_q * w.k_kv > 1),
+                 ("batch", w.batch), ("lanes", overrides["usp_lanes"])}
+    want = {("fwd_pair", 0), ("fwd_pair", 1), ("bwd_pair", 0), ("bwd_pair", 2), ("D", 64), ("D", 128), ("gqa", True), ("gqa", False),
+            ("layout", "striped"), ("layout", "contiguous"), ("layout", "nc"), ("kvr", True), ("kvr", False), ("order", "greedy"),
+            ("order", "row_major"), ("chunks", True), ("batch", 2), ("lanes", 2)}
+    assert want <= seen, want - seen
