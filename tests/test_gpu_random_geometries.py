@@ -62,3 +62,38 @@ def test_random_geometry_against_oracle(oracle, seed):
     print(f"\nseed {seed}: {w.a}x{w.b} L={w.L} B={w.batch} Hq/Hkv={w.heads_q}/{w.heads_kv} D={w.head_dim} causal={w.causal} {w.seq_layout} "
           f"kvr={w.kvr} {w.order} k={w.k_q}x{w.k_kv} lanes={overrides['usp_lanes']}: O {fwd[0]:.2e} lse {fwd[2]:.2e} "
           + " ".join(f"{k}={v:.2e}" for k, v in errs.items()))
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", SEEDS[::2])
+def test_random_geometry_step_host(seed):
+    """mesh_attn_step_host on the same draws (its copies are cut by Q group and KV column when batch == 1, whole tensors
+    otherwise; USP lanes change which wave / group is first / last): NaN-filled staging and host outputs, result against the
+    device-pointer calls (forward bit-identical; gradients up to the order of the fp32 atomics)."""
+    from paper_2512_20968_b200 import Buffers
+    from tests.test_gpu_backward import run_fwd_bwd
+
+    w, overrides = geometry(seed)
+    inp = W.make_inputs(w, "cuda")
+    plan, ref = run_fwd_bwd(w, inp, **overrides)
+    host_in = {k: v.cpu().pin_memory() for k, v in inp.items()}
+    buf = Buffers(plan, w, backward=True)
+    dev = {k: torch.empty_like(v) for k, v in inp.items()}
+    for t in dev.values():
+        t.view(torch.int16).fill_(0x7FC0)
+    for t in (buf.O, buf.lse, buf.dQ, buf.dK, buf.dV):
+        t.fill_(float("nan"))
+    out = {k: torch.full(t.shape, float("nan"), dtype=t.dtype).pin_memory() for k, t in
+           dict(O=buf.O, lse=buf.lse, dQ=buf.dQ, dK=buf.dK, dV=buf.dV).items()}
+    plan.step_host(Q_host=host_in["q"], K_host=host_in["k"], V_host=host_in["v"], dO_host=host_in["do"],
+                   O_host=out["O"], lse_host=out["lse"], dQ_host=out["dQ"], dK_host=out["dK"], dV_host=out["dV"],
+                   d_Q=dev["q"], d_K=dev["k"], d_V=dev["v"], d_dO=dev["do"], d_O=buf.O, d_lse=buf.lse, d_bwd_ws=buf.bwd_ws,
+                   d_dQ=buf.dQ, d_dK=buf.dK, d_dV=buf.dV, d_partial_O=buf.partial_O, d_partial_lse=buf.partial_lse)
+    plan.health()
+    for k in ("q", "k", "v", "do"):
+        assert torch.equal(dev[k].view(torch.int16), inp[k].view(torch.int16)), k
+    assert torch.equal(out["O"], ref.O.cpu()) and torch.equal(out["lse"], ref.lse.cpu())
+    for name, t in (("dQ", ref.dQ), ("dK", ref.dK), ("dV", ref.dV)):
+        assert torch.isfinite(out[name]).all(), name
+        assert (out[name] - t.cpu()).abs().max().item() <= 1e-3, name          # the order of the fp32 atomics differs run to run
+        assert torch.equal(out[name], getattr(buf, name).cpu()), name
