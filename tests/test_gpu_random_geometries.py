@@ -97,3 +97,36 @@ def test_random_geometry_step_host(seed):
         assert torch.isfinite(out[name]).all(), name
         assert (out[name] - t.cpu()).abs().max().item() <= 1e-3, name          # the order of the fp32 atomics differs run to run
         assert torch.equal(out[name], getattr(buf, name).cpu()), name
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", SEEDS[1::2])
+def test_random_geometry_goo_executors(seed):
+    """mesh_attn_forward_goo / mesh_attn_backward_goo (the step lists executed task by task, copies standing in for the
+    collectives) on the other half of the draws, Q group by Q group of every lane, against the fused calls: O at the level of the
+    bf16 P operand (each task rounds against its own running max), lse to 1e-4, gradients up to the order of the fp32 atomics."""
+    from paper_2512_20968_b200 import binding as B
+    from tests.test_gpu_backward import run_fwd_bwd
+
+    w, overrides = geometry(seed)
+    inp = W.make_inputs(w, "cuda")
+    plan, ref = run_fwd_bwd(w, inp, **overrides)
+    f32 = dict(dtype=torch.float32, device="cuda")
+    part_O = torch.full((plan.query(B.Q_GOO_PARTIAL_O_BYTES) * w.a // 4,), float("nan"), **f32)
+    part_lse = torch.full((plan.query(B.Q_GOO_PARTIAL_LSE_BYTES) * w.a // 4,), float("nan"), **f32)
+    comm_ws = torch.empty(1 << 20, dtype=torch.uint8, device="cuda")
+    O, lse = torch.full_like(ref.O, float("nan")), torch.full_like(ref.lse, float("nan"))
+    dQ, dK, dV = torch.zeros_like(ref.dQ), torch.zeros_like(ref.dK), torch.zeros_like(ref.dV)
+    for r in range(w.b * overrides["usp_lanes"]):
+        plan.forward_goo(r, inp["q"], inp["k"], inp["v"], O, lse, part_O, part_lse, comm_ws=comm_ws, comm_repeat=seed % 3, overlap=bool(seed % 4))
+        plan.backward_goo(r, inp["q"], inp["k"], inp["v"], inp["do"], ref.bwd_ws, dQ, dK, dV, comm_ws=comm_ws, comm_repeat=seed % 3, overlap=bool(seed % 4))
+    torch.cuda.synchronize()
+    plan.health()
+    assert (O - ref.O).abs().max().item() <= 3e-3
+    fin = torch.isfinite(ref.lse)
+    assert torch.equal(torch.isfinite(lse), fin) and (lse[fin] - ref.lse[fin]).abs().max().item() <= 1e-4
+    for name, got, want in (("dQ", dQ, ref.dQ), ("dK", dK, ref.dK), ("dV", dV, ref.dV)):
+        assert torch.isfinite(got).all(), name
+        err = (got - want).abs().max().item()
+        # the fused backward's pair exchange rounds half of the dQ partial sums to bf16; the executor's single-CTA launches do not
+        assert err <= (1e-2 if name == "dQ" else 1e-3) * max(1.0, want.abs().max().item()), f"{name}: {err:.3e} vs mesh_attn_backward"
