@@ -130,3 +130,34 @@ def test_random_geometry_goo_executors(seed):
         err = (got - want).abs().max().item()
         # the fused backward's pair exchange rounds half of the dQ partial sums to bf16; the executor's single-CTA launches do not
         assert err <= (1e-2 if name == "dQ" else 1e-3) * max(1.0, want.abs().max().item()), f"{name}: {err:.3e} vs mesh_attn_backward"
+
+
+def _rank_draws():
+    out = []
+    for seed in SEEDS:
+        w, overrides = geometry(seed)
+        if w.kvr and w.batch == 1 and overrides["usp_lanes"] == 1:      # the reduce-scatter of dK, dV needs g in I_g^KV (rotation)
+            out.append(seed)
+    return out
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", _rank_draws())
+def test_random_geometry_rank_calls(seed):
+    """The per-rank calls (one GPU's share of Alg.2 / Alg.3 on its gathered partitions, the n ranks played one after the other,
+    reduce-scatters through the peer-memory reducers) on the draws with KV rotation: forward bit-identical to the simulated-GPU
+    path, gradients up to the order of the fp32 atomics (and the pair exchange's bf16 halves of dQ, which the per-rank backward,
+    pairing inside its own lists, may group differently)."""
+    from tests.test_gpu_backward import run_fwd_bwd
+    from tests.test_gpu_rank_calls import play_ranks
+
+    w, _ = geometry(seed)
+    inp = W.make_inputs(w, "cuda")
+    plan, ref = run_fwd_bwd(w, inp)
+    O, lse, grads = play_ranks(plan, w, inp)
+    plan.health()
+    assert torch.equal(O, ref.O) and torch.equal(lse, ref.lse)
+    for name, got, want in zip(("dQ", "dK", "dV"), grads, (ref.dQ, ref.dK, ref.dV)):
+        assert torch.isfinite(got).all(), name
+        err = (got - want).abs().max().item()
+        assert err <= (1e-2 if name == "dQ" else 1e-3) * max(1.0, want.abs().max().item()), f"{name}: {err:.3e} vs the simulated-GPU path"
