@@ -161,3 +161,30 @@ def test_random_geometry_rank_calls(seed):
         assert torch.isfinite(got).all(), name
         err = (got - want).abs().max().item()
         assert err <= (1e-2 if name == "dQ" else 1e-3) * max(1.0, want.abs().max().item()), f"{name}: {err:.3e} vs the simulated-GPU path"
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", SEEDS[::3])
+def test_random_geometry_bf16_outputs_and_static_forward(seed):
+    """Plan desc field out_dtype = 1 and mesh_attn_forward_static on the draws: O (bf16) is the fp32 path's O rounded once, lse is
+    identical, dV within bf16 resolution of the fp32 path's, dQ / dK within the error the rounded O leaves in delta
+    (tests/test_gpu_out_dtype.py); the no-allocation forward returns the same bits wherever the plan fits its 32 MiB array."""
+    from tests.test_gpu_backward import TOL_GRAD, run_fwd_bwd
+
+    w, overrides = geometry(seed)
+    inp = W.make_inputs(w, "cuda")
+    _, b32 = run_fwd_bwd(w, inp, **overrides)
+    p16, b16 = run_fwd_bwd(w, inp, out_dtype=1, **overrides)
+    p16.health()
+    assert torch.equal(b16.lse, b32.lse) and torch.equal(b16.O, b32.O.to(torch.bfloat16))
+    for name, abs_tol in (("dQ", 2 * TOL_GRAD), ("dK", 2 * TOL_GRAD), ("dV", 0.25 * TOL_GRAD)):
+        got, ref = getattr(b16, name).double(), getattr(b32, name).double()
+        assert torch.isfinite(got).all(), name
+        assert ((got - ref).abs() <= abs_tol + 2.0 ** -8 * ref.abs()).all(), name
+    need, cap = p16.forward_static_limits()
+    if need <= cap:
+        O_s, lse_s = torch.full_like(b16.O, float("nan")), torch.full_like(b16.lse, float("nan"))
+        p16.forward_static(inp["q"], inp["k"], inp["v"], O_s, lse_s)
+        torch.cuda.synchronize()
+        assert torch.equal(O_s, b16.O) and torch.equal(lse_s, b16.lse)
+    print(f"\nseed {seed}: forward_static {'run' if need <= cap else 'refused'} ({need} of {cap} bytes)")
