@@ -1,11 +1,12 @@
 """GPU parity on RANDOM plan geometries: seeded draws over mesh shape (a x b, also a != b and a or b = 1), partition length
 (1..5 key blocks, so ragged against the 256-row forward items and the backward's pairing), heads / GQA group, head_dim,
-mask and sequence layout, KV rotation, tile order with k_Q x k_KV chunks, batch and Mesh-USP lanes -- the combinations the
+outlier data with the hi+lo operand mode, mask and sequence layout, KV rotation, tile order with k_Q x k_KV chunks, batch and Mesh-USP lanes -- the combinations the
 named BASELINE.json shapes do not reach.  Every draw runs mesh_attn_forward + mesh_attn_backward through the C ABI and is
 compared with the fp64 oracle (forward: sampled rows of every partition incl. its first and last row, all heads; backward:
 sampled query rows and keys, plus the three gradient invariants), tolerances of BASELINE.json.  The draw list is fixed by
 the seeds below; `geometry(seed)` is also exercised on the CPU (tests/test_planner.py) so that an invalid draw shows there."""
 import os
+from dataclasses import replace
 
 import numpy as np
 import pytest
@@ -36,6 +37,8 @@ def geometry(seed):
                    seq_total=a * b * L, heads_q=heads_kv * group, heads_kv=heads_kv, head_dim=int(rng.choice([64, 128, 128])),
                    kvr=bool(rng.random() < 0.6), order="greedy" if rng.random() < 0.5 else "row_major", k_q=k_q, k_kv=k_kv,
                    seq_layout="striped" if causal and rng.random() < 0.6 else "contiguous")
+    if w.head_dim == 128 and rng.random() < 0.25:                         # C3's data: 4 Q / K channels x 8, run with hi+lo operands (precision 1)
+        w = replace(w, outlier=True)
     return w, dict(usp_lanes=lanes)
 
 
@@ -95,7 +98,7 @@ def test_random_geometry_step_host(seed):
     assert torch.equal(out["O"], ref.O.cpu()) and torch.equal(out["lse"], ref.lse.cpu())
     for name, t in (("dQ", ref.dQ), ("dK", ref.dK), ("dV", ref.dV)):
         assert torch.isfinite(out[name]).all(), name
-        assert (out[name] - t.cpu()).abs().max().item() <= 1e-3, name          # the order of the fp32 atomics differs run to run
+        assert (out[name] - t.cpu()).abs().max().item() <= 1e-3 * max(1.0, t.abs().max().item()), name     # the order of the fp32 atomics differs run to run
         assert torch.equal(out[name], getattr(buf, name).cpu()), name
 
 
@@ -180,6 +183,8 @@ def test_random_geometry_bf16_outputs_and_static_forward(seed):
     for name, abs_tol in (("dQ", 2 * TOL_GRAD), ("dK", 2 * TOL_GRAD), ("dV", 0.25 * TOL_GRAD)):
         got, ref = getattr(b16, name).double(), getattr(b32, name).double()
         assert torch.isfinite(got).all(), name
+        if w.outlier and name != "dV":       # |K|, |Q| x 8 multiply what the rounded O leaves in delta: outside the gradient bar by design
+            continue                         # (out_dtype: outlier data keeps fp32 outputs)
         assert ((got - ref).abs() <= abs_tol + 2.0 ** -8 * ref.abs()).all(), name
     need, cap = p16.forward_static_limits()
     if need <= cap:
