@@ -1,7 +1,7 @@
 """GPU parity on RANDOM plan geometries: seeded draws over mesh shape (a x b, also a != b and a or b = 1), partition length
 (1..5 key blocks, so ragged against the 256-row forward items and the backward's pairing), heads / GQA group, head_dim,
-outlier data with the hi+lo operand mode, mask and sequence layout, KV rotation, tile order with k_Q x k_KV chunks, batch and Mesh-USP lanes -- the combinations the
-named BASELINE.json shapes do not reach.  Every draw runs mesh_attn_forward + mesh_attn_backward through the C ABI and is
+outlier data with the hi+lo operand mode, mask and sequence layout, KV rotation, tile order with k_Q x k_KV chunks, batch, Mesh-USP lanes and the kernel-variant fields
+(bwd_piece_blocks, bwd_pairing, fwd_pairing) -- the combinations the named BASELINE.json shapes do not reach.  Every draw runs mesh_attn_forward + mesh_attn_backward through the C ABI and is
 compared with the fp64 oracle (forward: sampled rows of every partition incl. its first and last row, all heads; backward:
 sampled query rows and keys, plus the three gradient invariants), tolerances of BASELINE.json.  The draw list is fixed by
 the seeds below; `geometry(seed)` is also exercised on the CPU (tests/test_planner.py) so that an invalid draw shows there."""
@@ -39,7 +39,10 @@ def geometry(seed):
                    seq_layout="striped" if causal and rng.random() < 0.6 else "contiguous")
     if w.head_dim == 128 and rng.random() < 0.25:                         # C3's data: 4 Q / K channels x 8, run with hi+lo operands (precision 1)
         w = replace(w, outlier=True)
-    return w, dict(usp_lanes=lanes)
+    # the kernel-variant fields of the plan desc: sweep pieces of the backward, the three backward kernels, the two forward kernels
+    variants = dict(bwd_piece_blocks=int(rng.choice([0, 0, 1, 2, 3, 7])), bwd_pairing=int(rng.choice([0, 0, 0, 1, 2])),
+                    fwd_pairing=int(rng.choice([0, 0, 1])))
+    return w, dict(usp_lanes=lanes, **variants)
 
 
 @pytest.mark.gpu
