@@ -196,3 +196,44 @@ def test_random_geometry_bf16_outputs_and_static_forward(seed):
         torch.cuda.synchronize()
         assert torch.equal(O_s, b16.O) and torch.equal(lse_s, b16.lse)
     print(f"\nseed {seed}: forward_static {'run' if need <= cap else 'refused'} ({need} of {cap} bytes)")
+
+
+@pytest.mark.gpu
+@pytest.mark.parametrize("seed", SEEDS[::4])
+def test_random_geometry_bhnd_layout(seed):
+    """tensor_layout = 1 ([B,H,N,D] tensors: other TMA maps, other strides in merge / preprocess / the dQ reduce boxes) on the draws:
+    forward bit-identical to the [B,N,H,D] plan's, gradients up to the order of the fp32 atomics; mesh_attn_step_host in this layout
+    (whole-tensor copies) returns the same tensors."""
+    from paper_2512_20968_b200 import Buffers, plan_for
+    from tests.test_gpu_backward import run_fwd_bwd
+
+    w, overrides = geometry(seed)
+    inp = W.make_inputs(w, "cuda")
+    _, ref = run_fwd_bwd(w, inp, **overrides)
+    tr = lambda t: t.permute(0, 2, 1, 3).contiguous()                      # noqa: E731
+    inp_t = {k: tr(v) for k, v in inp.items()}
+    plan = plan_for(w, tensor_layout=1, **overrides)
+    buf = Buffers(plan, w, backward=True)
+    O, dQ, dK, dV = (torch.full_like(tr(t), float("nan")) for t in (buf.O, buf.dQ, buf.dK, buf.dV))
+    plan.forward(inp_t["q"], inp_t["k"], inp_t["v"], O, buf.lse, buf.partial_O, buf.partial_lse)
+    plan.backward(inp_t["q"], inp_t["k"], inp_t["v"], O, inp_t["do"], buf.lse, buf.bwd_ws, dQ, dK, dV)
+    torch.cuda.synchronize()
+    plan.health()
+    assert torch.equal(tr(O), ref.O) and torch.equal(buf.lse, ref.lse)
+    for name, got, want in (("dQ", dQ, ref.dQ), ("dK", dK, ref.dK), ("dV", dV, ref.dV)):
+        assert (tr(got) - want).abs().max().item() <= 1e-3 * max(1.0, want.abs().max().item()), name
+    host_in = {k: v.cpu().pin_memory() for k, v in inp_t.items()}
+    dev = {k: torch.full_like(v, float("nan")) for k, v in inp_t.items()}
+    outs = dict(O=O, lse=buf.lse, dQ=dQ, dK=dK, dV=dV)
+    out = {k: torch.full(t.shape, float("nan"), dtype=t.dtype).pin_memory() for k, t in outs.items()}
+    dbuf = {k: torch.full_like(t, float("nan")) for k, t in outs.items()}
+    plan.step_host(Q_host=host_in["q"], K_host=host_in["k"], V_host=host_in["v"], dO_host=host_in["do"],
+                   O_host=out["O"], lse_host=out["lse"], dQ_host=out["dQ"], dK_host=out["dK"], dV_host=out["dV"],
+                   d_Q=dev["q"], d_K=dev["k"], d_V=dev["v"], d_dO=dev["do"], d_O=dbuf["O"], d_lse=dbuf["lse"], d_bwd_ws=buf.bwd_ws,
+                   d_dQ=dbuf["dQ"], d_dK=dbuf["dK"], d_dV=dbuf["dV"], d_partial_O=buf.partial_O, d_partial_lse=buf.partial_lse)
+    plan.health()
+    assert torch.equal(out["O"], O.cpu()) and torch.equal(out["lse"], buf.lse.cpu())
+    for name in ("dQ", "dK", "dV"):
+        want = outs[name].cpu()
+        assert torch.isfinite(out[name]).all(), name
+        assert (out[name] - want).abs().max().item() <= 1e-3 * max(1.0, want.abs().max().item()), name
