@@ -41,7 +41,7 @@ def geometry(seed):
         w = replace(w, outlier=True)
     # the kernel-variant fields of the plan desc: sweep pieces of the backward, the three backward kernels, the two forward kernels
     variants = dict(bwd_piece_blocks=int(rng.choice([0, 0, 1, 2, 3, 7])), bwd_pairing=int(rng.choice([0, 0, 0, 1, 2])),
-                    fwd_pairing=int(rng.choice([0, 0, 1])))
+                    fwd_pairing=int(rng.choice([0, 0, 1])), partial_mode=int(rng.choice([0, 0, 0, 1])))    # 1: per-pair partials
     return w, dict(usp_lanes=lanes, **variants)
 
 
@@ -128,7 +128,10 @@ def test_random_geometry_goo_executors(seed):
         plan.backward_goo(r, inp["q"], inp["k"], inp["v"], inp["do"], ref.bwd_ws, dQ, dK, dV, comm_ws=comm_ws, comm_repeat=seed % 3, overlap=bool(seed % 4))
     torch.cuda.synchronize()
     plan.health()
-    assert (O - ref.O).abs().max().item() <= 3e-3
+    # two evaluations that round P to bf16 against different running maxima (per task / per pair / fused): each is off by at most
+    # 2^-9 sum_t p_t |v_t| <= 2^-9 max|V| per element (the rows that come close see two or three keys), so they are at most twice
+    # that apart; each is within 1e-2 of the oracle (test_random_geometry_against_oracle).  Seen over 300 draws: up to 8.6e-3.
+    assert (O - ref.O).abs().max().item() <= 2 * 2.0 ** -9 * inp["v"].float().abs().max().item()
     fin = torch.isfinite(ref.lse)
     assert torch.equal(torch.isfinite(lse), fin) and (lse[fin] - ref.lse[fin]).abs().max().item() <= 1e-4
     for name, got, want in (("dQ", dQ, ref.dQ), ("dK", dK, ref.dK), ("dV", dV, ref.dV)):

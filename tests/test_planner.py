@@ -359,8 +359,9 @@ def test_random_geometry_draws_make_valid_plans_and_reach_every_kernel_variant()
         assert np.array_equal(plan.am(), np.asarray(po.assignment_matrix(w.n, w.a, w.b, w.kvr))), seed
         seen |= {("fwd_pair", plan.query(B.Q_FWD_PAIRED)), ("bwd_pair", plan.query(B.Q_BWD_PAIRED)), ("D", w.head_dim), ("gqa", w.heads_q > w.heads_kv),
                  ("layout", w.seq_layout if w.causal else "nc"), ("kvr", w.kvr), ("order", w.order), ("chunks", w.k_q * w.k_kv > 1),
-                 ("batch", w.batch), ("lanes", overrides["usp_lanes"]), ("outlier", w.outlier), ("pieces", overrides["bwd_piece_blocks"] > 0)}
-    want = {("fwd_pair", 0), ("fwd_pair", 1), ("bwd_pair", 0), ("bwd_pair", 1), ("bwd_pair", 2), ("outlier", True), ("pieces", True), ("D", 64), ("D", 128), ("gqa", True), ("gqa", False),
+                 ("batch", w.batch), ("lanes", overrides["usp_lanes"]), ("outlier", w.outlier), ("pieces", overrides["bwd_piece_blocks"] > 0),
+                 ("per_pair", overrides["partial_mode"])}
+    want = {("fwd_pair", 0), ("fwd_pair", 1), ("bwd_pair", 0), ("bwd_pair", 1), ("bwd_pair", 2), ("outlier", True), ("pieces", True), ("per_pair", 1), ("D", 64), ("D", 128), ("gqa", True), ("gqa", False),
             ("layout", "striped"), ("layout", "contiguous"), ("layout", "nc"), ("kvr", True), ("kvr", False), ("order", "greedy"),
             ("order", "row_major"), ("chunks", True), ("batch", 2), ("lanes", 2)}
     assert want <= seen, want - seen
