@@ -623,10 +623,14 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
             PT_MARK(1);
             if (kAblate & 1) { tc_fence_before(); mbar_arrive(ds_full); return; }
             uint32_t ra[16], rb[16];             // 16-column chunks: chunk c+1 is in flight while chunk c is processed
+            // delta of the NEXT 8 columns is loaded while the current 8 are computed: the shared memory is busy with the MMAs' operand
+            // reads and a broadcast ld.shared takes ~80 clocks here (ncu: 12 % of a compute warp's samples sat at the first use of it)
+            float4 da_next = dl4[0], db_next = dl4[1];
             auto ds_chunk = [&](int c16, const uint32_t (&r)[16]) {
 #pragma unroll
                 for (int k = 0; k < 2; ++k) {                              // 8 columns = one 16-byte chunk of the row
-                    const float4 da = dl4[c16 * 4 + k * 2], db = dl4[c16 * 4 + k * 2 + 1];
+                    const float4 da = da_next, db = db_next;
+                    if (c16 * 2 + k < 7) { da_next = dl4[c16 * 4 + k * 2 + 2]; db_next = dl4[c16 * 4 + k * 2 + 3]; }
                     const int c = c16 * 16 + k * 8;
                     float d0, d1, d2, d3, d4, d5, d6, d7;        // dS = P o (dP - delta), two elements per instruction
                     unpack2(mul2(pack2(pr[c + 0], pr[c + 1]), add2(pack2(__uint_as_float(r[k * 8 + 0]), __uint_as_float(r[k * 8 + 1])), pack2(-da.x, -da.y))), d0, d1);
