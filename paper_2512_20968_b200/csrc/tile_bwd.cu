@@ -422,7 +422,9 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 mbar_wait(do_full, do_ph);
                 do_ph ^= 1;
                 tc_fence_after();
-#pragma unroll
+                // the k-loops of the five MMAs are unrolled by 2, not 8: the issuer's warp sat at instruction fetch in 21 % of its ncu samples
+                // (four roles share an SM sub-partition's instruction cache); measured 8 / 4 / 2 / 1: tile_bwd C2 1031 / 1026 / 1039 / 1015 TFLOP/s
+#pragma unroll 2
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t o = (kk / 4) * (kBlock * 128) + (kk % 4) * 32;
                     umma_ss(tmem + Cfg::kColDP, umma_desc(aV + o, 16, 1024), umma_desc(adO + o, 16, 1024), idesc_kk, kk > 0);
@@ -430,7 +432,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                 umma_commit(dp_full);
             };
             auto mma_kmajor = [&](uint32_t dcol, uint32_t a, uint32_t b) {          // D = A B^T, both K-major over head_dim
-#pragma unroll
+#pragma unroll 2
                 for (int kk = 0; kk < D / 16; ++kk) {
                     const uint32_t o = (kk / 4) * (kBlock * 128) + (kk % 4) * 32;
                     umma_ss(tmem + dcol, umma_desc(a + o, 16, 1024), umma_desc(b + o, 16, 1024), idesc_kk, kk > 0);
@@ -469,7 +471,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     PT_MARK(1);
 #pragma unroll
                     for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
+#pragma unroll 2
                         for (int kk = 0; kk < kBlock / 16; ++kk)
                             umma_ts(tmem + Cfg::kColDV, tmem + Cfg::kColS + (kk >> 2) * 64 + x * 32 + (kk & 3) * 8,
                                     umma_desc(adO + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
@@ -491,7 +493,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     auto issue_dq = [&]() {
 #pragma unroll
                         for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
+#pragma unroll 2
                             for (int kk = 0; kk < kBlock / 16; ++kk)
                                 umma_ss(tmem + Cfg::kColDP, umma_desc(aK + kk * 2048, kBlock * 128, 1024),
                                         umma_desc(aDs + x * Cfg::kDsBytes + kk * 2048, kBlock * 128, 1024), idesc_nn, (kk > 0 || x > 0) ? 1u : 0u);
@@ -500,7 +502,7 @@ tile_bwd_kernel(const __grid_constant__ CUtensorMap tmQ, const __grid_constant__
                     auto issue_dk = [&]() {
 #pragma unroll
                         for (int x = 0; x < Cfg::kNumDs; ++x)
-#pragma unroll
+#pragma unroll 2
                             for (int kk = 0; kk < kBlock / 16; ++kk)
                                 umma_ss(tmem + Cfg::kColDK, umma_desc(aDs + x * Cfg::kDsBytes + (kk / 4) * (kBlock * 128) + (kk % 4) * 32, 16, 1024),
                                         umma_desc(aQ + kk * 2048, kBlock * 128, 1024), idesc_tn, (i > 0 || kk > 0 || x > 0) ? 1u : 0u);
