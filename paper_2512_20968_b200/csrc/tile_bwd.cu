@@ -186,11 +186,12 @@ __device__ __forceinline__ void red_add_v4(float* addr, float a, float b, float 
 {
     asm volatile("red.global.add.v4.f32 [%0], {%1, %2, %3, %4};" ::"l"(addr), "f"(a), "f"(b), "f"(c), "f"(d) : "memory");
 }
-// TMA tensor reduction: global[tile at (c0..c3)] += smem tile (fp32), tracked by the thread's bulk async-group
+// TMA tensor reduction: global[tile at (c0..c3)] += smem tile (fp32), tracked by the thread's bulk async-group.  The dQ lines are hit again by
+// every key block that sweeps the same query rows: evict_last keeps them in L2 (+0.3 % on C2 / C4, +0.15 % on C5, back to back)
 __device__ __forceinline__ void tma_reduce_add_4d(const CUtensorMap* m, const void* smem_src, int c0, int c1, int c2, int c3)
 {
-    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group [%0, {%2, %3, %4, %5}], [%1];"
-                 ::"l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3) : "memory");
+    asm volatile("cp.reduce.async.bulk.tensor.4d.global.shared::cta.add.tile.bulk_group.L2::cache_hint [%0, {%2, %3, %4, %5}], [%1], %6;"
+                 ::"l"(reinterpret_cast<uint64_t>(m)), "r"(smem_u32(smem_src)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(kEvictLast) : "memory");
 }
 // TMEM accumulator [128 lanes x D columns] -> x scale -> atomic add into a global row of D floats
 // (item epilogue only: once per 128-key block)
